@@ -1,0 +1,307 @@
+"""ctypes front end of the CPU oracle (oracle/refdef_oracle.c) -- TEST INFRASTRUCTURE.
+
+The arithmetic lives in the C file, written from PAPER.md step by step; this module only
+builds it (gcc -O2), marshals numpy arrays, and provides `reference_eigs`, the plain
+definition of what `build_reference` must produce: the k lowest eigenpairs of the full
+H = M + sigma K^T M^{-1} K (BASELINE.json north_star; nearest paper text Alg. 2 step 2,
+PAPER.md:382), computed with a library eigensolver on the assembled matrix.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import List, Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "refdef_oracle.c")
+_LIB = os.path.join(_HERE, "librefdef_oracle.so")
+
+JACOBI_CG, REFDEF, ZEROEXT = 0, 1, 2
+INIT_PAPER, INIT_ALL_ACTIVE, INIT_ALL_INACTIVE, INIT_GIVEN = 0, 1, 2, 3
+STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -5: "enotspd", -6: "ecap", -7: "esteps", -8: "ecycle",
+                -9: "eresid"}
+
+
+def build_oracle(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain -O2, no fast-math, single thread)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+class _StepReport(C.Structure):
+    _fields_ = [("n_inactive", C.c_int32), ("cg_iters", C.c_int32), ("rank_used", C.c_int32),
+                ("coarse_fallback", C.c_int32), ("replacements", C.c_int32), ("status", C.c_int32),
+                ("rel_resid_verified", C.c_double), ("cond_E", C.c_double), ("margin", C.c_double),
+                ("active_hash", C.c_uint64)]
+
+
+class _QueryReport(C.Structure):
+    _fields_ = [("n_steps", C.c_int32), ("status", C.c_int32), ("kkt", C.c_double * 5)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("eps", C.c_double), ("eps_c", C.c_double), ("cg_cap", C.c_int32), ("pdas_cap", C.c_int32),
+                ("replace_period", C.c_int32), ("jacobi", C.c_int32), ("c_is_diag", C.c_int32),
+                ("init", C.c_int32)]
+
+
+class _SolveReport(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("rank_used", C.c_int32), ("coarse_fallback", C.c_int32),
+                ("replacements", C.c_int32), ("status", C.c_int32), ("rel_resid_verified", C.c_double),
+                ("cond_E", C.c_double)]
+
+
+@dataclass
+class OracleOptions:
+    eps: float = 1e-8          # Verify tolerance (reading A11; the paper's own is 1e-10)
+    eps_c: float = 1e-8        # recurrence trigger
+    cg_cap: int = 500000       # reading A12
+    pdas_cap: int = 100
+    replace_period: int = 0    # reading A8
+    jacobi: int = 1
+    c_is_diag: int = 0         # reading A3: c = 1 (configs) or d_i (eq. (8))
+    init: int = INIT_PAPER
+
+    def c_struct(self) -> _Options:
+        return _Options(self.eps, self.eps_c, self.cg_cap, self.pdas_cap, self.replace_period, self.jacobi,
+                        self.c_is_diag, self.init)
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _load():
+    lib = C.CDLL(build_oracle())
+    lib.orc_create.restype = C.c_void_p
+    lib.orc_create.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
+    lib.orc_destroy.argtypes = [C.c_void_p]
+    lib.orc_reset_sequence.argtypes = [C.c_void_p]
+    for f in ("orc_apply_K", "orc_apply_KT", "orc_apply_H"):
+        getattr(lib, f).argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.orc_diag_H.argtypes = [C.c_void_p, C.c_void_p]
+    lib.orc_apply_B.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.orc_coarse_build.restype = C.c_void_p
+    lib.orc_coarse_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int]
+    lib.orc_coarse_free.argtypes = [C.c_void_p]
+    lib.orc_coarse_Q.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.orc_coarse_P.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.orc_coarse_rank.argtypes = [C.c_void_p]
+    lib.orc_coarse_fallback.argtypes = [C.c_void_p]
+    lib.orc_coarse_cond.restype = C.c_double
+    lib.orc_coarse_cond.argtypes = [C.c_void_p]
+    lib.orc_coarse_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.orc_alg1.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                             C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(_SolveReport)]
+    lib.orc_solve_query.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                    C.POINTER(_Options), C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.POINTER(_StepReport), C.c_void_p, C.POINTER(_QueryReport)]
+    lib.orc_restrict.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]
+    lib.orc_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    return lib
+
+
+_lib = None
+
+
+def _get_lib():
+    global _lib
+    if _lib is None:
+        _lib = _load()
+    return _lib
+
+
+class CoarseSpace:
+    """Handle on the oracle's coarse space of one inactive system (eq. (18))."""
+
+    def __init__(self, orc: "Oracle", idx: np.ndarray, Zt: np.ndarray):
+        self._lib = _get_lib()
+        self._orc = orc
+        self.idx = np.ascontiguousarray(idx, dtype=np.int64)
+        self.n = len(self.idx)
+        Zt = np.asfortranarray(Zt, dtype=np.float64)
+        k = Zt.shape[1] if Zt.ndim == 2 else 0
+        self._h = self._lib.orc_coarse_build(orc._h, self.idx.ctypes.data, self.n, Zt.ctypes.data, k)
+        self.rank = self._lib.orc_coarse_rank(self._h)
+        self.fallback = self._lib.orc_coarse_fallback(self._h)
+        self.cond_E = self._lib.orc_coarse_cond(self._h)
+
+    def Q(self, v):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        out = np.empty(self.n)
+        self._lib.orc_coarse_Q(self._h, v.ctypes.data, out.ctypes.data)
+        return out
+
+    def P(self, v):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        out = np.empty(self.n)
+        self._lib.orc_coarse_P(self._h, v.ctypes.data, out.ctypes.data)
+        return out
+
+    def factors(self):
+        Z = np.empty((self.n, self.rank), order="F")
+        BZ = np.empty((self.n, self.rank), order="F")
+        E = np.empty((self.rank, self.rank), order="F")
+        if self.rank:
+            self._lib.orc_coarse_get(self._h, Z.ctypes.data, BZ.ctypes.data, E.ctypes.data)
+        return Z, BZ, E
+
+    def __del__(self):
+        try:
+            self._lib.orc_coarse_free(self._h)
+        except Exception:
+            pass
+
+
+class Oracle:
+    """One operator = one context (host arrays).  sigma = alpha (reading A1)."""
+
+    def __init__(self, rowptr, colidx, val, m, sigma):
+        self._lib = _get_lib()
+        self.N = len(m)
+        self._rowptr = np.ascontiguousarray(rowptr, dtype=np.int64)
+        self._colidx = np.ascontiguousarray(colidx, dtype=np.int32)
+        self._val = np.ascontiguousarray(val, dtype=np.float64)
+        self._m = np.ascontiguousarray(m, dtype=np.float64)
+        self.sigma = float(sigma)
+        self._h = self._lib.orc_create(self.N, self._rowptr.ctypes.data, self._colidx.ctypes.data,
+                                       self._val.ctypes.data, self._m.ctypes.data, self.sigma)
+        if not self._h:
+            raise ValueError("orc_create failed (N <= 0 or m_i <= 0)")
+
+    @classmethod
+    def from_workload(cls, w):
+        return cls(w.rowptr, w.colidx, w.val, w.m, w.alpha)
+
+    def __del__(self):
+        try:
+            if self._h:
+                self._lib.orc_destroy(self._h)
+        except Exception:
+            pass
+
+    def reset_sequence(self):
+        self._lib.orc_reset_sequence(self._h)
+
+    def _apply(self, name, v):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        out = np.empty(self.N)
+        getattr(self._lib, name)(self._h, v.ctypes.data, out.ctypes.data)
+        return out
+
+    def apply_K(self, v):
+        return self._apply("orc_apply_K", v)
+
+    def apply_KT(self, v):
+        return self._apply("orc_apply_KT", v)
+
+    def apply_H(self, v):
+        return self._apply("orc_apply_H", v)
+
+    def diag_H(self):
+        d = np.empty(self.N)
+        self._lib.orc_diag_H(self._h, d.ctypes.data)
+        return d
+
+    def apply_B(self, idx, x):
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        out = np.empty(len(idx))
+        self._lib.orc_apply_B(self._h, idx.ctypes.data, len(idx), x.ctypes.data, out.ctypes.data)
+        return out
+
+    def restrict(self, method, W, idx):
+        """Restricted candidate basis Z~ (O3a) of the inactive set idx; updates the zero-extension history."""
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        W = np.asfortranarray(W, dtype=np.float64)
+        k = W.shape[1]
+        Zt = np.zeros((len(idx), k), order="F")
+        self._lib.orc_restrict(self._h, method, W.ctypes.data, k, idx.ctypes.data, len(idx), Zt.ctypes.data)
+        return Zt
+
+    def coarse(self, idx, Zt) -> CoarseSpace:
+        return CoarseSpace(self, idx, Zt)
+
+    def alg1(self, idx, b, x0, Zt=None, eps=1e-8, eps_c=None, cap=500000, replace_period=0, jacobi=1):
+        """Algorithm 1 on the inactive system (idx ascending).  Returns (x, report dict)."""
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        x = np.array(x0, dtype=np.float64, copy=True)
+        k = 0
+        zp = None
+        if Zt is not None and Zt.size:
+            Zt = np.asfortranarray(Zt, dtype=np.float64)
+            k = Zt.shape[1]
+            zp = Zt.ctypes.data
+        rep = _SolveReport()
+        self._lib.orc_alg1(self._h, idx.ctypes.data, len(idx), b.ctypes.data, x.ctypes.data, zp, k, eps,
+                           eps if eps_c is None else eps_c, cap, replace_period, jacobi, C.byref(rep))
+        return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+
+    def solve_query(self, method, y_d, psi, W=None, opt: Optional[OracleOptions] = None, J0=None,
+                    want_sets: bool = True):
+        """PDAS query (O2).  W: N x k (any order; copied column-major).  Returns a dict."""
+        opt = opt or OracleOptions()
+        N = self.N
+        y_d = np.ascontiguousarray(y_d, dtype=np.float64)
+        psi = np.ascontiguousarray(psi, dtype=np.float64)
+        k = 0
+        wp = None
+        if W is not None and method != JACOBI_CG:
+            W = np.asfortranarray(W, dtype=np.float64)
+            k = W.shape[1]
+            wp = W.ctypes.data
+        j0p = None
+        if J0 is not None:
+            J0 = np.ascontiguousarray(J0, dtype=np.uint8)
+            j0p = J0.ctypes.data
+        y = np.empty(N)
+        u = np.empty(N)
+        lam = np.empty(N)
+        steps = (_StepReport * opt.pdas_cap)()
+        nbytes = (N + 7) // 8
+        Jb = np.zeros((opt.pdas_cap, nbytes), dtype=np.uint8) if want_sets else None
+        rep = _QueryReport()
+        o = opt.c_struct()
+        st = self._lib.orc_solve_query(self._h, method, y_d.ctypes.data, psi.ctypes.data, j0p, wp, k, C.byref(o),
+                                       y.ctypes.data, u.ctypes.data, lam.ctypes.data, steps,
+                                       Jb.ctypes.data if want_sets else None, C.byref(rep))
+        ns = rep.n_steps
+        step_list: List[dict] = [{f: getattr(steps[i], f) for f, _ in _StepReport._fields_} for i in range(ns)]
+        return dict(status=st, n_steps=ns, kkt=[rep.kkt[i] for i in range(5)], y=y, u=u, lam=lam, steps=step_list,
+                    J_bits=(Jb[:ns] if want_sets else None),
+                    hashes=[s["active_hash"] for s in step_list])
+
+    def state(self):
+        y = np.empty(self.N)
+        J = np.empty(self.N, dtype=np.uint8)
+        A = np.empty(self.N, dtype=np.uint8)
+        self._lib.orc_get_state(self._h, y.ctypes.data, J.ctypes.data, A.ctypes.data)
+        return y, J, A
+
+
+def reference_eigs(rowptr, colidx, val, m, sigma, k, dense_below: int = 1500):
+    """The definition `build_reference` must reach: the k lowest eigenpairs (theta, W) of
+    H = M + sigma K^T M^{-1} K, W with orthonormal columns (N x k, column-major).
+
+    A library eigensolver on the assembled matrix (dense eigh for small N, shift-invert
+    Lanczos otherwise).  W is unique only up to sign / rotation inside clusters (reading A14)."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+
+    N = len(m)
+    K = sp.csr_matrix((val, colidx, rowptr), shape=(N, N))
+    H = (sp.diags(m) + sigma * (K.T @ sp.diags(1.0 / np.asarray(m)) @ K)).tocsc()
+    H = 0.5 * (H + H.T)
+    if N <= dense_below:
+        th, V = np.linalg.eigh(H.toarray())
+        return th[:k].copy(), np.asfortranarray(V[:, :k])
+    scale = float(np.mean(m))  # keep the shift-invert factorisation well scaled
+    th, V = spla.eigsh((H / scale).tocsc(), k=k, sigma=0.0, which="LM", tol=1e-12)
+    order = np.argsort(th)
+    return th[order] * scale, np.asfortranarray(V[:, order])

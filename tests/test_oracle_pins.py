@@ -1,0 +1,477 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Dense reference quantities are built here with
+numpy/scipy from the workload's K, m (an independent route: dense factorisations, brute force,
+closed forms), never by calling the oracle on itself.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from workloads import make_config, make_steady_2d, make_steady_3d, make_spacetime_2d
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def dense_H(w):
+    K = w.csr().toarray()
+    return np.diag(w.m) + w.alpha * K.T @ np.diag(1.0 / w.m) @ K
+
+
+def tiny_2d(n=8, seed_cfg=1):
+    return make_steady_2d(n=n, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-4, k=4, n_queries=2, n_bumps=3,
+                          psi_factor=0.6, pdas_cap=40, config=seed_cfg, name=f"tiny2d_{n}")
+
+
+def tiny_3d(n=5):
+    return make_steady_3d(n=n, bores=[(0.5, 0.5)], R=0.3, vpeak=30.0, alpha=1e-5, k=4, n_queries=1, n_bumps=4,
+                          psi_factor=0.6, pdas_cap=40, config=3, name=f"tiny3d_{n}")
+
+
+def tiny_st(n=6, nt=3):
+    return make_spacetime_2d(n=n, nt=nt, T=1.0, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-4, k=4, n_queries=1,
+                             n_bumps=3, psi_factor=0.6, pdas_cap=40, config=4, name=f"tinyst_{n}x{nt}")
+
+
+def pdas_dense(H, ell, psi, J0, cap=200):
+    """PDAS (eq. (7)-(8)) with dense direct solves; returns (y, lam, list of active sets)."""
+    N = len(ell)
+    J = J0.copy()
+    sets = []
+    y = np.zeros(N)
+    for _ in range(cap):
+        sets.append(J.copy())
+        I = ~J
+        y = np.where(J, psi, 0.0)
+        if I.any():
+            rhs = ell[I] - H[np.ix_(I, J)] @ psi[J]
+            y[I] = np.linalg.solve(H[np.ix_(I, I)], rhs)
+        lam = np.where(J, ell - H @ y, 0.0)
+        Jn = (lam + (y - psi)) > 0
+        if (Jn == J).all():
+            return y, lam, sets
+        J = Jn
+    raise AssertionError("dense PDAS did not converge")
+
+
+# ------------------------------------------------------------------ P2: symmetry, definiteness, masked apply
+@pytest.mark.parametrize("maker", [tiny_2d, tiny_3d, tiny_st])
+def test_P2_operator_matches_dense_and_is_spd(oracle_mod, maker):
+    w = maker()
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    rng = np.random.default_rng(0)
+    x, yv = rng.standard_normal(w.N), rng.standard_normal(w.N)
+    Hx, Hy = o.apply_H(x), o.apply_H(yv)
+    assert np.allclose(Hx, H @ x, rtol=1e-13, atol=1e-13 * np.abs(H @ x).max())
+    assert abs(x @ Hy - yv @ Hx) <= 1e-13 * abs(x @ Hy)
+    assert x @ Hx >= (w.m * x * x).sum()  # H - M = sigma (M^-1/2 K)^T (M^-1/2 K) >= 0
+    np.linalg.cholesky(H)
+    assert np.allclose(o.diag_H(), np.diag(H), rtol=1e-13)
+    # K, K^T legs on their own: a transposed operand must fail here
+    Kd = w.csr().toarray()
+    assert np.allclose(o.apply_K(x), Kd @ x, rtol=1e-13, atol=1e-13)
+    assert np.allclose(o.apply_KT(x), Kd.T @ x, rtol=1e-13, atol=1e-13)
+    assert not np.allclose(Kd @ x, Kd.T @ x)
+    # B x = (H R_I^T x)_I and every H_II is SPD
+    mask = rng.random(w.N) < 0.7
+    idx = np.flatnonzero(mask)
+    xi = rng.standard_normal(len(idx))
+    assert np.allclose(o.apply_B(idx, xi), H[np.ix_(idx, idx)] @ xi, rtol=1e-12, atol=1e-14)
+    np.linalg.cholesky(H[np.ix_(idx, idx)])
+
+
+# ------------------------------------------------------------------ P7: closed-form spectrum
+def test_P7_closed_form_spectrum(oracle_mod):
+    """Uniform kappa = 1, zero velocity: K has eigenvectors prod_a sin(pi k_a (j_a - 1/2)/n) and eigenvalues
+    h^(d-2) sum_a 4 sin^2(pi k_a/(2n)); theta = h^d + sigma (K-eig)^2 / h^d.
+    Cell-centred analogue of eq. (15)."""
+    n = 10
+    w = make_steady_2d(n=n, channels=[], vel=0.0, alpha=1e-4, k=6, n_queries=1, n_bumps=1, psi_factor=0.6,
+                       pdas_cap=5, config=1)
+    o = oracle_mod.Oracle.from_workload(w)
+    h = 1.0 / n
+    j = np.arange(1, n + 1)
+    thetas = []
+    for kx, ky in itertools.product(range(1, n + 1), repeat=2):
+        mu = 4 * np.sin(np.pi * kx / (2 * n)) ** 2 + 4 * np.sin(np.pi * ky / (2 * n)) ** 2  # h^(d-2) = 1
+        theta = h ** 2 + w.alpha * mu ** 2 / h ** 2
+        thetas.append(theta)
+        if (kx, ky) in [(1, 1), (2, 1), (1, 3), (n, n), (4, 7)]:
+            v = np.outer(np.sin(np.pi * ky * (j - 0.5) / n), np.sin(np.pi * kx * (j - 0.5) / n)).ravel()
+            assert np.allclose(o.apply_H(v), theta * v, rtol=1e-11, atol=1e-13 * theta)
+    thetas = np.sort(thetas)
+    th, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, 6)
+    assert np.allclose(th, thetas[:6], rtol=1e-10)
+    assert np.allclose(W.T @ W, np.eye(6), atol=1e-10)
+    # sparse shift-invert branch agrees with the dense branch
+    th2, W2 = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, 6, dense_below=10)
+    assert np.allclose(th2, thetas[:6], rtol=1e-9)
+    # 3D, the 7-point analogue
+    n3 = 5
+    w3 = make_steady_3d(n=n3, bores=[], R=0.1, vpeak=0.0, alpha=1e-5, k=4, n_queries=1, n_bumps=1, psi_factor=0.6,
+                        pdas_cap=5, config=3)
+    o3 = oracle_mod.Oracle.from_workload(w3)
+    h3 = 1.0 / n3
+    j3 = np.arange(1, n3 + 1)
+    kx, ky, kz = 2, 1, 3
+    s = lambda q: np.sin(np.pi * q * (j3 - 0.5) / n3)
+    v = np.einsum("z,y,x->zyx", s(kz), s(ky), s(kx)).ravel()
+    mu = h3 * sum(4 * np.sin(np.pi * q / (2 * n3)) ** 2 for q in (kx, ky, kz))
+    theta = h3 ** 3 + w3.alpha * mu ** 2 / h3 ** 3
+    assert np.allclose(o3.apply_H(v), theta * v, rtol=1e-11, atol=1e-14 * theta)
+
+
+# ------------------------------------------------------------------ P1/P3: PDAS against dense direct PDAS + KKT
+@pytest.mark.parametrize("maker,psi_factor", [(tiny_2d, 0.6), (tiny_2d, 0.3), (tiny_3d, 0.35), (tiny_st, 0.3)])
+@pytest.mark.parametrize("method", [0, 1, 2])
+def test_P1_P3_pdas_matches_dense_direct(oracle_mod, maker, psi_factor, method):
+    w = maker()
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    yd, _ = w.target(0)
+    psi = np.full(w.N, psi_factor * yd.max())
+    ell = w.m * yd
+    y_ref, lam_ref, sets_ref = pdas_dense(H, ell, psi, np.ones(w.N, dtype=bool))
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    opt = oracle_mod.OracleOptions(eps=1e-12, eps_c=1e-12, pdas_cap=60)
+    r = o.solve_query(method, yd, psi, W, opt)
+    assert r["status"] == 0
+    assert r["n_steps"] == len(sets_ref)
+    for s, Jb in zip(sets_ref, r["J_bits"]):
+        assert (np.unpackbits(Jb, bitorder="little")[: w.N].astype(bool) == s).all()
+    nrm = lambda v: np.sqrt((w.m * v * v).sum())
+    assert nrm(r["y"] - y_ref) <= 1e-9 * nrm(y_ref)
+    # P3: KKT system eq. (6) with the independent dense H
+    y, lam = r["y"], r["lam"]
+    assert np.abs(H @ y - ell + lam).max() <= 1e-10 * np.abs(ell).max()
+    assert (y <= psi + 1e-12).all() and (lam >= -1e-14).all()
+    assert np.abs(lam * (psi - y)).max() <= 1e-14
+    assert max(r["kkt"]) <= 1e-8  # eq. (25)
+    # recovery eq. (9): u = M^-1 K y uses all state values incl. the active ones
+    assert np.allclose(r["u"], (w.csr() @ y) / w.m, rtol=1e-12, atol=1e-12)
+    if psi_factor <= 0.35:
+        assert sets_ref[-1].any(), "bound must be active at the optimum for this pin to bite"
+
+
+def test_P1_bruteforce_active_sets(oracle_mod):
+    """N = 9: enumerate all 2^N active sets; strict convexity => exactly one satisfies eq. (6)."""
+    w = make_steady_2d(n=3, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-5, k=2, n_queries=1, n_bumps=3,
+                       psi_factor=0.3, pdas_cap=40, config=1)
+    H = dense_H(w)
+    yd, psi = w.target(0)
+    ell = w.m * yd
+    sols = []
+    for bits in itertools.product([False, True], repeat=w.N):
+        J = np.array(bits)
+        I = ~J
+        y = np.where(J, psi, 0.0)
+        if I.any():
+            y[I] = np.linalg.solve(H[np.ix_(I, I)], ell[I] - H[np.ix_(I, J)] @ psi[J])
+        lam = np.where(J, ell - H @ y, 0.0)
+        if (y[I] < psi[I]).all() and (lam[J] > 0).all():  # strict: excludes degenerate duplicates
+            sols.append((J, y))
+    assert len(sols) == 1
+    J_star, y_star = sols[0]
+    assert J_star.any() and not J_star.all()
+    o = oracle_mod.Oracle.from_workload(w)
+    r = o.solve_query(0, yd, psi, None, oracle_mod.OracleOptions(eps=1e-13, eps_c=1e-13, pdas_cap=40))
+    assert r["status"] == 0
+    J_fin = np.unpackbits(r["J_bits"][-1], bitorder="little")[: w.N].astype(bool)
+    assert (J_fin == J_star).all()
+    assert np.allclose(r["y"], y_star, rtol=1e-10, atol=1e-12)
+
+
+# ------------------------------------------------------------------ P4: unconstrained limit
+@pytest.mark.parametrize("method", [0, 1])
+def test_P4_unconstrained_limit(oracle_mod, method):
+    w = tiny_2d(10)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    yd, _ = w.target(0)
+    psi = np.full(w.N, np.inf)
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    r = o.solve_query(method, yd, psi, W, oracle_mod.OracleOptions(eps=1e-12, eps_c=1e-12))
+    y_ref = np.linalg.solve(H, w.m * yd)
+    assert r["status"] == 0 and r["n_steps"] == 1 and r["steps"][0]["n_inactive"] == w.N
+    assert np.allclose(r["y"], y_ref, rtol=1e-9, atol=1e-12)
+    assert (r["lam"] == 0).all()
+    assert np.allclose(r["u"], (w.csr() @ r["y"]) / w.m, rtol=1e-12)
+
+
+# ------------------------------------------------------------------ P5: projector identities
+def test_P5_projector_identities(oracle_mod):
+    w = tiny_2d(8)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    rng = np.random.default_rng(3)
+    idx = np.flatnonzero(rng.random(w.N) < 0.8)
+    n = len(idx)
+    B = H[np.ix_(idx, idx)]
+    Zt = rng.standard_normal((n, 5))
+    cs = o.coarse(idx, Zt)
+    assert cs.rank == 5 and not cs.fallback
+    Qm = np.column_stack([cs.Q(e) for e in np.eye(n)])
+    Pm = np.column_stack([cs.P(e) for e in np.eye(n)])
+    Z, BZ, E = cs.factors()
+    sc = np.abs(B).max()
+    assert np.allclose(Z.T @ Z, np.eye(5), atol=1e-12)
+    assert np.allclose(BZ, B @ Z, atol=1e-12 * sc)
+    assert np.allclose(E, Z.T @ B @ Z, atol=1e-12 * sc)
+    assert np.allclose(Qm, Z @ np.linalg.solve(E, Z.T), rtol=1e-9, atol=1e-9 / sc)
+    assert np.allclose(Pm, np.eye(n) - Qm @ B, atol=1e-9)
+    assert np.allclose(Qm @ B @ Qm, Qm, rtol=1e-9, atol=1e-9 / sc)      # QBQ = Q
+    assert np.allclose(Pm @ Pm, Pm, atol=1e-9)                          # P^2 = P
+    assert np.allclose(B @ Pm, Pm.T @ B, atol=1e-9 * sc)                # BP = P^T B
+    assert np.abs(Z.T @ B @ Pm).max() <= 1e-9 * sc                      # Z^T B P = 0
+    b = rng.standard_normal(n)
+    x0 = rng.standard_normal(n)
+    xc = x0 + cs.Q(b - B @ x0)
+    assert np.abs(Z.T @ (b - B @ xc)).max() <= 1e-9 * np.abs(b).max()   # Z^T (b - B x_c) = 0
+    # eq. (19): C_bal r = P J r when Z^T r = 0
+    Jm = np.diag(1.0 / np.diag(B))
+    Cbal = Pm @ Jm @ Pm.T + Qm
+    r = b - Z @ (Z.T @ b)
+    assert np.allclose(Cbal @ r, Pm @ Jm @ r, rtol=1e-8, atol=1e-8 * np.abs(Jm @ r).max())
+    np.linalg.cholesky(0.5 * (Cbal + Cbal.T))
+    # the span, not the columns, matters: a column-mixed copy of Z~ gives the same Q
+    cs2 = o.coarse(idx, Zt @ rng.standard_normal((5, 5)))
+    assert np.allclose(cs2.Q(b), cs.Q(b), rtol=1e-7, atol=1e-9 * np.abs(cs.Q(b)).max())
+
+
+def test_P5_rank_revealing(oracle_mod):
+    """dependent columns are dropped (singular values <= 1e-12 * largest)."""
+    w = tiny_2d(8)
+    o = oracle_mod.Oracle.from_workload(w)
+    rng = np.random.default_rng(4)
+    idx = np.arange(w.N)
+    Zt = rng.standard_normal((w.N, 4))
+    Zt = np.column_stack([Zt, Zt[:, 0] + Zt[:, 1], np.zeros(w.N)])
+    cs = o.coarse(idx, Zt)
+    assert cs.rank == 4
+    Z, _, _ = cs.factors()
+    assert np.allclose(Z.T @ Z, np.eye(4), atol=1e-12)
+    assert np.linalg.matrix_rank(np.column_stack([Z, Zt[:, :4]]), tol=1e-9) == 4
+    # fewer rows than columns: r_I <= min(|I|, r)
+    cs3 = o.coarse(np.array([3, 9, 20]), rng.standard_normal((3, 5)))
+    assert cs3.rank == 3
+
+
+# ------------------------------------------------------------------ P6: restriction-residual identity eq. (20)-(21)
+def test_P6_restriction_residual_identity(oracle_mod):
+    w = tiny_2d(8)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    rng = np.random.default_rng(5)
+    k = 5
+    th, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, k)
+    W = np.linalg.qr(W + 0.05 * rng.standard_normal(W.shape))[0]  # approximate, orthonormal reference
+    Lam = W.T @ H @ W
+    G0 = H @ W - W @ Lam
+    Jm = rng.random(w.N) < 0.25
+    I = np.flatnonzero(~Jm)
+    Jx = np.flatnonzero(Jm)
+    o.reset_sequence()
+    WI = o.restrict(oracle_mod.REFDEF, W, I)
+    assert (WI == W[I]).all()
+    BWI = np.column_stack([o.apply_B(I, WI[:, j]) for j in range(k)])
+    rhs = -H[np.ix_(I, Jx)] @ W[Jx] + G0[I]                           # eq. (20), Delta = 0
+    assert np.abs(BWI - WI @ Lam - rhs).max() <= 1e-13 * np.abs(H).max()
+    cs = o.coarse(I, WI)
+    Z, BZ, E = cs.factors()
+    R = Z.T @ WI                                                       # Phi_I = Z R
+    assert np.allclose(Z @ R, WI, atol=1e-12)
+    F = BZ - Z @ E
+    F21 = (np.eye(len(I)) - Z @ Z.T) @ rhs @ np.linalg.inv(R)          # eq. (21)
+    assert np.abs(F - F21).max() <= 1e-11 * np.abs(H).max()
+
+
+# ------------------------------------------------------------------ P8: rank zero == Jacobi-CG
+def test_P8_rank_zero_is_jacobi_cg(oracle_mod):
+    w = tiny_2d(12)
+    o = oracle_mod.Oracle.from_workload(w)
+    rng = np.random.default_rng(6)
+    idx = np.flatnonzero(rng.random(w.N) < 0.9)
+    b = rng.standard_normal(len(idx)) * w.m[0]
+    x0 = np.zeros(len(idx))
+    xa, ra = o.alg1(idx, b, x0, None)
+    xb, rb = o.alg1(idx, b, x0, np.zeros((len(idx), 3)))
+    assert ra["iters"] == rb["iters"] > 5 and rb["rank_used"] == 0
+    assert (xa == xb).all()
+    yd, psi = w.target(0)
+    o.reset_sequence()
+    q0 = o.solve_query(oracle_mod.JACOBI_CG, yd, psi, None)
+    o.reset_sequence()
+    q1 = o.solve_query(oracle_mod.REFDEF, yd, psi, np.zeros((w.N, 2)))
+    assert (q0["y"] == q1["y"]).all() and q0["hashes"] == q1["hashes"]
+    assert [s["cg_iters"] for s in q0["steps"]] == [s["cg_iters"] for s in q1["steps"]]
+
+
+# ------------------------------------------------------------------ P9: transfers, Figure 2
+def test_P9_fig2_transfer_pattern(oracle_mod):
+    rows = [ln.split() for ln in open(os.path.join(HERE, "golden", "fig2_transfer_pattern.txt"))
+            if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 6
+    w = make_steady_2d(n=3, channels=[], vel=0.0, alpha=1e-4, k=1, n_queries=1, n_bumps=1, psi_factor=0.6,
+                       pdas_cap=5, config=1)  # 9 DOFs; nodes 1..6 -> DOFs 0..5, DOFs 6..8 stay inactive
+    o = oracle_mod.Oracle.from_workload(w)
+    phi = np.arange(1.0, 10.0).reshape(-1, 1) / 7.0
+    prev_inactive = [int(r[0]) - 1 for r in rows if r[1] == "inactive"] + [6, 7, 8]
+    cur_inactive = [int(r[0]) - 1 for r in rows if r[2] == "inactive"] + [6, 7, 8]
+    for method, col in ((oracle_mod.REFDEF, 3), (oracle_mod.ZEROEXT, 4)):
+        o.reset_sequence()
+        first = o.restrict(method, phi, np.array(sorted(prev_inactive)))
+        assert (first[:, 0] == phi[sorted(prev_inactive), 0]).all()     # the first restriction is direct
+        Zt = o.restrict(method, phi, np.array(sorted(cur_inactive)))
+        got = dict(zip(sorted(cur_inactive), Zt[:, 0]))
+        for r in rows:
+            node = int(r[0]) - 1
+            if r[col] == "removed":
+                assert node not in got
+            elif r[col] == "phi":
+                assert got[node] == phi[node, 0]
+            else:
+                assert got[node] == 0.0
+        # eq. (13): the difference vanishes on shared inactive DOFs
+    # if J never changes, zero-extension == direct restriction
+    o.reset_sequence()
+    a = o.restrict(oracle_mod.ZEROEXT, phi, np.array([0, 1, 5, 6]))
+    b = o.restrict(oracle_mod.ZEROEXT, phi, np.array([0, 1, 5, 6]))
+    assert (a == b).all() and (a[:, 0] == phi[[0, 1, 5, 6], 0]).all()
+    # cumulative losses: a DOF active at ANY earlier restriction stays zero
+    o.reset_sequence()
+    o.restrict(oracle_mod.ZEROEXT, phi, np.array([0, 1, 2, 3]))        # 4.. active
+    o.restrict(oracle_mod.ZEROEXT, phi, np.array([0, 1, 2, 3, 4, 5, 6, 7, 8]))
+    c = o.restrict(oracle_mod.ZEROEXT, phi, np.array([0, 4, 8]))
+    assert (c[:, 0] == np.array([phi[0, 0], 0.0, 0.0])).all()
+
+
+# ------------------------------------------------------------------ P10: deflation with exact eigenvectors of B
+def test_P10_exact_eigenvector_deflation(oracle_mod):
+    w = make_steady_2d(n=4, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-3, k=6, n_queries=1, n_bumps=2,
+                       psi_factor=0.6, pdas_cap=5, config=1)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    idx = np.arange(w.N)
+    lamB, V = np.linalg.eigh(H)
+    k = 6
+    Z = V[:, :k]
+    rng = np.random.default_rng(7)
+    b = rng.standard_normal(w.N) * w.m[0]
+    xs = np.linalg.solve(H, b)
+    # cap = 0 returns the coarse-corrected x_c (Algorithm 1 line 3): it removes exactly the Z-components
+    xc, rep0 = o.alg1(idx, b, np.zeros(w.N), Z, eps=1e-12, cap=0, jacobi=0)
+    assert np.abs(Z.T @ (xs - xc)).max() <= 1e-9 * np.abs(xs).max()
+    assert np.allclose(xc, Z @ (Z.T @ xs), rtol=1e-8, atol=1e-10 * np.abs(xs).max())
+    # unpreconditioned CG then sees only the remaining N-k eigenvalues: <= N-k iterations
+    x, rep = o.alg1(idx, b, np.zeros(w.N), Z, eps=1e-10, jacobi=0)
+    assert rep["status"] == 0 and rep["iters"] <= w.N - k + 1
+    _, rep_plain = o.alg1(idx, b, np.zeros(w.N), None, eps=1e-10, jacobi=0)
+    assert rep_plain["iters"] > rep["iters"]
+    assert np.allclose(x, xs, rtol=1e-7, atol=1e-9 * np.abs(xs).max())
+
+
+# ------------------------------------------------------------------ P11: u-error identity (reading A16)
+def test_P11_u_error_identity(oracle_mod):
+    w = tiny_2d(10)
+    o = oracle_mod.Oracle.from_workload(w)
+    yd, psi = w.target(0)
+    o.reset_sequence()
+    a = o.solve_query(0, yd, psi, None, oracle_mod.OracleOptions(eps=1e-5, eps_c=1e-5))
+    o.reset_sequence()
+    b = o.solve_query(0, yd, psi, None, oracle_mod.OracleOptions(eps=1e-12, eps_c=1e-12))
+    e = a["y"] - b["y"]
+    du = a["u"] - b["u"]
+    lhs = (w.m * du * du).sum()
+    rhs = (e @ o.apply_H(e) - (w.m * e * e).sum()) / w.alpha
+    assert lhs > 0 and abs(lhs - rhs) <= 1e-8 * lhs
+
+
+# ------------------------------------------------------------------ P12: energy fraction eq. (24)
+def test_P12_energy_fraction(oracle_mod):
+    w = tiny_2d(8)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    rng = np.random.default_rng(8)
+    idx = np.flatnonzero(rng.random(w.N) < 0.85)
+    B = H[np.ix_(idx, idx)]
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, 4)
+    cs = o.coarse(idx, W[idx])
+    b = rng.standard_normal(len(idx)) * w.m[0]
+    xs = np.linalg.solve(B, b)
+    Qb = cs.Q(b)
+    en = lambda v: v @ B @ v
+    chi = en(Qb) / en(xs)
+    assert 0 < chi < 1
+    assert abs(en(xs - Qb) / en(xs) - (1 - chi)) <= 1e-10
+
+
+# ------------------------------------------------------------------ Algorithm 1 on its own: Verify, caps, replacement
+def test_alg1_statuses_and_verify(oracle_mod):
+    w = tiny_2d(12)
+    o = oracle_mod.Oracle.from_workload(w)
+    H = dense_H(w)
+    rng = np.random.default_rng(9)
+    idx = np.flatnonzero(rng.random(w.N) < 0.9)
+    B = H[np.ix_(idx, idx)]
+    b = rng.standard_normal(len(idx)) * w.m[0]
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, 4)
+    for Zt in (None, W[idx]):
+        x, rep = o.alg1(idx, b, np.zeros(len(idx)), Zt, eps=1e-9)
+        true_rel = np.linalg.norm(b - B @ x) / np.linalg.norm(b)
+        assert rep["status"] == 0 and true_rel <= 1e-9
+        assert abs(rep["rel_resid_verified"] - true_rel) <= 1e-3 * true_rel + 1e-16
+        x2, rep2 = o.alg1(idx, b, np.zeros(len(idx)), Zt, eps=1e-9, cap=3)
+        assert rep2["status"] == -6 and rep2["iters"] == 3                 # ECAP, last iterate returned
+        x3, rep3 = o.alg1(idx, b, np.zeros(len(idx)), Zt, eps=1e-9, replace_period=7)
+        assert rep3["status"] == 0 and rep3["replacements"] >= rep3["iters"] // 7
+        assert np.allclose(x3, x, rtol=1e-6, atol=1e-8 * np.abs(x).max())
+    # zero right-hand side with the exact initial guess: line 4 early exit, absolute criterion
+    x4, rep4 = o.alg1(idx, np.zeros(len(idx)), np.zeros(len(idx)), None)
+    assert rep4["status"] == 0 and rep4["iters"] == 0 and (x4 == 0).all()
+    # deflation never needs more iterations than Jacobi-CG here
+    _, rj = o.alg1(idx, b, np.zeros(len(idx)), None, eps=1e-9)
+    _, rd = o.alg1(idx, b, np.zeros(len(idx)), W[idx], eps=1e-9)
+    assert rd["iters"] <= rj["iters"]
+
+
+def test_config1_sequence_properties(oracle_mod):
+    """Config 1 as specified: all-active start, PDAS cap 20 (BASELINE.json); the three methods give the
+    same active-set sequence; direct restriction needs the fewest iterations (Table 3)."""
+    w = make_config(1)
+    o = oracle_mod.Oracle.from_workload(w)
+    yd, psi = w.target(0)
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    res = {}
+    for meth in (0, 1, 2):
+        o.reset_sequence()
+        res[meth] = o.solve_query(meth, yd, psi, W, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        assert res[meth]["steps"][0]["n_inactive"] == 0                   # first query starts all active
+        assert max(s["rel_resid_verified"] for s in res[meth]["steps"]) <= 1e-8
+    assert res[0]["hashes"] == res[1]["hashes"] == res[2]["hashes"]
+    it = {mth: sum(s["cg_iters"] for s in res[mth]["steps"]) for mth in res}
+    assert it[1] < it[2] <= it[0]
+    nrm = lambda v: np.sqrt((w.m * v * v).sum())
+    assert nrm(res[1]["y"] - res[0]["y"]) <= 1e-6 * nrm(res[0]["y"])
+
+
+def test_golden_config1_unchanged(oracle_mod):
+    """The stored oracle results (tests/golden/make_golden.py) still hold: sequence bit-exact, norms to 1e-9."""
+    import json
+
+    g = json.load(open(os.path.join(HERE, "golden", "config1_sequences.json")))
+    w = make_config(1)
+    assert g["operator_sha256"] == w.operator_hash()
+    o = oracle_mod.Oracle.from_workload(w)
+    yd, psi = w.target(0)
+    th, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    assert np.allclose(th, g["theta"], rtol=1e-9)
+    for name, meth in (("jacobi_cg", 0), ("refdef", 1), ("zeroext", 2)):
+        o.reset_sequence()
+        r = o.solve_query(meth, yd, psi, W, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        gm = g["methods"][name]
+        assert [f"{s['active_hash']:016x}" for s in r["steps"]] == gm["active_hash"]
+        assert [s["n_inactive"] for s in r["steps"]] == gm["n_inactive"]
+        assert abs(np.sqrt((w.m * r["y"] ** 2).sum()) - gm["y_Mnorm"]) <= 1e-9 * gm["y_Mnorm"]
