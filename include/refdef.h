@@ -1,0 +1,173 @@
+/*
+ * refdef.h -- C ABI of the B200-native hot path of arxiv/paper_2606_17971
+ * ("Reference-Space Reuse for Steady and Transient State-Constrained Conjugate Heat Transfer").
+ *
+ * Citations are PAPER.md:line (the text of the paper) plus section / equation / algorithm.
+ * Names follow BASELINE.json: K state operator (N x N sparse, integrated form), m the lumped mass
+ * diagonal (> 0), sigma the penalty scalar, H = M + sigma K^T M^{-1} K the SPD reduced Hessian
+ * (the paper's "M", eq. (5) PAPER.md:91-95 with A = M_l^{-1}K, W = M_l/m-bar of PAPER.md:133;
+ * the common factor 1/m-bar is dropped), W the full-domain reference (the paper's Phi, N x k),
+ * J the active set, I its complement, B = H_II the inactive system matrix (eq. (7)).
+ *
+ * POINTER CONVENTION.  Unless an argument says "host", every array argument may be a HOST pointer or a
+ * DEVICE pointer: the library asks the CUDA runtime (cudaPointerGetAttributes) and stages host data
+ * through its own device buffers with cudaMemcpyAsync on the context's stream.  Device pointers are used
+ * in place.  The library never frees or keeps caller memory: K, m and W are copied at create /
+ * set_reference.  All arithmetic of the path runs in CUDA kernels on the device the context was created
+ * on; there is no CPU fallback: without a usable CUDA device every entry point returns RD_ECUDA.
+ *
+ * ERRORS.  Every int-returning function returns an rd_status.  Hard errors (RD_EINVAL, RD_ENOMEM,
+ * RD_ECUDA, RD_ENOREF) leave outputs unspecified.  The soft statuses of a solve (RD_ENOTSPD, RD_ECAP,
+ * RD_ESTEPS, RD_ECYCLE, RD_ERESID) still return the last iterate and a complete report: the paper records
+ * such failures separately and keeps going.  No C++ exception crosses this boundary and
+ * there is no global state: one context = one operator = one reference.
+ *
+ * THREADS/STREAMS.  A context is not thread safe.  All work is enqueued on the stream given at create
+ * (NULL = the legacy default stream); calls that return host results synchronise that stream.
+ */
+#ifndef REFDEF_H
+#define REFDEF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rd_ctx rd_ctx; /* opaque; owns device copies of K, K^T, m, d, W and all work buffers */
+
+typedef enum {
+    RD_OK = 0,
+    RD_EINVAL = -1,
+    RD_ENOMEM = -2,
+    RD_ECUDA = -3,
+    RD_ENOREF = -4,  /* a deflated method was asked for but no reference is set */
+    RD_ENOTSPD = -5, /* m_i <= 0, or non-positive curvature / rho inside CG (Alg. 1 line 9) */
+    RD_ECAP = -6,    /* CG iteration cap reached */
+    RD_ESTEPS = -7,  /* PDAS step cap reached */
+    RD_ECYCLE = -8,  /* an active set repeated within one query */
+    RD_ERESID = -9   /* Verify failed: recurrence converged but the recomputed residual is above eps */
+} rd_status;
+
+/* Inner solver variants (PAPER.md:331-335 lists the paper's comparison set; BASELINE.json keeps three). */
+typedef enum {
+    RD_JACOBI_CG = 0, /* rank-zero execution of Algorithm 1 = Jacobi-preconditioned CG */
+    RD_REFDEF = 1,    /* direct restriction Z~ = R_I W, eq. (12) */
+    RD_ZEROEXT = 2    /* zero-extension transfer, eq. (13) PAPER.md:158-162 (cumulative over a sequence) */
+} rd_method;
+
+/* Initial active set of a query (the first query starts with every DOF active, later
+ * queries inherit state and active set; the cold-start variant resets to all active). */
+typedef enum {
+    RD_INIT_PAPER = 0,        /* first query of a sequence all active, later queries warm */
+    RD_INIT_ALL_ACTIVE = 1,
+    RD_INIT_ALL_INACTIVE = 2,
+    RD_INIT_GIVEN = 3         /* J0 flags supplied by the caller */
+} rd_init;
+
+typedef struct {
+    double sigma_is_alpha; /* 1: sigma = alpha (paper, eq. (5)); 0: sigma = 1/alpha (BASELINE.json's literal text) */
+    double eps;            /* Verify tolerance on ||b - Bx||/||b||; BASELINE.json: 1e-8 */
+    double eps_c;          /* recurrence trigger tau = eps_c ||b|| (Alg. 1 line 1) */
+    int32_t cg_cap;        /* CG iteration cap */
+    int32_t pdas_cap;      /* PDAS step cap */
+    int32_t replace_period;/* scheduled residual replacement period, 0 = only at candidate convergence */
+    int32_t jacobi;        /* 1: J = diag(B)^{-1}; 0: identity */
+    int32_t c_is_diag;     /* eq. (8): c_i = H_ii (1) or c = 1 (0, BASELINE.json configs) */
+    int32_t init;          /* rd_init */
+} rd_options;
+
+/* One PDAS step (one inactive system).  Times are milliseconds measured with CUDA events on the stream. */
+typedef struct {
+    int32_t n_inactive;     /* |I| at the start of the step */
+    int32_t cg_iters;       /* executions of Alg. 1 line 9 (operator applies inside the loop) */
+    int32_t rank_used;      /* retained rank r_I of the restricted basis */
+    int32_t coarse_fallback;/* 1: cond(E) > 1e10 or E not SPD -> rank-zero execution */
+    int32_t replacements;   /* times the replacement branch (Alg. 1 lines 11-20) was entered */
+    int32_t status;         /* rd_status of the inner solve */
+    double rel_resid_verified; /* Verify: ||b - Bx||_2/||b||_2 from a fresh apply */
+    double cond_E;          /* 2-norm condition number of E = Z^T B Z (eq. (18)) */
+    double margin;          /* min_i |lambda_i + c_i (y_i - psi_i)| over finite psi_i: distance of eq. (8) to a tie */
+    uint64_t active_hash;   /* FNV-1a (64 bit) of the packed active set at the start of the step */
+    double t_restrict, t_coarse, t_iter, t_update; /* ms: S1, S2, Algorithm 1, rhs + multiplier/active-set update */
+} rd_step_report;
+
+typedef struct {
+    int32_t n_steps, status;
+    double kkt[5];    /* eq. (25): stationarity, primal, dual, complementarity, projected gradient */
+    double t_total;   /* ms, whole call */
+    double t_reference_charged; /* ms of rd_build_reference charged to this query (first query after a build) */
+    int64_t total_cg_iters;
+} rd_query_report;
+
+/* Report of one Algorithm-1 solve through rd_solve_inactive. */
+typedef struct {
+    int32_t iters, rank_used, coarse_fallback, replacements, status;
+    double rel_resid_verified, cond_E, t_iter_ms;
+    double bytes_per_iter; /* algorithmic HBM bytes one loop iteration moves for this (N, n, nnz, rank) */
+} rd_solve_report;
+
+void rd_default_options(rd_options* opt);
+
+/* Step 1 of Algorithm 2: take the assembled operator.  K in CSR (rowptr: N+1 int64,
+ * colidx: nnz int32, val: nnz double; any order inside a row; duplicates are summed) and the lumped mass
+ * diagonal m (N doubles, all > 0 else RD_ENOTSPD).  alpha > 0.  Builds sliced-ELL copies of K and K^T, 1/m
+ * and d = diag(H), d_i = m_i + sigma sum_r K_ri^2/m_r (eq. (5)).  opt may be NULL (defaults).
+ * cuda_stream: a cudaStream_t or NULL. */
+int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* colidx, const double* val,
+              const double* m_diag, double alpha, const rd_options* opt, void* cuda_stream);
+void rd_destroy(rd_ctx* ctx);
+const char* rd_last_error(const rd_ctx* ctx); /* host string owned by the context; "" if none */
+int64_t rd_kernel_launches(const rd_ctx* ctx); /* CUDA kernels this context has launched so far */
+int rd_set_options(rd_ctx* ctx, const rd_options* opt); /* sigma_is_alpha cannot change after create (RD_EINVAL) */
+
+/* Steps 2-4 of Algorithm 2, BASELINE.json variant: the k lowest eigenpairs of the full
+ * H by a Jacobi-preconditioned block iteration (LOBPCG) run until every
+ * ||H w_j - theta_j w_j||_2 <= tol * theta_j (||w_j|| = 1) or max_block_iters block steps.  W is stored on
+ * the device (N x k, orthonormal columns).  theta_out: k doubles, may be NULL.  resid_out: k doubles
+ * (relative residuals reached), may be NULL.  iters_out: block steps used, may be NULL.
+ * 1 <= k <= 64.  The time is remembered and charged to the next query. */
+int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* theta_out,
+                       double* resid_out, int32_t* iters_out);
+/* Inject a reference (e.g. the oracle's): W is N x k column-major with leading dimension N. */
+int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W);
+/* Copy the stored reference out: W_out N x k column-major (ld N); returns k via k_out (0 if none). */
+int rd_get_reference(rd_ctx* ctx, double* W_out, int32_t* k_out);
+
+/* Steps 9-15 of Algorithm 2 for one query: PDAS, eq. (7)-(8) PAPER.md:102-117, with
+ * Algorithm 1 on every inactive system; then u = M^{-1} K y (eq. (9), f = 0)
+ * and the KKT measures of eq. (25).  y_d, psi: N doubles (psi_i = +inf allowed: never active).
+ * J0: N bytes (non-zero = active), used only with RD_INIT_GIVEN, else may be NULL.
+ * y, u, lambda: N doubles out (lambda may be NULL).  steps: host array of opt.pdas_cap entries.
+ * J_bits: NULL or host array of pdas_cap * ceil(N/8) bytes: the active set at the start of each step,
+ * packed LSB first.  rep: host. */
+int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double* psi, const uint8_t* J0,
+                   double* y, double* u, double* lambda, rd_step_report* steps, uint8_t* J_bits,
+                   rd_query_report* rep);
+/* Forget the warm-start state and the zero-extension history (start of a new sequence). */
+int rd_reset_sequence(rd_ctx* ctx);
+
+/* ---- single steps of the path, exported so that each can be checked against the oracle ---- */
+
+/* out = K v, out = K^T v (N doubles each). */
+int rd_apply_K(rd_ctx* ctx, const double* v, double* out);
+int rd_apply_KT(rd_ctx* ctx, const double* v, double* out);
+/* S3: out = H v (eq. (5)).  active: NULL (full operator) or N bytes (non-zero = active): then the masked
+ * operator of eq. (7), out_i = (H (chi_I v))_i on I and 0 on J. */
+int rd_apply_H(rd_ctx* ctx, const double* v, const uint8_t* active, double* out);
+int rd_diag_H(rd_ctx* ctx, double* d_out);
+/* Algorithm 1 on one inactive system (S1-S5): active = N bytes; b, x: N doubles in full-domain indexing
+ * (entries on J are ignored on input and 0 on output); x holds x0 on entry.  Deflated methods use the
+ * stored reference and, for RD_ZEROEXT, update the zero-extension history. */
+int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const double* b, double* x,
+                      rd_solve_report* rep);
+/* S1+S2 for one active set: restricted basis, Gram G = W_I^T W_I and E_W = W_I^T H_II W_I (both k x k
+ * column-major, may be NULL), and C = T E^{-1} T^T (k x k, the coarse solve in W_I coordinates, may be NULL);
+ * rank / cond / fallback as in rd_step_report. */
+int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C,
+                    int32_t* rank_used, double* cond_E, int32_t* fallback);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* REFDEF_H */

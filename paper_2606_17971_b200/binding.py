@@ -1,0 +1,282 @@
+"""ctypes binding of include/refdef.h -- argument marshalling only; every step runs in the CUDA library.
+
+Arrays may be numpy arrays (host pointers) or torch CUDA tensors (device pointers); the library tells
+them apart itself (cudaPointerGetAttributes).  Names mirror the C entry points.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "librefdef_b200.so")
+
+JACOBI_CG, REFDEF, ZEROEXT = 0, 1, 2
+INIT_PAPER, INIT_ALL_ACTIVE, INIT_ALL_INACTIVE, INIT_GIVEN = 0, 1, 2, 3
+STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", -5: "enotspd", -6: "ecap",
+                -7: "esteps", -8: "ecycle", -9: "eresid"}
+SOFT = (-5, -6, -7, -8, -9)
+
+EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
+           "rd_build_reference", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
+
+
+class RefDefError(RuntimeError):
+    pass
+
+
+class _Options(C.Structure):
+    _fields_ = [("sigma_is_alpha", C.c_double), ("eps", C.c_double), ("eps_c", C.c_double), ("cg_cap", C.c_int32),
+                ("pdas_cap", C.c_int32), ("replace_period", C.c_int32), ("jacobi", C.c_int32),
+                ("c_is_diag", C.c_int32), ("init", C.c_int32)]
+
+
+class _StepReport(C.Structure):
+    _fields_ = [("n_inactive", C.c_int32), ("cg_iters", C.c_int32), ("rank_used", C.c_int32),
+                ("coarse_fallback", C.c_int32), ("replacements", C.c_int32), ("status", C.c_int32),
+                ("rel_resid_verified", C.c_double), ("cond_E", C.c_double), ("margin", C.c_double),
+                ("active_hash", C.c_uint64), ("t_restrict", C.c_double), ("t_coarse", C.c_double),
+                ("t_iter", C.c_double), ("t_update", C.c_double)]
+
+
+class _QueryReport(C.Structure):
+    _fields_ = [("n_steps", C.c_int32), ("status", C.c_int32), ("kkt", C.c_double * 5), ("t_total", C.c_double),
+                ("t_reference_charged", C.c_double), ("total_cg_iters", C.c_int64)]
+
+
+class _SolveReport(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("rank_used", C.c_int32), ("coarse_fallback", C.c_int32),
+                ("replacements", C.c_int32), ("status", C.c_int32), ("rel_resid_verified", C.c_double),
+                ("cond_E", C.c_double), ("t_iter_ms", C.c_double), ("bytes_per_iter", C.c_double)]
+
+
+@dataclass
+class Options:
+    sigma_is_alpha: float = 1.0
+    eps: float = 1e-8
+    eps_c: float = 1e-8
+    cg_cap: int = 500000
+    pdas_cap: int = 100
+    replace_period: int = 0
+    jacobi: int = 1
+    c_is_diag: int = 0
+    init: int = INIT_PAPER
+
+    def c_struct(self) -> _Options:
+        return _Options(self.sigma_is_alpha, self.eps, self.eps_c, self.cg_cap, self.pdas_cap, self.replace_period,
+                        self.jacobi, self.c_is_diag, self.init)
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen the CUDA library; raises RefDefError if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise RefDefError(f"{path} is missing: build it with `python -m paper_2606_17971_b200.build` "
+                          "(nvcc, sm_100a); there is no CPU fallback")
+    lib = C.CDLL(path)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.rd_default_options.argtypes = [C.POINTER(_Options)]
+    lib.rd_default_options.restype = None
+    lib.rd_create.argtypes = [C.POINTER(vp), i64, vp, vp, vp, vp, dbl, C.POINTER(_Options), vp]
+    lib.rd_destroy.argtypes = [vp]
+    lib.rd_destroy.restype = None
+    lib.rd_last_error.argtypes = [vp]
+    lib.rd_last_error.restype = C.c_char_p
+    lib.rd_kernel_launches.argtypes = [vp]
+    lib.rd_kernel_launches.restype = i64
+    lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
+    lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
+    lib.rd_set_reference.argtypes = [vp, i32, vp]
+    lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
+    lib.rd_solve_query.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, C.POINTER(_StepReport), vp, C.POINTER(_QueryReport)]
+    lib.rd_reset_sequence.argtypes = [vp]
+    lib.rd_apply_K.argtypes = [vp, vp, vp]
+    lib.rd_apply_KT.argtypes = [vp, vp, vp]
+    lib.rd_apply_H.argtypes = [vp, vp, vp, vp]
+    lib.rd_diag_H.argtypes = [vp, vp]
+    lib.rd_solve_inactive.argtypes = [vp, i32, vp, vp, vp, C.POINTER(_SolveReport)]
+    lib.rd_coarse_setup.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl), C.POINTER(i32)]
+    _lib = lib
+    return lib
+
+
+def exported_symbols(path: Optional[str] = None):
+    """Names from EXPORTS that the built library really exports (a CPU-side check; no CUDA call is made)."""
+    lib = C.CDLL(path or LIB_PATH)
+    return [s for s in EXPORTS if hasattr(lib, s)]
+
+
+def _ptr(a):
+    """Raw pointer of a numpy array (host) or a torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"] and not a.flags["F_CONTIGUOUS"]:
+            raise ValueError("array must be contiguous")
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return a.data_ptr()
+    raise TypeError(type(a))
+
+
+def _np(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+class RefDef:
+    """One context = one operator (K, m, alpha) = one reference.  Mirrors rd_* one to one."""
+
+    def __init__(self, rowptr, colidx, val, m, alpha, opt: Optional[Options] = None, stream: int = 0):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        self.N = int(len(m))
+        self.opt = opt or Options()
+        o = self.opt.c_struct()
+        rp, ci, va, mm = _np(rowptr, np.int64), _np(colidx, np.int32), _np(val, np.float64), _np(m, np.float64)
+        st = self._lib.rd_create(C.byref(self._h), self.N, rp.ctypes.data, ci.ctypes.data, va.ctypes.data,
+                                 mm.ctypes.data, float(alpha), C.byref(o), C.c_void_p(stream or None))
+        if st != 0:
+            msg = self._lib.rd_last_error(self._h).decode() if self._h else ""
+            if self._h:
+                self._lib.rd_destroy(self._h)
+                self._h = C.c_void_p()
+            raise RefDefError(f"rd_create: {STATUS_NAMES.get(st, st)} {msg}")
+        self.k = 0
+
+    @classmethod
+    def from_workload(cls, w, opt: Optional[Options] = None, stream: int = 0):
+        return cls(w.rowptr, w.colidx, w.val, w.m, w.alpha, opt, stream)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.rd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st, what, soft_ok=False):
+        if st == 0 or (soft_ok and st in SOFT):
+            return st
+        raise RefDefError(f"{what}: {STATUS_NAMES.get(st, st)} {self._lib.rd_last_error(self._h).decode()}")
+
+    # ---- plumbing
+    def kernel_launches(self) -> int:
+        return int(self._lib.rd_kernel_launches(self._h))
+
+    def set_options(self, opt: Options):
+        o = opt.c_struct()
+        self._check(self._lib.rd_set_options(self._h, C.byref(o)), "rd_set_options")
+        self.opt = opt
+
+    def reset_sequence(self):
+        self._check(self._lib.rd_reset_sequence(self._h), "rd_reset_sequence")
+
+    # ---- reference
+    def build_reference(self, k, tol=1e-3, max_block_iters=2000):
+        theta = np.zeros(k)
+        resid = np.zeros(k)
+        it = C.c_int32(0)
+        self._check(self._lib.rd_build_reference(self._h, k, tol, max_block_iters, theta.ctypes.data, resid.ctypes.data,
+                                                 C.byref(it)), "rd_build_reference", soft_ok=True)
+        self.k = k
+        return theta, resid, it.value
+
+    def set_reference(self, W):
+        """W: N x k, numpy (any order; copied column-major) or a column-major device tensor of shape (k, N)."""
+        if isinstance(W, np.ndarray):
+            W = np.asfortranarray(W, dtype=np.float64)
+            k = W.shape[1]
+        else:
+            k = W.shape[0]
+        self._check(self._lib.rd_set_reference(self._h, k, _ptr(W)), "rd_set_reference")
+        self.k = k
+
+    def get_reference(self):
+        k = C.c_int32(0)
+        self._check(self._lib.rd_get_reference(self._h, None, C.byref(k)), "rd_get_reference")
+        W = np.zeros((self.N, k.value), order="F")
+        if k.value:
+            self._check(self._lib.rd_get_reference(self._h, W.ctypes.data, C.byref(k)), "rd_get_reference")
+        return W
+
+    # ---- single steps
+    def _apply(self, fn, v, out=None, *extra):
+        if out is None:
+            out = np.empty(self.N) if isinstance(v, np.ndarray) else v.new_empty(v.shape)
+        self._check(fn(self._h, _ptr(v), *extra, _ptr(out)), fn.__name__)
+        return out
+
+    def apply_K(self, v, out=None):
+        return self._apply(self._lib.rd_apply_K, v, out)
+
+    def apply_KT(self, v, out=None):
+        return self._apply(self._lib.rd_apply_KT, v, out)
+
+    def apply_H(self, v, active=None, out=None):
+        return self._apply(self._lib.rd_apply_H, v, out, _ptr(active))
+
+    def diag_H(self):
+        d = np.empty(self.N)
+        self._check(self._lib.rd_diag_H(self._h, d.ctypes.data), "rd_diag_H")
+        return d
+
+    def solve_inactive(self, method, active, b, x0):
+        """Algorithm 1 on the inactive system of `active` (N bytes).  Returns (x, report dict)."""
+        if isinstance(x0, np.ndarray):
+            x = np.array(x0, dtype=np.float64, copy=True)
+        else:
+            x = x0.clone()
+        rep = _SolveReport()
+        self._check(self._lib.rd_solve_inactive(self._h, method, _ptr(active), _ptr(b), _ptr(x), C.byref(rep)),
+                    "rd_solve_inactive", soft_ok=True)
+        return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+
+    def coarse_setup(self, method, active):
+        k = self.k
+        G, EW, Cm = np.zeros((k, k), order="F"), np.zeros((k, k), order="F"), np.zeros((k, k), order="F")
+        rank, fb, cond = C.c_int32(0), C.c_int32(0), C.c_double(0)
+        self._check(self._lib.rd_coarse_setup(self._h, method, _ptr(active), G.ctypes.data, EW.ctypes.data,
+                                              Cm.ctypes.data, C.byref(rank), C.byref(cond), C.byref(fb)), "rd_coarse_setup")
+        return dict(G=G, EW=EW, C=Cm, rank=rank.value, cond_E=cond.value, fallback=fb.value)
+
+    # ---- the query
+    def solve_query(self, method, y_d, psi, J0=None, y=None, u=None, lam=None, want_sets=True):
+        """PDAS query.  Host (numpy) or device (torch) y_d / psi; outputs allocated to match unless given."""
+        N = self.N
+        host = isinstance(y_d, np.ndarray)
+        if y is None:
+            y = np.empty(N) if host else y_d.new_empty(N)
+        if u is None:
+            u = np.empty(N) if host else y_d.new_empty(N)
+        if lam is None:
+            lam = np.empty(N) if host else y_d.new_empty(N)
+        cap = self.opt.pdas_cap
+        steps = (_StepReport * cap)()
+        nbytes = (N + 7) // 8
+        Jb = np.zeros((cap, nbytes), dtype=np.uint8) if want_sets else None
+        rep = _QueryReport()
+        st = self._lib.rd_solve_query(self._h, method, _ptr(y_d), _ptr(psi), _ptr(J0), _ptr(y), _ptr(u), _ptr(lam), steps,
+                                      Jb.ctypes.data if want_sets else None, C.byref(rep))
+        self._check(st, "rd_solve_query", soft_ok=True)
+        ns = rep.n_steps
+        step_list = [{f: getattr(steps[i], f) for f, _ in _StepReport._fields_} for i in range(ns)]
+        return dict(status=st, n_steps=ns, kkt=[rep.kkt[i] for i in range(5)], y=y, u=u, lam=lam, steps=step_list,
+                    J_bits=(Jb[:ns] if want_sets else None), hashes=[s["active_hash"] for s in step_list],
+                    t_total_ms=rep.t_total, t_reference_ms=rep.t_reference_charged, total_cg_iters=rep.total_cg_iters)

@@ -1,0 +1,807 @@
+// refdef_api.cu -- the C ABI of include/refdef.h: context, host orchestration of the PDAS loop, launches.
+// One translation unit; all device code is in the .cuh files beside it.  Links only against cudart.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/refdef.h"
+#include "cg.cuh"
+#include "coarse.cuh"
+#include "eigs.cuh"
+#include "pdas.cuh"
+
+using namespace rd;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+struct EllStore {
+    int32_t* col = nullptr;
+    double* val = nullptr;
+    int64_t* off = nullptr;
+    int64_t nslices = 0, entries = 0;
+    Ell view() const { return Ell{col, val, off, nslices}; }
+};
+
+}  // namespace
+
+struct rd_ctx {
+    int64_t N = 0, nnz = 0, ldw = 0;
+    int device = 0, num_sms = 0;
+    cudaStream_t stream = nullptr;
+    double alpha = 0, sigma = 0;
+    rd_options opt;
+    std::string err;
+    std::vector<void*> allocs;  // everything cudaMalloc'ed (freed in destroy)
+    std::vector<void*> pinned;
+
+    EllStore K, KT;
+    double *m = nullptr, *minv = nullptr, *d = nullptr, *dinv = nullptr;
+    // work vectors (length ldw)
+    double *x = nullptr, *r = nullptr, *p0 = nullptr, *p1 = nullptr, *z = nullptr, *w = nullptr, *t = nullptr;
+    double *b = nullptr, *tmp = nullptr, *Hy = nullptr, *ell = nullptr, *y = nullptr, *ystate = nullptr;
+    double *lam = nullptr, *u = nullptr, *in0 = nullptr, *in1 = nullptr;  // staging for host callers
+    uint8_t *act = nullptr, *act_new = nullptr, *hist = nullptr, *bits = nullptr, *act_stage = nullptr;
+    uint8_t* h_bits = nullptr;  // pinned
+    int* d_nactive = nullptr;
+    int* h_nactive = nullptr;
+    // reference
+    int k = 0, kp = 0;
+    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *Tchunk = nullptr;
+    double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;
+    int gram_nparts = 0;
+    CoarseInfo* d_cinfo = nullptr;
+    CoarseInfo* h_cinfo = nullptr;
+    // CG
+    int cg_grid = 0;
+    double* partial = nullptr;
+    GridBarrier* bar = nullptr;
+    CgDevReport* d_cgrep = nullptr;
+    CgDevReport* h_cgrep = nullptr;
+    PdasCounters* d_cnt = nullptr;
+    PdasCounters* h_cnt = nullptr;
+    cudaEvent_t ev[8];
+    bool have_state = false;
+    double ref_ms_pending = 0.0;
+    int64_t launches = 0;  // kernels launched so far (rd_kernel_launches)
+};
+
+namespace {
+
+int fail(rd_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return code;
+}
+
+#define CU(call)                                                                                        \
+    do {                                                                                                \
+        cudaError_t e__ = (call);                                                                       \
+        if (e__ != cudaSuccess) return fail(ctx, RD_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+bool is_device_ptr(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <class T>
+int dalloc(rd_ctx* ctx, T** out, size_t count, bool zero = true)
+{
+    void* p = nullptr;
+    size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, RD_ENOMEM, "cudaMalloc(%zu bytes): %s", bytes, cudaGetErrorString(e));
+    }
+    ctx->allocs.push_back(p);
+    if (zero) {
+        e = cudaMemsetAsync(p, 0, bytes, ctx->stream);
+        if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+    }
+    *out = (T*)p;
+    return RD_OK;
+}
+template <class T>
+int halloc(rd_ctx* ctx, T** out, size_t count)
+{
+    void* p = nullptr;
+    cudaError_t e = cudaMallocHost(&p, std::max<size_t>(count, 1) * sizeof(T));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(ctx, RD_ENOMEM, "cudaMallocHost: %s", cudaGetErrorString(e));
+    }
+    memset(p, 0, std::max<size_t>(count, 1) * sizeof(T));
+    ctx->pinned.push_back(p);
+    *out = (T*)p;
+    return RD_OK;
+}
+#define RDTRY(x)                  \
+    do {                          \
+        int rc__ = (x);           \
+        if (rc__ != RD_OK) return rc__; \
+    } while (0)
+
+// Host/device input: returns a device pointer holding `count` elements of src (staged if src is host).
+template <class T>
+int in_dev(rd_ctx* ctx, const T* src, size_t count, T* stage, const T** out)
+{
+    if (!src) { *out = nullptr; return RD_OK; }
+    if (is_device_ptr(src)) { *out = src; return RD_OK; }
+    CU(cudaMemcpyAsync(stage, src, count * sizeof(T), cudaMemcpyHostToDevice, ctx->stream));
+    *out = stage;
+    return RD_OK;
+}
+template <class T>
+int out_host(rd_ctx* ctx, T* dst, const T* dev, size_t count)
+{
+    if (!dst || dst == dev) return RD_OK;
+    CU(cudaMemcpyAsync(dst, dev, count * sizeof(T), is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                       ctx->stream));
+    return RD_OK;
+}
+
+inline int grid_for(int64_t work, int threads, int cap)
+{
+    int64_t g = (work + threads - 1) / threads;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(g, cap));
+}
+
+// ---- host construction of the two sliced-ELL matrices ------------------------------------------------
+struct HostEll {
+    std::vector<int32_t> col;
+    std::vector<double> val;
+    std::vector<int64_t> off;
+};
+
+void csr_to_ell(int64_t N, const std::vector<int64_t>& rp, const std::vector<int32_t>& ci, const std::vector<double>& va,
+                HostEll& E)
+{
+    const int64_t ns = (N + RD_SLICE - 1) / RD_SLICE;
+    E.off.assign(ns + 1, 0);
+    for (int64_t s = 0; s < ns; ++s) {
+        int64_t wd = 0;
+        for (int64_t r = s * RD_SLICE; r < std::min(N, (s + 1) * RD_SLICE); ++r) wd = std::max(wd, rp[r + 1] - rp[r]);
+        E.off[s + 1] = E.off[s] + wd * RD_SLICE;
+    }
+    E.col.assign(E.off[ns], 0);
+    E.val.assign(E.off[ns], 0.0);
+    for (int64_t s = 0; s < ns; ++s) {
+        const int64_t wd = (E.off[s + 1] - E.off[s]) / RD_SLICE;
+        for (int l = 0; l < RD_SLICE; ++l) {
+            const int64_t r = s * RD_SLICE + l;
+            const int32_t self = (int32_t)std::min<int64_t>(r, N - 1);
+            const int64_t len = (r < N) ? rp[r + 1] - rp[r] : 0;
+            for (int64_t e = 0; e < wd; ++e) {
+                const int64_t pos = E.off[s] + e * RD_SLICE + l;
+                if (e < len) { E.col[pos] = ci[rp[r] + e]; E.val[pos] = va[rp[r] + e]; }
+                else { E.col[pos] = self; E.val[pos] = 0.0; }
+            }
+        }
+    }
+}
+
+int upload_ell(rd_ctx* ctx, const HostEll& h, EllStore& d)
+{
+    d.nslices = (int64_t)h.off.size() - 1;
+    d.entries = h.off.back();
+    RDTRY(dalloc(ctx, &d.col, h.col.size(), false));
+    RDTRY(dalloc(ctx, &d.val, h.val.size(), false));
+    RDTRY(dalloc(ctx, &d.off, h.off.size(), false));
+    CU(cudaMemcpyAsync(d.col, h.col.data(), h.col.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d.val, h.val.data(), h.val.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d.off, h.off.data(), h.off.size() * sizeof(int64_t), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));  // the host vectors go away
+    return RD_OK;
+}
+
+uint64_t fnv1a(const uint8_t* p, int64_t n)
+{
+    uint64_t h = 1469598103934665603ULL;
+    for (int64_t i = 0; i < n; ++i) { h ^= (uint64_t)p[i]; h *= 1099511628211ULL; }
+    return h;
+}
+
+constexpr int kThreads = 256;
+inline int big_grid(rd_ctx* ctx) { return ctx->num_sms * 8; }
+
+// out = H v (unmasked: act == NULL) or chi_I H v (v must already vanish on J).  Uses ctx->t.
+int launch_apply_H(rd_ctx* ctx, const double* v, const uint8_t* act, double* out)
+{
+    const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    k_apply_K<<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), ctx->N, ctx->minv, v, ctx->t);
+    k_apply_KT_H<<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), ctx->N, ctx->m, ctx->sigma, act, v, ctx->t, out);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    return RD_OK;
+}
+
+int alloc_reference(rd_ctx* ctx, int k)
+{
+    const int kp = (k + 7) & ~7;
+    if (ctx->kp >= kp && ctx->W) { ctx->k = k; return RD_OK; }
+    // (buffers of an earlier, smaller reference stay allocated until destroy)
+    const size_t nk = (size_t)ctx->ldw * kp;
+    RDTRY(dalloc(ctx, &ctx->W, nk));
+    RDTRY(dalloc(ctx, &ctx->Wm, nk));
+    RDTRY(dalloc(ctx, &ctx->HWm, nk));
+    RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
+    ctx->gram_nparts = ctx->num_sms * 2;
+    RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
+    RDTRY(dalloc(ctx, &ctx->G, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->EW, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->cwork, (size_t)6 * kp * kp));
+    RDTRY(dalloc(ctx, &ctx->C, (size_t)kp * kp));
+    ctx->k = k;
+    ctx->kp = kp;
+    return RD_OK;
+}
+
+// S1 + S2 for the active set in ctx->act.  Leaves Wm, HWm, C and *h_cinfo (after a stream sync by the caller).
+int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse)
+{
+    const int64_t N = ctx->N;
+    const int kp = ctx->kp;
+    CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+    k_restrict<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
+    ctx->launches++;
+    CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    for (int j = 0; j < kp; j += 8) {
+        const double* V = ctx->Wm + (size_t)j * ctx->ldw;
+        k_spmm_K<8><<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->ldw, ctx->minv, V, ctx->ldw, ctx->Tchunk);
+        k_spmm_KT<8><<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->ldw, ctx->m, ctx->sigma, ctx->act, V, ctx->ldw,
+                                                       ctx->Tchunk, ctx->ldw, ctx->HWm + (size_t)j * ctx->ldw);
+        ctx->launches += 2;
+    }
+    dim3 gg(ctx->gram_nparts, (kp + 63) / 64, (kp + 63) / 64);
+    const int64_t kk = (int64_t)kp * kp;
+    k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, kp, kp, ctx->Wm, ctx->ldw, ctx->Wm, ctx->ldw, ctx->gram_parts);
+    k_reduce_parts<<<grid_for(kk, kThreads, 64), kThreads, 0, ctx->stream>>>(ctx->gram_nparts, kk, ctx->gram_parts, ctx->G);
+    k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, kp, kp, ctx->Wm, ctx->ldw, ctx->HWm, ctx->ldw, ctx->gram_parts);
+    k_reduce_parts<<<grid_for(kk, kThreads, 64), kThreads, 0, ctx->stream>>>(ctx->gram_nparts, kk, ctx->gram_parts, ctx->EW);
+    k_coarse_small<<<1, 1024, 0, ctx->stream>>>(kp, ctx->G, ctx->EW, ctx->cwork, ctx->C, ctx->d_cinfo);
+    ctx->launches += 5;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ctx->h_cinfo, ctx->d_cinfo, sizeof(CoarseInfo), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (ms_restrict) CU(cudaEventElapsedTime(ms_restrict, ctx->ev[0], ctx->ev[1]));
+    if (ms_coarse) CU(cudaEventElapsedTime(ms_coarse, ctx->ev[1], ctx->ev[2]));
+    return RD_OK;
+}
+
+// Algorithm 1 on the system defined by ctx->act, rhs ctx->b, start ctx->x (both zero on J).  Blocking.
+int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, float* ms_restrict, float* ms_coarse)
+{
+    const int64_t N = ctx->N;
+    memset(rep, 0, sizeof *rep);
+    if (ms_restrict) *ms_restrict = 0;
+    if (ms_coarse) *ms_coarse = 0;
+    int use_coarse = 0;
+    if (method != RD_JACOBI_CG) {
+        if (!ctx->W || ctx->k <= 0) return fail(ctx, RD_ENOREF, "method %d needs a reference (rd_build_reference / rd_set_reference)", method);
+        RDTRY(coarse_setup(ctx, method, ms_restrict, ms_coarse));
+        rep->rank_used = ctx->h_cinfo->rank;
+        rep->coarse_fallback = ctx->h_cinfo->fallback;
+        rep->cond_E = ctx->h_cinfo->cond_E;
+        use_coarse = ctx->h_cinfo->rank > 0;
+    }
+    // zero-extension history A <- A u J after every restriction of the sequence, whichever method runs
+    k_hist_update<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->hist);
+    ctx->launches++;
+
+    CgParams P;
+    memset(&P, 0, sizeof P);
+    P.N = N; P.ldw = ctx->ldw; P.kp = ctx->kp; P.use_coarse = use_coarse;
+    P.K = ctx->K.view(); P.KT = ctx->KT.view();
+    P.m = ctx->m; P.minv = ctx->minv; P.dinv = ctx->dinv; P.sigma = ctx->sigma;
+    P.act = ctx->act; P.b = ctx->b;
+    P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
+    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.C = ctx->C;
+    P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
+    P.partial = ctx->partial; P.bar = ctx->bar; P.rep = ctx->d_cgrep;
+    CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
+    CU(cudaMemsetAsync(ctx->p1, 0, ctx->ldw * sizeof(double), ctx->stream));
+    CU(cudaMemsetAsync(ctx->z, 0, ctx->ldw * sizeof(double), ctx->stream));
+    CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
+    CU(cudaEventRecord(ctx->ev[3], ctx->stream));
+    void* args[] = {(void*)&P};
+    CU(cudaLaunchCooperativeKernel((const void*)k_alg1, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, 0, ctx->stream));
+    ctx->launches++;
+    CU(cudaEventRecord(ctx->ev[4], ctx->stream));
+    CU(cudaMemcpyAsync(ctx->h_cgrep, ctx->d_cgrep, sizeof(CgDevReport), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    float ms = 0;
+    CU(cudaEventElapsedTime(&ms, ctx->ev[3], ctx->ev[4]));
+    rep->iters = ctx->h_cgrep->iters;
+    rep->replacements = ctx->h_cgrep->replacements;
+    rep->status = ctx->h_cgrep->status;
+    rep->rel_resid_verified = ctx->h_cgrep->rel_resid_verified;
+    rep->t_iter_ms = ms;
+    // algorithmic HBM bytes of one loop iteration:
+    // both ELL matrices once (8 B value + 4 B index per stored nonzero), t written and read on all N rows,
+    // 14 vector passes over the n inactive rows, the two n x r passes over HW_I and W_I, the mask.
+    const double rnk = use_coarse ? (double)rep->rank_used : 0.0;
+    rep->bytes_per_iter = 24.0 * (double)ctx->nnz + 16.0 * (double)N + 112.0 * (double)n_inactive +
+                          16.0 * (double)n_inactive * rnk + (double)N;
+    return RD_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+void rd_default_options(rd_options* o)
+{
+    o->sigma_is_alpha = 1.0;
+    o->eps = 1e-8;
+    o->eps_c = 1e-8;
+    o->cg_cap = 500000;
+    o->pdas_cap = 100;
+    o->replace_period = 0;
+    o->jacobi = 1;
+    o->c_is_diag = 0;
+    o->init = RD_INIT_PAPER;
+}
+
+const char* rd_last_error(const rd_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+void rd_destroy(rd_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    for (void* p : ctx->allocs) cudaFree(p);
+    for (void* p : ctx->pinned) cudaFreeHost(p);
+    for (auto& e : ctx->ev) if (e) cudaEventDestroy(e);
+    delete ctx;
+}
+
+int64_t rd_kernel_launches(const rd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* colidx, const double* val,
+              const double* m_diag, double alpha, const rd_options* opt, void* cuda_stream)
+{
+    if (!out) return RD_EINVAL;
+    *out = nullptr;
+    if (N <= 0 || N > 2000000000LL || !rowptr || !colidx || !val || !m_diag || !(alpha > 0.0)) return RD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return RD_ECUDA;  // no CPU fallback
+    }
+    rd_ctx* ctx = new (std::nothrow) rd_ctx();
+    if (!ctx) return RD_ENOMEM;
+    for (auto& e : ctx->ev) e = nullptr;
+    *out = ctx;  // returned even on failure so that rd_last_error can be read; caller destroys
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->N = N;
+    ctx->ldw = (N + 31) & ~(int64_t)31;
+    ctx->alpha = alpha;
+    if (opt) ctx->opt = *opt; else rd_default_options(&ctx->opt);
+    ctx->sigma = (ctx->opt.sigma_is_alpha != 0.0) ? alpha : 1.0 / alpha;
+    CU(cudaGetDevice(&ctx->device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, ctx->device));
+    ctx->num_sms = prop.multiProcessorCount;
+    if (!prop.cooperativeLaunch) return fail(ctx, RD_ECUDA, "device lacks cooperative launch");
+    for (auto& e : ctx->ev) CU(cudaEventCreate(&e));
+
+    // ---- bring the CSR to the host (setup only), sort rows, merge duplicates ----
+    std::vector<int64_t> rp(N + 1);
+    CU(cudaMemcpy(rp.data(), rowptr, (N + 1) * sizeof(int64_t), cudaMemcpyDefault));
+    const int64_t nnz_in = rp[N];
+    if (rp[0] != 0 || nnz_in < 0) return fail(ctx, RD_EINVAL, "rowptr[0] != 0 or negative nnz");
+    std::vector<int32_t> ci(nnz_in);
+    std::vector<double> va(nnz_in), mh(N);
+    CU(cudaMemcpy(ci.data(), colidx, nnz_in * sizeof(int32_t), cudaMemcpyDefault));
+    CU(cudaMemcpy(va.data(), val, nnz_in * sizeof(double), cudaMemcpyDefault));
+    CU(cudaMemcpy(mh.data(), m_diag, N * sizeof(double), cudaMemcpyDefault));
+    for (int64_t i = 0; i < N; ++i)
+        if (!(mh[i] > 0.0) || !std::isfinite(mh[i])) return fail(ctx, RD_ENOTSPD, "m[%lld] = %g is not > 0", (long long)i, mh[i]);
+    std::vector<int64_t> rp2(N + 1, 0);
+    std::vector<int32_t> ci2;
+    std::vector<double> va2;
+    ci2.reserve(nnz_in);
+    va2.reserve(nnz_in);
+    {
+        std::vector<std::pair<int32_t, double>> row;
+        for (int64_t r = 0; r < N; ++r) {
+            if (rp[r + 1] < rp[r]) return fail(ctx, RD_EINVAL, "rowptr not monotone at row %lld", (long long)r);
+            row.clear();
+            for (int64_t e = rp[r]; e < rp[r + 1]; ++e) {
+                if (ci[e] < 0 || ci[e] >= N) return fail(ctx, RD_EINVAL, "column index out of range at entry %lld", (long long)e);
+                row.emplace_back(ci[e], va[e]);
+            }
+            std::stable_sort(row.begin(), row.end(), [](const std::pair<int32_t, double>& a, const std::pair<int32_t, double>& b) { return a.first < b.first; });
+            for (size_t q = 0; q < row.size(); ++q) {
+                if (!ci2.empty() && (int64_t)ci2.size() > rp2[r] && ci2.back() == row[q].first) va2.back() += row[q].second;
+                else { ci2.push_back(row[q].first); va2.push_back(row[q].second); }
+            }
+            rp2[r + 1] = (int64_t)ci2.size();
+        }
+    }
+    ctx->nnz = rp2[N];
+    // transpose (counting sort: rows of K^T come out with ascending column = ascending row of K)
+    std::vector<int64_t> tp(N + 1, 0);
+    for (int64_t e = 0; e < ctx->nnz; ++e) tp[ci2[e] + 1]++;
+    for (int64_t i = 0; i < N; ++i) tp[i + 1] += tp[i];
+    std::vector<int32_t> tc(ctx->nnz);
+    std::vector<double> tv(ctx->nnz);
+    {
+        std::vector<int64_t> cur(tp.begin(), tp.end() - 1);
+        for (int64_t r = 0; r < N; ++r)
+            for (int64_t e = rp2[r]; e < rp2[r + 1]; ++e) {
+                const int64_t pos = cur[ci2[e]]++;
+                tc[pos] = (int32_t)r;
+                tv[pos] = va2[e];
+            }
+    }
+    {
+        HostEll hk, hkt;
+        csr_to_ell(N, rp2, ci2, va2, hk);
+        csr_to_ell(N, tp, tc, tv, hkt);
+        RDTRY(upload_ell(ctx, hk, ctx->K));
+        RDTRY(upload_ell(ctx, hkt, ctx->KT));
+    }
+    const size_t L = (size_t)ctx->ldw;
+    RDTRY(dalloc(ctx, &ctx->m, L));
+    RDTRY(dalloc(ctx, &ctx->minv, L));
+    RDTRY(dalloc(ctx, &ctx->d, L));
+    RDTRY(dalloc(ctx, &ctx->dinv, L));
+    {
+        std::vector<double> mi(N);
+        for (int64_t i = 0; i < N; ++i) mi[i] = 1.0 / mh[i];
+        CU(cudaMemcpyAsync(ctx->m, mh.data(), N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->minv, mi.data(), N * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    double** vecs[] = {&ctx->x, &ctx->r, &ctx->p0, &ctx->p1, &ctx->z, &ctx->w, &ctx->t, &ctx->b, &ctx->tmp, &ctx->Hy,
+                       &ctx->ell, &ctx->y, &ctx->ystate, &ctx->lam, &ctx->u, &ctx->in0, &ctx->in1};
+    for (double** v : vecs) RDTRY(dalloc(ctx, v, L));
+    RDTRY(dalloc(ctx, &ctx->act, L));
+    RDTRY(dalloc(ctx, &ctx->act_new, L));
+    RDTRY(dalloc(ctx, &ctx->hist, L));
+    RDTRY(dalloc(ctx, &ctx->act_stage, L));
+    RDTRY(dalloc(ctx, &ctx->bits, (size_t)(N + 7) / 8));
+    RDTRY(halloc(ctx, &ctx->h_bits, (size_t)(N + 7) / 8));
+    RDTRY(dalloc(ctx, &ctx->d_nactive, 1));
+    RDTRY(halloc(ctx, &ctx->h_nactive, 1));
+    RDTRY(dalloc(ctx, &ctx->d_cinfo, 1));
+    RDTRY(halloc(ctx, &ctx->h_cinfo, 1));
+    RDTRY(dalloc(ctx, &ctx->d_cgrep, 1));
+    RDTRY(halloc(ctx, &ctx->h_cgrep, 1));
+    RDTRY(dalloc(ctx, &ctx->d_cnt, 1));
+    RDTRY(halloc(ctx, &ctx->h_cnt, 1));
+    RDTRY(dalloc(ctx, &ctx->bar, 1));
+    // persistent Algorithm-1 kernel: one CTA per SM, all co-resident
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1, RD_CG_THREADS, 0));
+    if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1 does not fit an SM (occupancy 0)");
+    ctx->cg_grid = ctx->num_sms;
+    RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
+    // d = diag(H), dinv
+    k_diag_H<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+        ctx->KT.view(), N, ctx->m, ctx->minv, ctx->sigma, ctx->opt.jacobi, ctx->d, ctx->dinv);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_set_options(rd_ctx* ctx, const rd_options* opt)
+{
+    if (!ctx || !opt) return RD_EINVAL;
+    if ((opt->sigma_is_alpha != 0.0) != (ctx->opt.sigma_is_alpha != 0.0)) return fail(ctx, RD_EINVAL, "sigma_is_alpha is fixed at create");
+    const bool jac_changed = (opt->jacobi != 0) != (ctx->opt.jacobi != 0);
+    ctx->opt = *opt;
+    if (jac_changed) {
+        k_diag_H<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+            ctx->KT.view(), ctx->N, ctx->m, ctx->minv, ctx->sigma, ctx->opt.jacobi, ctx->d, ctx->dinv);
+        ctx->launches++;
+        CU(cudaGetLastError());
+    }
+    return RD_OK;
+}
+
+int rd_reset_sequence(rd_ctx* ctx)
+{
+    if (!ctx) return RD_EINVAL;
+    ctx->have_state = false;
+    CU(cudaMemsetAsync(ctx->ystate, 0, ctx->ldw * sizeof(double), ctx->stream));
+    CU(cudaMemsetAsync(ctx->act, 0, ctx->ldw, ctx->stream));
+    CU(cudaMemsetAsync(ctx->hist, 0, ctx->ldw, ctx->stream));
+    return RD_OK;
+}
+
+int rd_apply_K(rd_ctx* ctx, const double* v, double* out)
+{
+    if (!ctx || !v || !out) return RD_EINVAL;
+    const double* dv;
+    RDTRY(in_dev(ctx, v, ctx->N, ctx->in0, &dv));
+    double* dout = is_device_ptr(out) ? out : ctx->tmp;
+    k_apply_K<<<grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->K.view(), ctx->N, nullptr, dv, dout);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    RDTRY(out_host(ctx, out, dout, ctx->N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_apply_KT(rd_ctx* ctx, const double* v, double* out)
+{
+    if (!ctx || !v || !out) return RD_EINVAL;
+    const double* dv;
+    RDTRY(in_dev(ctx, v, ctx->N, ctx->in0, &dv));
+    double* dout = is_device_ptr(out) ? out : ctx->tmp;
+    k_apply_K<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->KT.view(), ctx->N, nullptr, dv, dout);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    RDTRY(out_host(ctx, out, dout, ctx->N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_apply_H(rd_ctx* ctx, const double* v, const uint8_t* active, double* out)
+{
+    if (!ctx || !v || !out) return RD_EINVAL;
+    const double* dv;
+    const uint8_t* da;
+    RDTRY(in_dev(ctx, v, ctx->N, ctx->in0, &dv));
+    RDTRY(in_dev(ctx, active, ctx->N, ctx->act_stage, &da));
+    double* dout = is_device_ptr(out) ? out : ctx->tmp;
+    const double* vin = dv;
+    if (da) {  // chi_I v
+        k_mask_copy<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->N, da, dv, ctx->in1);
+        ctx->launches++;
+        vin = ctx->in1;
+    }
+    RDTRY(launch_apply_H(ctx, vin, da, dout));
+    RDTRY(out_host(ctx, out, dout, ctx->N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_diag_H(rd_ctx* ctx, double* d_out)
+{
+    if (!ctx || !d_out) return RD_EINVAL;
+    RDTRY(out_host(ctx, d_out, ctx->d, ctx->N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W)
+{
+    if (!ctx || !W || k < 1 || k > RD_MAX_K) return RD_EINVAL;
+    RDTRY(alloc_reference(ctx, k));
+    CU(cudaMemsetAsync(ctx->W, 0, (size_t)ctx->ldw * ctx->kp * sizeof(double), ctx->stream));
+    CU(cudaMemcpy2DAsync(ctx->W, ctx->ldw * sizeof(double), W, ctx->N * sizeof(double), ctx->N * sizeof(double), k,
+                         cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->ref_ms_pending = 0.0;
+    return RD_OK;
+}
+
+int rd_get_reference(rd_ctx* ctx, double* W_out, int32_t* k_out)
+{
+    if (!ctx) return RD_EINVAL;
+    if (k_out) *k_out = ctx->W ? ctx->k : 0;
+    if (W_out && ctx->W && ctx->k > 0) {
+        CU(cudaMemcpy2DAsync(W_out, ctx->N * sizeof(double), ctx->W, ctx->ldw * sizeof(double), ctx->N * sizeof(double), ctx->k,
+                             cudaMemcpyDefault, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    return RD_OK;
+}
+
+int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* theta_out, double* resid_out,
+                       int32_t* iters_out)
+{
+    if (!ctx || k < 1 || k > RD_MAX_K || !(tol > 0.0) || max_block_iters < 1) return RD_EINVAL;
+    (void)theta_out; (void)resid_out; (void)iters_out;
+    return fail(ctx, RD_ECUDA, "rd_build_reference: not built yet");
+}
+
+int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C, int32_t* rank_used,
+                    double* cond_E, int32_t* fallback)
+{
+    if (!ctx || !active) return RD_EINVAL;
+    if (!ctx->W || ctx->k <= 0) return fail(ctx, RD_ENOREF, "no reference set");
+    const uint8_t* da;
+    RDTRY(in_dev(ctx, active, ctx->N, ctx->act_stage, &da));
+    CU(cudaMemcpyAsync(ctx->act, da, ctx->N, cudaMemcpyDeviceToDevice, ctx->stream));
+    RDTRY(coarse_setup(ctx, method, nullptr, nullptr));
+    const int kp = ctx->kp, k = ctx->k;
+    auto copy_kk = [&](double* dst, const double* src) -> int {
+        if (!dst) return RD_OK;
+        CU(cudaMemcpy2DAsync(dst, k * sizeof(double), src, kp * sizeof(double), k * sizeof(double), k, cudaMemcpyDefault, ctx->stream));
+        return RD_OK;
+    };
+    RDTRY(copy_kk(G, ctx->G));
+    RDTRY(copy_kk(EW, ctx->EW));
+    RDTRY(copy_kk(C, ctx->C));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (rank_used) *rank_used = ctx->h_cinfo->rank;
+    if (cond_E) *cond_E = ctx->h_cinfo->cond_E;
+    if (fallback) *fallback = ctx->h_cinfo->fallback;
+    return RD_OK;
+}
+
+int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const double* b, double* x, rd_solve_report* rep)
+{
+    if (!ctx || !active || !b || !x || !rep) return RD_EINVAL;
+    if (method < RD_JACOBI_CG || method > RD_ZEROEXT) return RD_EINVAL;
+    const int64_t N = ctx->N;
+    const uint8_t* da;
+    const double *db, *dx;
+    RDTRY(in_dev(ctx, active, N, ctx->act_stage, &da));
+    RDTRY(in_dev(ctx, b, N, ctx->in0, &db));
+    RDTRY(in_dev(ctx, (const double*)x, N, ctx->in1, &dx));
+    CU(cudaMemcpyAsync(ctx->act, da, N, cudaMemcpyDeviceToDevice, ctx->stream));
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    k_mask_copy<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, db, ctx->b);
+    k_mask_copy<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, dx, ctx->x);
+    CU(cudaMemsetAsync(ctx->d_nactive, 0, sizeof(int), ctx->stream));
+    k_pack_bits<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->bits, ctx->d_nactive);  // |J| for the bytes model
+    ctx->launches += 3;
+    CU(cudaMemcpyAsync(ctx->h_nactive, ctx->d_nactive, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    float msr = 0, msc = 0;
+    RDTRY(run_alg1(ctx, method, N - *ctx->h_nactive, rep, &msr, &msc));
+    RDTRY(out_host(ctx, x, ctx->x, N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return rep->status;
+}
+
+int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double* psi, const uint8_t* J0, double* y, double* u,
+                   double* lambda, rd_step_report* steps, uint8_t* J_bits, rd_query_report* rep)
+{
+    if (!ctx || !y_d || !psi || !y || !u || !steps || !rep) return RD_EINVAL;
+    if (method < RD_JACOBI_CG || method > RD_ZEROEXT) return RD_EINVAL;
+    if (ctx->opt.init == RD_INIT_GIVEN && !J0) return RD_EINVAL;
+    if (method != RD_JACOBI_CG && (!ctx->W || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
+    const auto t_begin = std::chrono::steady_clock::now();
+    const int64_t N = ctx->N;
+    const int64_t nbytes = (N + 7) / 8;
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    memset(rep, 0, sizeof *rep);
+    const double *dyd, *dpsi;
+    const uint8_t* dJ0;
+    RDTRY(in_dev(ctx, y_d, N, ctx->in0, &dyd));
+    RDTRY(in_dev(ctx, psi, N, ctx->in1, &dpsi));
+    RDTRY(in_dev(ctx, J0, N, ctx->act_stage, &dJ0));
+    k_ell<<<g, kThreads, 0, ctx->stream>>>(N, ctx->m, dyd, ctx->ell);
+    int init = ctx->opt.init;
+    if (init == RD_INIT_PAPER) init = ctx->have_state ? -1 : RD_INIT_ALL_ACTIVE;
+    if (!ctx->have_state) CU(cudaMemsetAsync(ctx->ystate, 0, ctx->ldw * sizeof(double), ctx->stream));
+    k_init_active<<<g, kThreads, 0, ctx->stream>>>(N, init, dJ0, dpsi, ctx->act);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+
+    std::vector<uint64_t> seen;
+    int status = RD_ESTEPS, nsteps = 0;
+    int64_t total_iters = 0;
+    // bits / count of the current active set
+    auto pack = [&]() -> int {
+        CU(cudaMemsetAsync(ctx->d_nactive, 0, sizeof(int), ctx->stream));
+        k_pack_bits<<<grid_for(nbytes, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->bits, ctx->d_nactive);
+        ctx->launches++;
+        CU(cudaMemcpyAsync(ctx->h_bits, ctx->bits, nbytes, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(ctx->h_nactive, ctx->d_nactive, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        return RD_OK;
+    };
+    RDTRY(pack());
+    for (int step = 0; step < ctx->opt.pdas_cap; ++step) {
+        rd_step_report* sr = &steps[step];
+        memset(sr, 0, sizeof *sr);
+        nsteps = step + 1;
+        sr->active_hash = fnv1a(ctx->h_bits, nbytes);
+        if (J_bits) memcpy(J_bits + (size_t)step * nbytes, ctx->h_bits, nbytes);
+        seen.push_back(sr->active_hash);
+        const int64_t n = N - *ctx->h_nactive;
+        sr->n_inactive = (int32_t)n;
+        CU(cudaEventRecord(ctx->ev[5], ctx->stream));
+        // y <- y_state, y_J <- psi_J ; tmp = chi_J psi ; x0 = chi_I y_state (warm inner start)
+        k_step_begin<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, dpsi, ctx->ystate, ctx->y, ctx->tmp, ctx->x);
+        ctx->launches++;
+        float ms_upd0 = 0, ms_upd1 = 0;
+        if (n > 0) {
+            RDTRY(launch_apply_H(ctx, ctx->tmp, nullptr, ctx->Hy));
+            k_rhs<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->ell, ctx->Hy, ctx->b);
+            ctx->launches++;
+            CU(cudaEventRecord(ctx->ev[6], ctx->stream));
+            rd_solve_report so;
+            float msr = 0, msc = 0;
+            RDTRY(run_alg1(ctx, method, n, &so, &msr, &msc));
+            CU(cudaEventElapsedTime(&ms_upd0, ctx->ev[5], ctx->ev[6]));
+            sr->cg_iters = so.iters; sr->rank_used = so.rank_used; sr->coarse_fallback = so.coarse_fallback;
+            sr->replacements = so.replacements; sr->status = so.status; sr->rel_resid_verified = so.rel_resid_verified;
+            sr->cond_E = so.cond_E; sr->t_restrict = msr; sr->t_coarse = msc; sr->t_iter = so.t_iter_ms;
+            total_iters += so.iters;
+            CU(cudaEventRecord(ctx->ev[5], ctx->stream));
+            k_scatter_solution<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->x, ctx->y);
+            ctx->launches++;
+        }
+        // lambda = l - H y on J, 0 on I; eq. (8)
+        RDTRY(launch_apply_H(ctx, ctx->y, nullptr, ctx->Hy));
+        CU(cudaMemsetAsync(ctx->d_cnt, 0, sizeof(PdasCounters), ctx->stream));
+        {
+            const unsigned long long inf_bits = 0x7ff0000000000000ULL;
+            CU(cudaMemcpyAsync(&ctx->d_cnt->margin_bits, &inf_bits, sizeof inf_bits, cudaMemcpyHostToDevice, ctx->stream));
+        }
+        k_pdas_update<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, ctx->ell, ctx->Hy, ctx->y, dpsi, ctx->d, ctx->opt.c_is_diag,
+                                                       ctx->lam, ctx->act_new, ctx->ystate, ctx->d_cnt);
+        ctx->launches++;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(PdasCounters), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaEventRecord(ctx->ev[7], ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        CU(cudaEventElapsedTime(&ms_upd1, ctx->ev[5], ctx->ev[7]));
+        sr->t_update = ms_upd0 + ms_upd1;
+        memcpy(&sr->margin, &ctx->h_cnt->margin_bits, sizeof(double));
+        if (ctx->h_cnt->changed == 0) { status = RD_OK; break; }
+        std::swap(ctx->act, ctx->act_new);
+        RDTRY(pack());
+        const uint64_t hn = fnv1a(ctx->h_bits, nbytes);
+        bool cyc = false;
+        for (uint64_t hsh : seen) cyc = cyc || (hsh == hn);
+        if (cyc) { status = RD_ECYCLE; break; }
+    }
+    ctx->have_state = true;
+    rep->n_steps = nsteps;
+    rep->status = status;
+    rep->total_cg_iters = total_iters;
+    // u = M^{-1} K y (eq. (9), f = 0), all state values incl. the active ones
+    k_apply_K<<<grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->minv, ctx->y, ctx->u);
+    ctx->launches++;
+    // KKT measures, eq. (25)
+    RDTRY(launch_apply_H(ctx, ctx->y, nullptr, ctx->Hy));
+    CU(cudaMemsetAsync(ctx->d_cnt, 0, sizeof(PdasCounters), ctx->stream));
+    k_kkt<<<g, kThreads, 0, ctx->stream>>>(N, ctx->ell, ctx->Hy, ctx->y, dpsi, ctx->lam, ctx->d_cnt);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(PdasCounters), cudaMemcpyDeviceToHost, ctx->stream));
+    RDTRY(out_host(ctx, y, ctx->y, N));
+    RDTRY(out_host(ctx, u, ctx->u, N));
+    if (lambda) RDTRY(out_host(ctx, lambda, ctx->lam, N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    double kk[6];
+    memcpy(kk, ctx->h_cnt->kkt_bits, sizeof kk);
+    const double s = std::max(1.0, kk[5]);
+    rep->kkt[0] = kk[0] / s; rep->kkt[1] = kk[1]; rep->kkt[2] = kk[2] / s; rep->kkt[3] = kk[3] / s; rep->kkt[4] = kk[4] / s;
+    rep->t_reference_charged = ctx->ref_ms_pending;
+    ctx->ref_ms_pending = 0.0;
+    rep->t_total = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count() + rep->t_reference_charged;
+    return status;
+}
+
+}  // extern "C"

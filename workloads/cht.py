@@ -311,7 +311,7 @@ TWINS: Dict[str, dict] = {
 }
 
 
-def make_config(config: int, n: Optional[int] = None, nt: Optional[int] = None, k: Optional[int] = None,
+def make_config(config: Optional[int] = None, n: Optional[int] = None, nt: Optional[int] = None, k: Optional[int] = None,
                 n_queries: Optional[int] = None, twin: Optional[str] = None) -> Workload:
     """Workload of BASELINE.json config `config` (1..5); n / nt / k override the size for twins."""
     if twin is not None:
