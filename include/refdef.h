@@ -122,13 +122,21 @@ int64_t rd_kernel_launches(const rd_ctx* ctx); /* CUDA kernels this context has 
 int rd_set_options(rd_ctx* ctx, const rd_options* opt); /* sigma_is_alpha cannot change after create (RD_EINVAL) */
 
 /* Steps 2-4 of Algorithm 2, BASELINE.json variant: the k lowest eigenpairs of the full
- * H by a Jacobi-preconditioned block iteration (LOBPCG) run until every
- * ||H w_j - theta_j w_j||_2 <= tol * theta_j (||w_j|| = 1) or max_block_iters block steps.  W is stored on
- * the device (N x k, orthonormal columns).  theta_out: k doubles, may be NULL.  resid_out: k doubles
- * (relative residuals reached), may be NULL.  iters_out: block steps used, may be NULL.
- * 1 <= k <= 64.  The time is remembered and charged to the next query. */
+ * H (the paper builds its reference once, before the sequence, and charges it to the first
+ * query).  Block Krylov method: Chebyshev-filtered subspace iteration on a block of
+ * b = k + max(8, k/4) vectors (rounded up to a multiple of 8) with Rayleigh-Ritz after every filter sweep,
+ * started from a fixed counter-based random block, run until every
+ * ||H w_j - theta_j w_j||_2 <= tol * theta_j (||w_j|| = 1, j < k) or max_block_iters sweeps (then RD_ECAP is
+ * returned and the best block so far is kept as the reference).  W is stored on the device (N x k,
+ * orthonormal columns).  theta_out: k doubles (ascending), may be NULL.  resid_out: k doubles (relative
+ * residuals reached), may be NULL.  iters_out: sweeps used, may be NULL.  All three are host pointers.
+ * 1 <= k <= 64, k <= N.  The wall time is remembered and charged to the next query.  W is unique only up to
+ * sign and rotation inside clusters: compare by eigenvalues and principal angles, never by columns. */
 int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* theta_out,
                        double* resid_out, int32_t* iters_out);
+/* Facts about the last rd_build_reference: block size b, total Chebyshev degree (each degree = one application
+ * of H to all b columns), wall milliseconds.  Any pointer may be NULL. */
+int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms);
 /* Inject a reference (e.g. the oracle's): W is N x k column-major with leading dimension N. */
 int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W);
 /* Copy the stored reference out: W_out N x k column-major (ld N); returns k via k_out (0 if none). */

@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
 
 
@@ -97,6 +97,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_kernel_launches.restype = i64
     lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
     lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
+    lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
     lib.rd_set_reference.argtypes = [vp, i32, vp]
     lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
     lib.rd_solve_query.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, C.POINTER(_StepReport), vp, C.POINTER(_QueryReport)]
@@ -115,6 +116,15 @@ def exported_symbols(path: Optional[str] = None):
     """Names from EXPORTS that the built library really exports (a CPU-side check; no CUDA call is made)."""
     lib = C.CDLL(path or LIB_PATH)
     return [s for s in EXPORTS if hasattr(lib, s)]
+
+
+def declared_in_header(path: Optional[str] = None):
+    """Names of the functions include/refdef.h declares (parsed from the header text)."""
+    import re
+
+    path = path or os.path.join(os.path.dirname(HERE), "include", "refdef.h")
+    text = re.sub(r"/\*.*?\*/", "", open(path).read(), flags=re.S)
+    return sorted(set(re.findall(r"\b(rd_[a-z_A-Z0-9]+)\s*\(", text)))
 
 
 def _ptr(a):
@@ -189,14 +199,20 @@ class RefDef:
         self._check(self._lib.rd_reset_sequence(self._h), "rd_reset_sequence")
 
     # ---- reference
-    def build_reference(self, k, tol=1e-3, max_block_iters=2000):
+    def build_reference(self, k, tol=1e-3, max_block_iters=200):
+        """Returns (theta, relative residuals, sweeps, status); status -6 = not converged within the sweeps."""
         theta = np.zeros(k)
         resid = np.zeros(k)
         it = C.c_int32(0)
-        self._check(self._lib.rd_build_reference(self._h, k, tol, max_block_iters, theta.ctypes.data, resid.ctypes.data,
-                                                 C.byref(it)), "rd_build_reference", soft_ok=True)
+        st = self._check(self._lib.rd_build_reference(self._h, k, tol, max_block_iters, theta.ctypes.data,
+                                                      resid.ctypes.data, C.byref(it)), "rd_build_reference", soft_ok=True)
         self.k = k
-        return theta, resid, it.value
+        return theta, resid, it.value, st
+
+    def reference_info(self):
+        b, deg, ms = C.c_int32(0), C.c_int64(0), C.c_double(0)
+        self._check(self._lib.rd_reference_info(self._h, C.byref(b), C.byref(deg), C.byref(ms)), "rd_reference_info")
+        return dict(block=b.value, total_degree=deg.value, build_ms=ms.value)
 
     def set_reference(self, W):
         """W: N x k, numpy (any order; copied column-major) or a column-major device tensor of shape (k, N)."""

@@ -75,7 +75,9 @@ struct rd_ctx {
     PdasCounters* h_cnt = nullptr;
     cudaEvent_t ev[8];
     bool have_state = false;
-    double ref_ms_pending = 0.0;
+    double ref_ms_pending = 0.0, ref_ms_last = 0.0;
+    int64_t ref_degree = 0;  // total Chebyshev degree of the last rd_build_reference
+    int ref_block = 0;       // its block size b
     int64_t launches = 0;  // kernels launched so far (rd_kernel_launches)
 };
 
@@ -626,8 +628,168 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
                        int32_t* iters_out)
 {
     if (!ctx || k < 1 || k > RD_MAX_K || !(tol > 0.0) || max_block_iters < 1) return RD_EINVAL;
-    (void)theta_out; (void)resid_out; (void)iters_out;
-    return fail(ctx, RD_ECUDA, "rd_build_reference: not built yet");
+    if (k > ctx->N) return fail(ctx, RD_EINVAL, "k = %d exceeds N = %lld", k, (long long)ctx->N);
+    const int64_t N = ctx->N, ld = ctx->ldw;
+    // block size: k plus a guard of max(8, k/4) vectors, a multiple of 8, never more than N rounded up
+    int b = (k + std::max(8, k / 4) + 7) & ~7;
+    while (b - 8 >= k && b > N) b -= 8;
+    const int nchunk = b / RD_EIG_CB;
+    const auto t_begin = std::chrono::steady_clock::now();
+
+    // ---- scratch of this call (released before returning)
+    struct Scratch {
+        std::vector<void*> p;
+        ~Scratch() { for (void* q : p) cudaFree(q); }
+    } scratch;
+    auto salloc = [&](double** out, size_t count) -> int {
+        void* q = nullptr;
+        cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, RD_ENOMEM, "cudaMalloc(%zu doubles): %s", count, cudaGetErrorString(e)); }
+        scratch.p.push_back(q);
+        cudaMemsetAsync(q, 0, std::max<size_t>(count, 1) * sizeof(double), ctx->stream);
+        *out = (double*)q;
+        return RD_OK;
+    };
+    const size_t nb = (size_t)ld * b;
+    double *P[4], *T, *parts, *Gs, *work, *Tm, *d_theta, *rparts, *rsum, *gersh;
+    for (auto& q : P) RDTRY(salloc(&q, nb));
+    RDTRY(salloc(&T, nb));
+    const int nparts = ctx->num_sms * 2;
+    RDTRY(salloc(&parts, (size_t)nparts * b * b));
+    RDTRY(salloc(&Gs, (size_t)b * b));
+    RDTRY(salloc(&work, (size_t)2 * b * b));
+    RDTRY(salloc(&Tm, (size_t)b * b));
+    RDTRY(salloc(&d_theta, b));
+    const int rgrid = ctx->num_sms * 2;
+    RDTRY(salloc(&rparts, (size_t)rgrid * b));
+    RDTRY(salloc(&rsum, b));
+    RDTRY(salloc(&gersh, 1));
+    std::vector<double> theta(b), res2(b), resid(b, INFINITY);
+
+    const int gs = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    const dim3 gblk(std::max(1, gs / std::min(nchunk, 4)), nchunk);
+    const dim3 ggram(nparts, (b + 63) / 64, (b + 63) / 64);
+    const int64_t bb = (int64_t)b * b;
+
+    // ---- upper bound of the spectrum
+    k_abs_rowsum<<<gs, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->minv, T);
+    k_gershgorin<<<gs, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->m, ctx->sigma, T, (unsigned long long*)gersh);
+    ctx->launches += 2;
+    double beta = 0.0;
+    CU(cudaMemcpyAsync(&beta, gersh, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (!(beta > 0.0) || !std::isfinite(beta)) return fail(ctx, RD_ENOTSPD, "spectrum bound %g", beta);
+    beta *= 1.0 + 1e-10;
+
+    auto block_apply = [&](const double* Y, double c1, double cshift, double c2, const double* Yprev, double* Ynext) {
+        k_blk_K<<<gblk, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y, T);
+        k_blk_KT<<<gblk, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y, T, Yprev, Ynext);
+        ctx->launches += 2;
+    };
+    auto gram = [&](const double* A, const double* B, double* out) {
+        k_gram_dmma<<<ggram, 256, 0, ctx->stream>>>(N, b, b, A, ld, B, ld, parts);
+        k_reduce_parts<<<grid_for(bb, kThreads, 64), kThreads, 0, ctx->stream>>>(nparts, bb, parts, out);
+        ctx->launches += 2;
+    };
+    const size_t smem_rm = (size_t)b * b * sizeof(double);
+    if (smem_rm > 48 * 1024) CU(cudaFuncSetAttribute(k_right_mult, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_rm));
+    auto right_mult = [&](const double* X, const double* M, double* Out) {
+        k_right_mult<<<grid_for(N, 256, big_grid(ctx)), 256, smem_rm, ctx->stream>>>(N, ld, b, b, X, M, Out);
+        ctx->launches++;
+    };
+
+    int cur = 0;  // P[cur] holds X
+    k_rand_block<<<grid_for(N * b, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(N, ld, b, 0x5EEDULL, P[cur]);
+    ctx->launches++;
+    int sweeps = 0, status = RD_ECAP;
+    int64_t total_degree = 0;
+    for (int sweep = 0; sweep < max_block_iters; ++sweep) {
+        sweeps = sweep + 1;
+        // orthonormalise twice (the second pass removes the cond^2 loss of the first)
+        for (int pass = 0; pass < 2; ++pass) {
+            const int nxt = (cur + 1) & 3;
+            gram(P[cur], P[cur], Gs);
+            k_orth_small<<<1, 1024, 0, ctx->stream>>>(b, Gs, work, Tm);
+            ctx->launches++;
+            right_mult(P[cur], Tm, P[nxt]);
+            cur = nxt;
+        }
+        // Rayleigh-Ritz
+        double* X = P[cur];
+        double* HX = P[(cur + 1) & 3];
+        block_apply(X, 1.0, 0.0, 0.0, nullptr, HX);
+        gram(X, HX, Gs);
+        k_rr_small<<<1, 1024, 0, ctx->stream>>>(b, Gs, work, Tm, d_theta);
+        ctx->launches++;
+        double* Xr = P[(cur + 2) & 3];
+        double* HXr = P[(cur + 3) & 3];
+        right_mult(X, Tm, Xr);
+        right_mult(HX, Tm, HXr);
+        k_resid_parts<<<rgrid, 256, 0, ctx->stream>>>(N, ld, b, Xr, HXr, d_theta, rparts);
+        k_reduce_parts<<<1, kThreads, 0, ctx->stream>>>(rgrid, b, rparts, rsum);
+        ctx->launches += 2;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(theta.data(), d_theta, b * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(res2.data(), rsum, b * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        cur = (cur + 2) & 3;  // X = Xr; HXr sits in P[(cur+1)&3]
+        bool ok = true;
+        for (int j = 0; j < b; ++j) {
+            if (!(theta[j] > 0.0) || !std::isfinite(theta[j])) return fail(ctx, RD_ENOTSPD, "Ritz value %d = %g", j, theta[j]);
+            resid[j] = std::sqrt(std::max(res2[j], 0.0)) / theta[j];
+            if (j < k && !(resid[j] <= tol)) ok = false;
+        }
+        if (ok) { status = RD_OK; break; }
+        if (sweep + 1 == max_block_iters) break;
+        // Chebyshev filter on [a, beta], scaled at lo (a lower estimate of theta_1), degree from the growth target
+        const double a = theta[b - 1];
+        const double abs_r0 = resid[0] * theta[0];
+        const double lo = std::max(0.0, theta[0] - abs_r0);
+        if (!(a < beta)) return fail(ctx, RD_ECUDA, "Ritz value %g above the spectrum bound %g", a, beta);
+        const double e = 0.5 * (beta - a), c = 0.5 * (beta + a);
+        const double growth = std::acosh((c - lo) / e);  // per degree, at lo, relative to the cut a
+        int deg = (int)std::ceil(std::log(1e4) / growth);
+        deg = std::max(8, std::min(deg, 200000));
+        total_degree += deg;
+        double sg = e / (lo - c);
+        const double tau = 2.0 / sg;
+        double* Y0 = P[cur];
+        double* Y1 = P[(cur + 1) & 3];
+        double* Y2 = P[(cur + 2) & 3];
+        block_apply(Y0, sg / e, c, 0.0, nullptr, Y1);
+        for (int j = 2; j <= deg; ++j) {
+            const double sn = 1.0 / (tau - sg);
+            block_apply(Y1, 2.0 * sn / e, c, -sg * sn, Y0, Y2);
+            double* tmp = Y0; Y0 = Y1; Y1 = Y2; Y2 = tmp;
+            sg = sn;
+        }
+        CU(cudaGetLastError());
+        for (int q = 0; q < 4; ++q) if (P[q] == Y1) cur = q;
+    }
+    // W <- the k lowest Ritz vectors (pad columns zero)
+    RDTRY(alloc_reference(ctx, k));
+    CU(cudaMemsetAsync(ctx->W, 0, (size_t)ld * ctx->kp * sizeof(double), ctx->stream));
+    CU(cudaMemcpyAsync(ctx->W, P[cur], (size_t)ld * k * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (theta_out) memcpy(theta_out, theta.data(), k * sizeof(double));
+    if (resid_out) memcpy(resid_out, resid.data(), k * sizeof(double));
+    if (iters_out) *iters_out = sweeps;
+    ctx->ref_degree = total_degree;
+    ctx->ref_block = b;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    if (status != RD_OK) fail(ctx, status, "reference not converged to tol %g in %d sweeps (worst residual %g)", tol, sweeps,
+                              *std::max_element(resid.begin(), resid.begin() + k));
+    return status;
+}
+
+int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms)
+{
+    if (!ctx) return RD_EINVAL;
+    if (block) *block = ctx->ref_block;
+    if (total_degree) *total_degree = ctx->ref_degree;
+    if (build_ms) *build_ms = ctx->ref_ms_last;
+    return RD_OK;
 }
 
 int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C, int32_t* rank_used,
