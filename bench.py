@@ -1,0 +1,433 @@
+#!/usr/bin/env python
+"""bench.py -- complete PDAS query time of the B200-native RefDef hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 1..5 | --twin NAME] [--method refdef|jacobi|zeroext] [--ref-tol T]
+
+A STEP is one complete optimization query of the config's sequence: S1-S7 of DESIGN.md for every PDAS step
+(restriction, coarse setup, Algorithm 1, multiplier / active-set update) plus recovery and KKT.  Queries run in
+sequence order under the paper's warm-start policy; when the sequence wraps, the context is reset
+and the reference is rebuilt (S0), its time charged to the first query of the new pass.  `value` is
+the mean complete time per query in seconds, reference builds inside the timed region included.
+
+The JSON line also carries
+  roofline      the persistent Algorithm-1 kernel: algorithmic bytes / CUDA-event time
+  cpu_baseline  the CPU oracle as it stands, timed on the host cores on a bounded sample (rank 0, N = 1)
+  e2e           the same metric through the C ABI with HOST buffers (H2D of y_d, psi and D2H of y, u, lambda inside)
+  clocks        nvidia-smi samples during the timed region
+
+Multi-GPU (torchrun, one rank per GPU): the path is one GPU by definition (BASELINE.json); ranks run independent
+replicas of the sequence on different query seeds ("replicas only", weak scaling), no data-path collective.
+`--impl reference` runs the oracle (test infrastructure) on the host cores for the same metric, rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METHODS = {"jacobi": 0, "refdef": 1, "zeroext": 2}
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+# ----------------------------------------------------------------------------------------------- helpers
+def algorithmic_bytes_per_iter(nnz: int, N: int, n: int, r: int) -> float:
+    """HBM bytes one Algorithm-1 loop iteration must move:
+    K and K^T once (8 B value + 4 B index per nonzero), t written and read on all N rows, 14 passes of
+    8 B over the n inactive rows, the two n x r passes over HW_I and W_I, one mask byte per row."""
+    return 24.0 * nnz + 16.0 * N + 112.0 * n + 16.0 * n * r + 1.0 * N
+
+
+def shard_queries(rank: int, world: int, n_queries: int):
+    """Replica r of `world` runs the config's sequence on its own seeds: query ids r*n .. r*n + n - 1."""
+    return [rank * n_queries + q for q in range(n_queries)]
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def reduce_max(values, backend_device=None):
+    """Max over ranks of a list of floats (torch.distributed all_reduce MAX); identity without a process group."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return list(values)
+    t = torch.tensor(list(values), dtype=torch.float64, device=backend_device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def reduce_sum(values, backend_device=None):
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return list(values)
+    t = torch.tensor(list(values), dtype=torch.float64, device=backend_device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t.cpu()]
+
+
+class ClockSampler:
+    """nvidia-smi samples of one GPU while the timed region runs (the recipe's clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def make_workload(args):
+    from workloads import make_config
+
+    if args.twin:
+        return make_config(twin=args.twin)
+    return make_config(args.config)
+
+
+def workload_name(args, w):
+    return f"{w.name}: {w.kind} CHT {'x'.join(map(str, w.dims))}" + (f" x{w.nt} slabs" if w.nt > 1 else "") + \
+           f", N={w.N}, k={w.k}, {w.n_queries} queries/sequence, PDAS cap {w.pdas_cap}"
+
+
+def load_profile():
+    p = os.path.join(ROOT, "profiles", "bench_workload_profile.json")
+    if os.path.exists(p):
+        return json.load(open(p))
+    return {}
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+class Sequence:
+    """The config's query sequence on one context: warm starts inside a pass, reset + reference rebuild on wrap."""
+
+    def __init__(self, g, w, method, ref_tol, qids):
+        self.g, self.w, self.method, self.ref_tol, self.qids = g, w, method, ref_tol, qids
+        self.pos = 0
+        self.ref_builds = 0
+        self.ref_ms = 0.0
+
+    def _target(self, q):
+        qid = self.qids[q]
+        yd = self.w._target(1000 * self.w.config + qid)
+        psi = np.full(self.w.N, self.w.psi_factor * float(yd.max()))
+        return yd, psi
+
+    def begin_pass(self):
+        self.g.reset_sequence()
+        if self.method != 0:
+            _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
+            info = self.g.reference_info()
+            self.ref_builds += 1
+            self.ref_ms += info["build_ms"]
+            self.ref_status = st
+
+    def next_inputs(self):
+        q = self.pos % len(self.qids)
+        return q, self._target(q)
+
+    def run(self, yd, psi, **kw):
+        if self.pos % len(self.qids) == 0:
+            self.begin_pass()
+        self.pos += 1
+        return self.g.solve_query(self.method, yd, psi, want_sets=False, **kw)
+
+
+def run_ours(args):
+    import torch
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    import paper_2606_17971_b200 as pkg
+
+    pkg.load_library()
+    w = make_workload(args)
+    method = METHODS[args.method]
+    stream = torch.cuda.current_stream()
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap), stream=stream.cuda_stream)
+    seq = Sequence(g, w, method, args.ref_tol, shard_queries(rank, world, w.n_queries))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step(host: bool):
+        """One query.  Device mode: inputs already resident in HBM, outputs stay there.  Host mode (e2e): numpy in/out."""
+        q, (yd, psi) = seq.next_inputs()
+        if not host:
+            yd_in, psi_in = torch.from_numpy(yd).to(dev), torch.from_numpy(psi).to(dev)
+        else:
+            yd_in, psi_in = yd, psi
+        flush.fill_(q & 0xFF)  # L2 flush between steps
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        res = seq.run(yd_in, psi_in)
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), res
+
+    for _ in range(args.warmup):
+        one_step(False)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    launches0 = g.kernel_launches()
+    builds0, refms0 = seq.ref_builds, seq.ref_ms
+    step_ms, results = [], []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        ms, res = one_step(False)
+        step_ms.append(ms)
+        results.append(res)
+    barrier()
+    wall_ms = (time.perf_counter() - t_wall0) * 1e3
+    clocks = sampler.stop()
+    launches = g.kernel_launches() - launches0
+    ref_builds, ref_ms = seq.ref_builds - builds0, seq.ref_ms - refms0
+    total_ms = sum(step_ms)
+
+    # ---- roofline of the dominant kernel (persistent Algorithm-1 kernel, one launch per PDAS step with I != {})
+    alg_bytes = alg_ms = 0.0
+    alg_launches = iters = 0
+    coarse_ms = upd_ms = 0.0
+    n_steps = 0
+    statuses = {}
+    for res in results:
+        statuses[res["status"]] = statuses.get(res["status"], 0) + 1
+        n_steps += res["n_steps"]
+        for s in res["steps"]:
+            coarse_ms += s["t_coarse"] + s["t_restrict"]
+            upd_ms += s["t_update"]
+            if s["n_inactive"] > 0:
+                alg_launches += 1
+                iters += s["cg_iters"]
+                alg_ms += s["t_iter"]
+                # + 3 applies outside the loop body (lines 3, 12, Verify) counted as iterations' worth of operator traffic
+                alg_bytes += algorithmic_bytes_per_iter(w.nnz, w.N, s["n_inactive"], s["rank_used"]) * s["cg_iters"]
+    peak, peak_src = load_peaks()
+    achieved = alg_bytes / (alg_ms * 1e-3) / 1e9 if alg_ms > 0 else 0.0
+    prof = load_profile().get(w.name, {})
+    roofline = {"kernel": "k_alg1 (persistent Algorithm-1 kernel: S3+S4+S5)", "bound": "hbm", "achieved": round(achieved, 1),
+                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                "traffic": prof.get("dram_bytes_per_launch"),
+                "bytes_per_launch": alg_bytes / max(alg_launches, 1), "ms_per_launch": alg_ms / max(alg_launches, 1),
+                "launches": alg_launches, "cg_iters": iters, "us_per_iter": 1e3 * alg_ms / max(iters, 1),
+                "share_of_step": round(alg_ms / total_ms, 4) if total_ms else None}
+
+    # ---- e2e: the same step with host buffers (one timed query; the context is already warm)
+    e2e_steps = max(1, args.e2e_steps)
+    e2e_ms = [one_step(True)[0] for _ in range(e2e_steps)]
+    h2d = 2 * 8 * w.N
+    d2h = 3 * 8 * w.N
+    mx_total, mx_e2e = reduce_max([total_ms, sum(e2e_ms)], dev if world > 1 else None)
+    tot_steps = reduce_sum([float(args.steps)], dev if world > 1 else None)[0]
+    value = mx_total * 1e-3 / tot_steps  # whole job: max-over-ranks time / queries all ranks processed
+    e2e_value = mx_e2e * 1e-3 / (e2e_steps * world)
+
+    out = None
+    if rank == 0:
+        out = {
+            "metric": "complete PDAS query time (incl. reference build)", "value": round(value, 4), "unit": "s/query",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(mx_total / args.steps, 3),
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": f"replicas x{world}",
+                       "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
+                       "l2": "flushed between steps (256 MiB write); the deflated working set (W, HW, K, K^T) exceeds L2"},
+            "e2e": {"value": round(e2e_value, 4), "unit": "s/query", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": roofline,
+            "breakdown": {"pdas_steps": n_steps, "query_status_counts": {str(k): v for k, v in statuses.items()},
+                          "reference_builds_in_timed_region": ref_builds, "reference_ms": round(ref_ms, 1),
+                          "alg1_ms": round(alg_ms, 1), "coarse_setup_ms": round(coarse_ms, 1), "update_ms": round(upd_ms, 1),
+                          "wall_ms_incl_host": round(wall_ms, 1)},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(args, w, g, method, iters / max(args.steps, 1), n_steps / max(args.steps, 1))
+    g.close()
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.destroy_process_group()
+    return out
+
+
+# ----------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, method, W, iters_per_query, steps_per_query, budget_s, seed_qid=0):
+    """Times the oracle, as it stands (single thread), on a bounded sample of one query of the workload: Algorithm 1
+    on the full inactive system of the first query (b = l), `cap` iterations, coarse setup included; the time per
+    iteration is scaled to a complete query with the CG iterations per query the CUDA arm observed."""
+    import oracle
+
+    o = oracle.Oracle.from_workload(w)
+    yd = w._target(1000 * w.config + seed_qid)
+    b = w.m * yd
+    idx = np.arange(w.N, dtype=np.int64)
+    Zt = W if (method != 0 and W is not None) else None
+    # calibrate: 4 iterations, then as many as fit the budget
+    t0 = time.perf_counter()
+    o.alg1(idx, b, np.zeros(w.N), Zt, cap=4)
+    t4 = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    o.alg1(idx, b, np.zeros(w.N), Zt, cap=12)
+    t12 = time.perf_counter() - t0
+    per_it = max((t12 - t4) / 8.0, 1e-9)
+    setup = max(t4 - 4 * per_it, 0.0)
+    cap = int(max(16, min(20000, (budget_s - setup) / per_it)))
+    t0 = time.perf_counter()
+    _, rep = o.alg1(idx, b, np.zeros(w.N), Zt, cap=cap)
+    t = time.perf_counter() - t0
+    done = max(rep["iters"], 1)
+    per_it = max((t - setup) / done, 1e-9)
+    per_query = per_it * iters_per_query + setup * steps_per_query
+    return per_query, dict(s_per_cg_iter=per_it, s_coarse_setup=setup, iters_timed=done, seconds_timed=t,
+                           iters_per_query=iters_per_query, steps_per_query=steps_per_query)
+
+
+def cpu_baseline(args, w, g, method, iters_per_query, steps_per_query):
+    W = g.get_reference() if method != 0 else None
+    v, d = oracle_sample(w, method, W, iters_per_query, steps_per_query, args.cpu_budget)
+    return {"value": round(v, 2), "unit": "s/query (extrapolated: measured s per CG iteration x the CG iterations per query of this run)",
+            "cores": 1, "kind": "oracle",
+            "sample": f"oracle Algorithm 1 ({args.method}) on the full-domain inactive system of query 0, {d['iters_timed']} iterations "
+                      f"timed in {d['seconds_timed']:.1f} s ({d['s_per_cg_iter'] * 1e3:.3f} ms/iteration, coarse setup "
+                      f"{d['s_coarse_setup']:.2f} s/PDAS step); scaled by {d['iters_per_query']:.0f} iterations and "
+                      f"{d['steps_per_query']:.0f} PDAS steps per query",
+            "detail": d}
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return None
+    import oracle
+
+    oracle.build_oracle()
+    w = make_workload(args)
+    method = METHODS[args.method]
+    prof = load_profile().get(w.name, {}).get(args.method, {})
+    iters_per_query = float(prof.get("cg_iters_per_query", 0.0))
+    steps_per_query = float(prof.get("pdas_steps_per_query", w.pdas_cap))
+    W = None
+    t_ref = 0.0
+    if method != 0:
+        t0 = time.perf_counter()
+        _, W = oracle.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+        t_ref = time.perf_counter() - t0
+    budget = max(2.0, min(args.cpu_budget, 240.0 / max(args.steps + args.warmup, 1)))
+    vals, detail = [], None
+    for i in range(args.warmup + args.steps):
+        v, detail = oracle_sample(w, method, W, iters_per_query or 1.0, steps_per_query, budget, seed_qid=i % w.n_queries)
+        if i >= args.warmup:
+            vals.append(v)
+    value = sum(vals) / len(vals) + t_ref / w.n_queries
+    if not iters_per_query:
+        unit_note = " (no recorded CG iterations per query for this workload: value is s per CG ITERATION-equivalent)"
+    else:
+        unit_note = ""
+    sample = (f"oracle Algorithm 1 ({args.method}) on the full-domain inactive system, {detail['iters_timed']} iterations per step "
+              f"({detail['s_per_cg_iter'] * 1e3:.3f} ms/iteration), scaled to a query by the recorded {iters_per_query:.0f} CG iterations "
+              f"and {steps_per_query:.0f} PDAS steps per query (profiles/bench_workload_profile.json); reference by a library "
+              f"eigensolver ({t_ref:.1f} s) charged over the {w.n_queries} queries of a pass{unit_note}")
+    return {"impl": "reference", "metric": "complete PDAS query time (incl. reference build)", "value": round(value, 2),
+            "unit": "s/query", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": round(1e3 * value, 1), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": "host cores, rank 0 only"},
+            "cpu_baseline": {"value": round(value, 2), "unit": "s/query", "kind": "oracle", "cores": 1, "sample": sample},
+            "e2e": {"value": round(value, 2), "unit": "s/query", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--twin", default=None)
+    ap.add_argument("--method", default="refdef", choices=list(METHODS))
+    ap.add_argument("--ref-tol", type=float, default=1e-3)
+    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    out = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
