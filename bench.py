@@ -322,6 +322,69 @@ def run_ours(args):
     return out
 
 
+def run_loop(args):
+    """--mode loop: the deflated-CG iteration loop alone (second half of BASELINE.json's metric: HBM GB/s of the loop
+    against peak).  One step = one Algorithm-1 solve (S1-S5) of the full-domain system H y = l of query 0 from a zero
+    start, at most --cg-cap iterations; the reference is built once, outside the timed region."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    import paper_2606_17971_b200 as pkg
+
+    pkg.load_library()
+    w = make_workload(args)
+    method = METHODS[args.method]
+    stream = torch.cuda.current_stream()
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, cg_cap=args.cg_cap), stream=stream.cuda_stream)
+    ref = None
+    if method != 0:
+        _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
+        ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
+    yd = w._target(1000 * w.config)
+    b = torch.from_numpy(w.m * yd).to(dev)
+    act = torch.zeros(w.N, dtype=torch.uint8, device=dev)
+    x0 = torch.zeros(w.N, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    reps = []
+    sampler = ClockSampler(0)
+    for i in range(args.warmup + args.steps):
+        if i == args.warmup:
+            torch.cuda.synchronize()
+            sampler.start()
+            launches0 = g.kernel_launches()
+        flush.fill_(i & 0xFF)
+        torch.cuda.synchronize()
+        _, rep = g.solve_inactive(method, act, b, x0)
+        if i >= args.warmup:
+            reps.append(rep)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launches = g.kernel_launches() - launches0
+    ms = sum(r["t_iter_ms"] for r in reps)
+    iters = sum(r["iters"] for r in reps)
+    nbytes = sum(algorithmic_bytes_per_iter(w.nnz, w.N, w.N, r["rank_used"]) * r["iters"] for r in reps)
+    peak, peak_src = load_peaks()
+    achieved = nbytes / (ms * 1e-3) / 1e9
+    prof = load_profile().get(w.name, {})
+    out = {"metric": "deflated-CG loop HBM throughput", "value": round(achieved, 1), "unit": "GB/s", "n_gpus": 1,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(args, w), "method": args.method, "mode": "loop", "cg_cap": args.cg_cap,
+                      "reference_tol": args.ref_tol, "l2": "flushed between steps (256 MiB write)"},
+           "gpu_launches": int(launches), "clocks": clocks,
+           "roofline": {"kernel": "k_alg1", "bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "peak_source": peak_src,
+                        "unit": "GB/s", "frac": round(achieved / peak, 4), "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
+                        "traffic": prof.get("dram_bytes_per_iter"), "bytes_per_iter": nbytes / max(iters, 1),
+                        "us_per_iter": 1e3 * ms / max(iters, 1), "cg_iters": iters, "rank": reps[-1]["rank_used"],
+                        "status": reps[-1]["status"]},
+           "reference": ref}
+    g.close()
+    return out
+
+
 # ----------------------------------------------------------------------------------------------- oracle legs
 def oracle_sample(w, method, W, iters_per_query, steps_per_query, budget_s, seed_qid=0):
     """Times the oracle, as it stands (single thread), on a bounded sample of one query of the workload: Algorithm 1
@@ -422,8 +485,16 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="query", choices=["query", "loop"], help="query: the metric; loop: the CG loop alone")
+    ap.add_argument("--cg-cap", type=int, default=500000, help="--mode loop: iteration cap of each solve")
+    ap.add_argument("--ref-sweeps", type=int, default=60, help="--mode loop: filter sweeps of the reference build")
     args = ap.parse_args(argv)
-    out = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.impl == "reference":
+        out = run_reference(args)
+    elif args.mode == "loop":
+        out = run_loop(args)
+    else:
+        out = run_ours(args)
     if out is not None:
         print(json.dumps(out), flush=True)
     return 0
