@@ -75,6 +75,9 @@ typedef struct {
     int32_t jacobi;        /* 1: J = diag(B)^{-1}; 0: identity */
     int32_t c_is_diag;     /* eq. (8): c_i = H_ii (1) or c = 1 (0, BASELINE.json configs) */
     int32_t init;          /* rd_init */
+    int32_t alg1_variant;  /* 0: projection carried in coefficient form, one pass over H_II W_I per iteration (default);
+                              1: the literal recurrence of Alg. 1 (passes over H_II W_I and W_I); same method, same results
+                              up to rounding */
 } rd_options;
 
 /* One PDAS step (one inactive system).  Times are milliseconds measured with CUDA events on the stream. */

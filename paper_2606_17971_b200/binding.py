@@ -33,7 +33,7 @@ class RefDefError(RuntimeError):
 class _Options(C.Structure):
     _fields_ = [("sigma_is_alpha", C.c_double), ("eps", C.c_double), ("eps_c", C.c_double), ("cg_cap", C.c_int32),
                 ("pdas_cap", C.c_int32), ("replace_period", C.c_int32), ("jacobi", C.c_int32),
-                ("c_is_diag", C.c_int32), ("init", C.c_int32)]
+                ("c_is_diag", C.c_int32), ("init", C.c_int32), ("alg1_variant", C.c_int32)]
 
 
 class _StepReport(C.Structure):
@@ -66,10 +66,11 @@ class Options:
     jacobi: int = 1
     c_is_diag: int = 0
     init: int = INIT_PAPER
+    alg1_variant: int = 0
 
     def c_struct(self) -> _Options:
         return _Options(self.sigma_is_alpha, self.eps, self.eps_c, self.cg_cap, self.pdas_cap, self.replace_period,
-                        self.jacobi, self.c_is_diag, self.init)
+                        self.jacobi, self.c_is_diag, self.init, self.alg1_variant)
 
 
 _lib = None

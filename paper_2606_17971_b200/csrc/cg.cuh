@@ -39,6 +39,7 @@ struct CgParams {
     double *x, *r, *p0, *p1, *z, *w, *t;
     const double *Wm, *HWm;  // chi_I W and chi_I H chi_I W, N x kp column-major (ld = ldw)
     const double* C;         // kp x kp column-major
+    const double* EW;        // W_I^T H_II W_I, kp x kp column-major (k_alg1_v2)
     double eps, eps_c;
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]

@@ -15,6 +15,7 @@
 
 #include "../../include/refdef.h"
 #include "cg.cuh"
+#include "cg2.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
 #include "pdas.cuh"
@@ -327,7 +328,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.m = ctx->m; P.minv = ctx->minv; P.dinv = ctx->dinv; P.sigma = ctx->sigma;
     P.act = ctx->act; P.b = ctx->b;
     P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
-    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.C = ctx->C;
+    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.C = ctx->C; P.EW = ctx->EW;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
     P.partial = ctx->partial; P.bar = ctx->bar; P.rep = ctx->d_cgrep;
     CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
@@ -336,7 +337,11 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
-    CU(cudaLaunchCooperativeKernel((const void*)k_alg1, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, 0, ctx->stream));
+    const bool v2 = ctx->opt.alg1_variant == 0;
+    if (v2)
+        CU(cudaLaunchCooperativeKernel((const void*)k_alg1_v2, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, sizeof(Cg2Shared), ctx->stream));
+    else
+        CU(cudaLaunchCooperativeKernel((const void*)k_alg1, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, 0, ctx->stream));
     ctx->launches++;
     CU(cudaEventRecord(ctx->ev[4], ctx->stream));
     CU(cudaMemcpyAsync(ctx->h_cgrep, ctx->d_cgrep, sizeof(CgDevReport), cudaMemcpyDeviceToHost, ctx->stream));
@@ -352,8 +357,9 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     // both ELL matrices once (8 B value + 4 B index per stored nonzero), t written and read on all N rows,
     // 14 vector passes over the n inactive rows, the two n x r passes over HW_I and W_I, the mask.
     const double rnk = use_coarse ? (double)rep->rank_used : 0.0;
+    // k_alg1_v2 (default) passes over HW_I only: 8 n r instead of 16 n r.
     rep->bytes_per_iter = 24.0 * (double)ctx->nnz + 16.0 * (double)N + 112.0 * (double)n_inactive +
-                          16.0 * (double)n_inactive * rnk + (double)N;
+                          (v2 ? 8.0 : 16.0) * (double)n_inactive * rnk + (double)N;
     return RD_OK;
 }
 
@@ -373,6 +379,7 @@ void rd_default_options(rd_options* o)
     o->jacobi = 1;
     o->c_is_diag = 0;
     o->init = RD_INIT_PAPER;
+    o->alg1_variant = 0;
 }
 
 const char* rd_last_error(const rd_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
@@ -508,6 +515,9 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1, RD_CG_THREADS, 0));
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1 does not fit an SM (occupancy 0)");
+    CU(cudaFuncSetAttribute(k_alg1_v2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Cg2Shared)));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1_v2, RD_CG_THREADS, sizeof(Cg2Shared)));
+    if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v2 does not fit an SM (occupancy 0)");
     ctx->cg_grid = ctx->num_sms;
     RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
     // d = diag(H), dinv

@@ -58,8 +58,10 @@ def test_default_options(lib_path):
     o = binding._Options()
     lib.rd_default_options(C.byref(o))
     d = pkg.Options()
-    assert (o.sigma_is_alpha, o.eps, o.eps_c, o.cg_cap, o.pdas_cap, o.replace_period, o.jacobi, o.c_is_diag, o.init) == \
-           (d.sigma_is_alpha, d.eps, d.eps_c, d.cg_cap, d.pdas_cap, d.replace_period, d.jacobi, d.c_is_diag, d.init)
+    assert (o.sigma_is_alpha, o.eps, o.eps_c, o.cg_cap, o.pdas_cap, o.replace_period, o.jacobi, o.c_is_diag, o.init,
+            o.alg1_variant) == \
+           (d.sigma_is_alpha, d.eps, d.eps_c, d.cg_cap, d.pdas_cap, d.replace_period, d.jacobi, d.c_is_diag, d.init,
+            d.alg1_variant)
 
 
 def test_product_never_imports_oracle():
