@@ -41,11 +41,13 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 
 
 # ----------------------------------------------------------------------------------------------- helpers
-def algorithmic_bytes_per_iter(nnz: int, N: int, n: int, r: int) -> float:
+def algorithmic_bytes_per_iter(nnz: int, N: int, n: int, r: int, tall_passes: int = 1) -> float:
     """HBM bytes one Algorithm-1 loop iteration must move:
     K and K^T once (8 B value + 4 B index per nonzero), t written and read on all N rows, 14 passes of
-    8 B over the n inactive rows, the two n x r passes over HW_I and W_I, one mask byte per row."""
-    return 24.0 * nnz + 16.0 * N + 112.0 * n + 16.0 * n * r + 1.0 * N
+    8 B over the n inactive rows, one mask byte per row, and `tall_passes` passes over an n x r tall-skinny
+    block: ONE (HW_I only) for the default kernel, which carries the projection in coefficient form; two
+    (HW_I and W_I) for the literal recurrence (alg1_variant = 1), which is what SURVEY.md 8(d) counted."""
+    return 24.0 * nnz + 16.0 * N + 112.0 * n + 8.0 * tall_passes * n * r + 1.0 * N
 
 
 def shard_queries(rank: int, world: int, n_queries: int):
@@ -208,7 +210,8 @@ def run_ours(args):
     w = make_workload(args)
     method = METHODS[args.method]
     stream = torch.cuda.current_stream()
-    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap), stream=stream.cuda_stream)
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant), stream=stream.cuda_stream)
+    tall = 2 if args.alg1_variant == 1 else 1
     seq = Sequence(g, w, method, args.ref_tol, shard_queries(rank, world, w.n_queries))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
@@ -272,7 +275,7 @@ def run_ours(args):
                 iters += s["cg_iters"]
                 alg_ms += s["t_iter"]
                 # + 3 applies outside the loop body (lines 3, 12, Verify) counted as iterations' worth of operator traffic
-                alg_bytes += algorithmic_bytes_per_iter(w.nnz, w.N, s["n_inactive"], s["rank_used"]) * s["cg_iters"]
+                alg_bytes += algorithmic_bytes_per_iter(w.nnz, w.N, s["n_inactive"], s["rank_used"], tall) * s["cg_iters"]
     peak, peak_src = load_peaks()
     achieved = alg_bytes / (alg_ms * 1e-3) / 1e9 if alg_ms > 0 else 0.0
     prof = load_profile().get(w.name, {})
@@ -300,7 +303,7 @@ def run_ours(args):
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(mx_total / args.steps, 3),
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": f"replicas x{world}",
-                       "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
+                       "alg1_variant": args.alg1_variant, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
                        "l2": "flushed between steps (256 MiB write); the deflated working set (W, HW, K, K^T) exceeds L2"},
             "e2e": {"value": round(e2e_value, 4), "unit": "s/query", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
@@ -338,7 +341,9 @@ def run_loop(args):
     w = make_workload(args)
     method = METHODS[args.method]
     stream = torch.cuda.current_stream()
-    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, cg_cap=args.cg_cap), stream=stream.cuda_stream)
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, cg_cap=args.cg_cap, alg1_variant=args.alg1_variant),
+                                 stream=stream.cuda_stream)
+    tall = 2 if args.alg1_variant == 1 else 1
     ref = None
     if method != 0:
         _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
@@ -365,14 +370,14 @@ def run_loop(args):
     launches = g.kernel_launches() - launches0
     ms = sum(r["t_iter_ms"] for r in reps)
     iters = sum(r["iters"] for r in reps)
-    nbytes = sum(algorithmic_bytes_per_iter(w.nnz, w.N, w.N, r["rank_used"]) * r["iters"] for r in reps)
+    nbytes = sum(algorithmic_bytes_per_iter(w.nnz, w.N, w.N, r["rank_used"], tall) * r["iters"] for r in reps)
     peak, peak_src = load_peaks()
     achieved = nbytes / (ms * 1e-3) / 1e9
     prof = load_profile().get(w.name, {})
     out = {"metric": "deflated-CG loop HBM throughput", "value": round(achieved, 1), "unit": "GB/s", "n_gpus": 1,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": workload_name(args, w), "method": args.method, "mode": "loop", "cg_cap": args.cg_cap,
+           "config": {"workload": workload_name(args, w), "method": args.method, "mode": "loop", "cg_cap": args.cg_cap, "alg1_variant": args.alg1_variant,
                       "reference_tol": args.ref_tol, "l2": "flushed between steps (256 MiB write)"},
            "gpu_launches": int(launches), "clocks": clocks,
            "roofline": {"kernel": "k_alg1", "bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "peak_source": peak_src,
@@ -487,6 +492,7 @@ def main(argv=None):
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default="query", choices=["query", "loop"], help="query: the metric; loop: the CG loop alone")
     ap.add_argument("--cg-cap", type=int, default=500000, help="--mode loop: iteration cap of each solve")
+    ap.add_argument("--alg1-variant", type=int, default=0, help="rd_options.alg1_variant (0: default kernel; 1: literal recurrence)")
     ap.add_argument("--ref-sweeps", type=int, default=60, help="--mode loop: filter sweeps of the reference build")
     args = ap.parse_args(argv)
     if args.impl == "reference":

@@ -52,11 +52,14 @@ def test_single_process_reductions_are_identity():
 
 
 def test_bytes_model():
-    # Jacobi-CG (r = 0) and deflated: the deflation adds exactly 16 n r bytes (two n x r passes)
+    # Jacobi-CG (r = 0) and deflated: the default kernel adds one n x r pass (8 n r bytes), the literal
+    # recurrence two (16 n r, the count of SURVEY.md 8(d))
     a = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=0)
     b = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=8)
+    c = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=8, tall_passes=2)
     assert a == 24 * 1000 + 16 * 200 + 112 * 150 + 200
-    assert b - a == 16 * 150 * 8
+    assert b - a == 8 * 150 * 8
+    assert c - a == 16 * 150 * 8
 
 
 def test_reference_arm_runs_on_cpu(capsys):
