@@ -75,9 +75,10 @@ typedef struct {
     int32_t jacobi;        /* 1: J = diag(B)^{-1}; 0: identity */
     int32_t c_is_diag;     /* eq. (8): c_i = H_ii (1) or c = 1 (0, BASELINE.json configs) */
     int32_t init;          /* rd_init */
-    int32_t alg1_variant;  /* 0: projection carried in coefficient form, one pass over H_II W_I per iteration (default);
-                              1: the literal recurrence of Alg. 1 (passes over H_II W_I and W_I); same method, same results
-                              up to rounding */
+    int32_t alg1_variant;  /* 0: projection carried in coefficient form, one pass over H_II W_I per iteration, operands
+                              staged through shared memory by TMA bulk copies (default);
+                              1: the literal recurrence of Alg. 1 (passes over H_II W_I and W_I), register-staged;
+                              2: coefficient form, register-staged.  Same method, same results up to rounding */
 } rd_options;
 
 /* One PDAS step (one inactive system).  Times are milliseconds measured with CUDA events on the stream. */
@@ -108,6 +109,10 @@ typedef struct {
     int32_t iters, rank_used, coarse_fallback, replacements, status;
     double rel_resid_verified, cond_E, t_iter_ms;
     double bytes_per_iter; /* algorithmic HBM bytes one loop iteration moves for this (N, n, nnz, rank) */
+    double t_stage_us[8];  /* alg1_variant 0: microseconds CTA 0 spent in  [0] stage A (K product)  [1] grid barrier
+                              [2] stage B (K^T product)  [3] grid barrier + reduction  [4] k x k coefficient updates
+                              [5] stage C (updates + H_II W_I pass)  [6] grid barrier + reduction  [7] outside the loop;
+                              zeros for the other variants */
 } rd_solve_report;
 
 void rd_default_options(rd_options* opt);

@@ -52,7 +52,8 @@ class _QueryReport(C.Structure):
 class _SolveReport(C.Structure):
     _fields_ = [("iters", C.c_int32), ("rank_used", C.c_int32), ("coarse_fallback", C.c_int32),
                 ("replacements", C.c_int32), ("status", C.c_int32), ("rel_resid_verified", C.c_double),
-                ("cond_E", C.c_double), ("t_iter_ms", C.c_double), ("bytes_per_iter", C.c_double)]
+                ("cond_E", C.c_double), ("t_iter_ms", C.c_double), ("bytes_per_iter", C.c_double),
+                ("t_stage_us", C.c_double * 8)]
 
 
 @dataclass
@@ -263,7 +264,9 @@ class RefDef:
         rep = _SolveReport()
         self._check(self._lib.rd_solve_inactive(self._h, method, _ptr(active), _ptr(b), _ptr(x), C.byref(rep)),
                     "rd_solve_inactive", soft_ok=True)
-        return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+        d = {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+        d["t_stage_us"] = list(rep.t_stage_us)
+        return x, d
 
     def coarse_setup(self, method, active):
         k = self.k

@@ -25,6 +25,7 @@ enum { SL_BB = 0, SL_DOT = 1, SL_RR = 2, SL_RHO = 3, SL_NSCAL = 4, SL_NSLOT = SL
 struct CgDevReport {
     int32_t iters, replacements, status, pad;
     double rel_resid_verified, bnorm, rr_last;
+    double t_stage_us[8];  // CTA 0's time per phase (k_alg1_v3): A, bar, B, bar, small dense, C, bar, outside the loop
 };
 
 struct CgParams {

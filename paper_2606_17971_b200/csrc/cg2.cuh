@@ -42,14 +42,15 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-struct Cg2Cta {
+template <class SH>
+struct Cg2CtaT {
     const CgParams& P;
-    Cg2Shared& sh;
+    SH& sh;
     int64_t s0, s1, row0, row1;
     unsigned int nbar;
     int G;
 
-    __device__ Cg2Cta(const CgParams& p, Cg2Shared& s) : P(p), sh(s), nbar(0)
+    __device__ Cg2CtaT(const CgParams& p, SH& s) : P(p), sh(s), nbar(0)
     {
         G = gridDim.x;
         const int64_t per = (P.K.nslices + G - 1) / G;
@@ -265,22 +266,34 @@ struct Cg2Cta {
         }
     }
 
-    // w = B v (both SpMVs with the barrier between them); v^T w goes to SL_DOT.
-    __device__ void apply_B_plain(const double* v)
+    // the two SpMVs of S3 over this CTA's slices (operator.cuh)
+    template <bool COMBINE>
+    __device__ void opK(const double* v0, const double* v1, double beta, double* pnew)
     {
-        stage_K<false>(P.K, P.N, s0, s1, P.minv, v, nullptr, 0.0, nullptr, P.t);
-        sync_fetch(false, false);
-        double d = stage_KT(P.KT, P.N, s0, s1, P.m, P.sigma, P.act, v, P.t, P.w);
-        d = block_sum(d, sh.red);
-        put(SL_DOT, d);
+        stage_K<COMBINE>(P.K, P.N, s0, s1, P.minv, v0, v1, beta, pnew, P.t);
     }
+    __device__ double opKT(const double* v) { return stage_KT(P.KT, P.N, s0, s1, P.m, P.sigma, P.act, v, P.t, P.w); }
+    __device__ void tick(int) {}
+    __device__ void finish(CgDevReport*) {}
 };
 
-__global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
+// w = B v (both SpMVs with the barrier between them); v^T w goes to SL_DOT.
+template <class CTA>
+__device__ __forceinline__ void apply_B_plain(CTA& cta, const double* v)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    Cg2Shared& sh = *reinterpret_cast<Cg2Shared*>(smem_raw);
-    Cg2Cta cta(P, sh);
+    cta.template opK<false>(v, nullptr, 0.0, nullptr);
+    cta.sync_fetch(false, false);
+    double d = cta.opKT(v);
+    d = block_sum(d, cta.sh.red);
+    cta.put(SL_DOT, d);
+}
+
+using Cg2Cta = Cg2CtaT<Cg2Shared>;
+
+// Algorithm 1, the whole solve; CTA supplies the stages (Cg2Cta here, Cg3Cta in cg3.cuh).
+template <class CTA, class SH>
+__device__ __forceinline__ void alg1_coeff_body(const CgParams& P, SH& sh, CTA& cta)
+{
     const bool coarse = P.use_coarse != 0;
     const int kp = P.kp;
     if (coarse)
@@ -295,12 +308,12 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
         cta.put(SL_BB, bb);
     }
     // line 3: x <- x0 + Q (b - B x0);  r <- b - B x
-    stage_K<false>(P.K, P.N, cta.s0, cta.s1, P.minv, P.x, nullptr, 0.0, nullptr, P.t);
+    cta.template opK<false>(P.x, nullptr, 0.0, nullptr);
     cta.sync_fetch(true, false);
     const double bnorm = sqrt(sh.scal[SL_BB]);
     const double tau = (bnorm > 0.0) ? P.eps_c * bnorm : P.eps_c;
     __syncthreads();
-    (void)stage_KT(P.KT, P.N, cta.s0, cta.s1, P.m, P.sigma, P.act, P.x, P.t, P.w);
+    (void)cta.opKT(P.x);
     int status = RD_ECAP_DEV;
     int iters = 0, replacements = 0;
     bool done = false;
@@ -314,7 +327,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
         cta.small_matvec(sh.C, sh.c, sh.mu);
         cta.stage_add_W(sh.mu, 1.0);  // x += W_I C W_I^T r
         cta.sync_fetch(false, false);
-        cta.apply_B_plain(P.x);
+        apply_B_plain(cta, P.x);
     }
     cta.stage_recompute(P.HWm, true);  // r = b - B x, z~ = J r, ||r||^2, r^T z~, c = (HW_I)^T z~
     cta.sync_fetch(true, coarse);
@@ -323,6 +336,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
     bool restart = true;  // line 7 / line 20: p <- z, i.e. p~ = z~, nu = mu, g = c, s = 0
     double rho_prime = sh.scal[SL_RHO];
     // line 8
+    cta.tick(7);
     while (!done && iters < P.cap) {
         // ---- coefficient part of lines 7 / 20 / 22-23
         if (coarse) {
@@ -346,19 +360,24 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
             rho = rho_prime;
         }
         restart = false;
+        cta.tick(4);
         // ---- stage A: line 23 fused into line 9's first product
         double* pold = cur ? P.p1 : P.p0;
         double* pnew = cur ? P.p0 : P.p1;
-        stage_K<true>(P.K, P.N, cta.s0, cta.s1, P.minv, P.z, pold, beta, pnew, P.t);
+        cta.template opK<true>(P.z, pold, beta, pnew);
         cur ^= 1;
+        cta.tick(0);
         cta.sync_fetch(false, false);
+        cta.tick(1);
         // ---- stage B
         {
-            double d = stage_KT(P.KT, P.N, cta.s0, cta.s1, P.m, P.sigma, P.act, pnew, P.t, P.w);
+            double d = cta.opKT(pnew);
             d = block_sum(d, sh.red);
             cta.put(SL_DOT, d);
         }
+        cta.tick(2);
         cta.sync_fetch(true, false);
+        cta.tick(3);
         iters++;
         double pw = sh.scal[SL_DOT];
         if (coarse) {
@@ -379,11 +398,15 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
             }
             __syncthreads();
             x_split = true;
+            cta.tick(4);
             cta.stage_update_coarse(a, pnew);
         } else {
+            cta.tick(4);
             cta.stage_update_plain(a, pnew);
         }
+        cta.tick(5);
         cta.sync_fetch(true, coarse);
+        cta.tick(6);
         rho_prime = sh.scal[SL_RHO];
         // line 11
         const bool scheduled = P.replace_period > 0 && (iters % P.replace_period) == 0;
@@ -397,7 +420,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
                 cta.sync_fetch(false, false);
             }
             // line 12: recompute r = b - B x
-            cta.apply_B_plain(P.x);
+            apply_B_plain(cta, P.x);
             cta.stage_recompute(coarse ? P.Wm : P.HWm, !coarse);
             cta.sync_fetch(true, coarse);
             if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 13-15
@@ -406,7 +429,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
                 cta.small_matvec(sh.C, sh.c, sh.mu);
                 cta.stage_add_W(sh.mu, 1.0);
                 cta.sync_fetch(false, false);
-                cta.apply_B_plain(P.x);
+                apply_B_plain(cta, P.x);
                 cta.stage_recompute(P.HWm, true);
                 cta.sync_fetch(true, true);
                 if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 17-19
@@ -422,7 +445,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
         cta.stage_add_W(sh.xi, -1.0);
         cta.sync_fetch(false, false);
     }
-    cta.apply_B_plain(P.x);
+    apply_B_plain(cta, P.x);
     cta.stage_recompute(nullptr, false);
     cta.sync_fetch(true, false);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -435,7 +458,17 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
         P.rep->rel_resid_verified = rel;
         P.rep->bnorm = bnorm;
         P.rep->rr_last = rr_last;
+        cta.tick(7);
+        cta.finish(P.rep);
     }
+}
+
+__global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v2(const CgParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Cg2Shared& sh = *reinterpret_cast<Cg2Shared*>(smem_raw);
+    Cg2Cta cta(P, sh);
+    alg1_coeff_body(P, sh, cta);
 }
 
 }  // namespace rd

@@ -1,0 +1,321 @@
+// cg3.cuh -- k_alg1_v3: Algorithm 1 in the coefficient form of cg2.cuh, with every streamed
+// operand staged through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier, async.cuh) instead of
+// register loads.  Default kernel of the library (rd_options.alg1_variant = 0).
+//
+// Why: the loop is HBM-bound (DESIGN.md bytes model) and a register-staged kernel at 64 registers per thread
+// cannot keep enough bytes in flight: every 32-row tile of the HW_I pass waited on its own loads.  Here
+//   stage C  the n x kp block HW_I streams through a ring of NST = min(32, 512/kp) tiles of 32 rows x kp columns
+//            (256 kp bytes each, 128 KB in total); consumer warp cw owns ring slot cw and its mbarrier, processes
+//            tiles cw, cw + NST, ... and refills its slot as soon as its lanes have read it.  A tile is consumed
+//            by ONE warp in two passes over shared memory: lane = row for q_i = sum_j HW_ij (a nu_j) and the
+//            row updates, then lane = column for c_j += sum_i HW_ij z~_i, rows visited in a skewed order
+//            (i + lane) mod 32 so that the transposed reads are bank-conflict free.  No cross-warp exchange.
+//   stage A/B the sliced-ELL streams of K and K^T: every warp prefetches the values and column indices of its
+//            next 32-row slice into its own 4 KB slot while it gathers for the current one.
+// The arithmetic per row and all reduction orders are fixed, so results are bit-reproducible run to run.
+#pragma once
+#include "async.cuh"
+#include "cg2.cuh"
+
+namespace rd {
+
+#define RD_RING_BYTES (128 * 1024)
+#define RD_SPMV_WD 8             // ELL entries per row that the staged SpMV path holds (wider slices: direct loads)
+#define RD_SPMV_SLOT_BYTES 4096  // per warp: values 8 x 256 B, then indices 8 x 128 B
+
+struct __align__(128) Cg3Shared {
+    double C[RD_MAX_K * RD_MAX_K];
+    double EW[RD_MAX_K * RD_MAX_K];
+    double s[RD_CG_THREADS];  // transposition buffer of stage_recompute (outside the loop)
+    double zb[32][32];        // stage C: z~ of the warp's tile, for the transposed pass
+    double cpart[512];        // stage C: c partials of the consumer warps, NST x kp <= 512
+    double c[RD_MAX_K], mu[RD_MAX_K], nu[RD_MAX_K], g[RD_MAX_K], sv[RD_MAX_K], xi[RD_MAX_K], anu[RD_MAX_K], e[RD_MAX_K];
+    double scal[SL_NSCAL];
+    double small[4];
+    double red[32];
+    uint64_t full[32];  // one mbarrier per warp
+    uint64_t tacc[8];
+    uint64_t tlast;
+    __align__(128) unsigned char ring[RD_RING_BYTES];  // written by the async proxy only
+};
+
+struct Cg3Cta : Cg2CtaT<Cg3Shared> {
+    using Base = Cg2CtaT<Cg3Shared>;
+    uint32_t ph;  // phase parity of this warp's mbarrier (uniform in the warp)
+
+    __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : Base(p, s), ph(0)
+    {
+        if (threadIdx.x == 0) {
+            for (int w = 0; w < 32; ++w) mbar_init(&sh.full[w], 1);
+            mbar_fence_init();
+            for (int q = 0; q < 8; ++q) sh.tacc[q] = 0;
+            sh.tlast = global_timer_ns();
+        }
+        __syncthreads();
+    }
+
+    __device__ void tick(int slot)
+    {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            const uint64_t t = global_timer_ns();
+            sh.tacc[slot] += t - sh.tlast;
+            sh.tlast = t;
+        }
+    }
+    __device__ void finish(CgDevReport* rep)
+    {
+        for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = 1e-3 * (double)sh.tacc[q];
+    }
+
+    // ---- staged sliced-ELL product over this CTA's slices; epi(row, acc) consumes sum_e A[row,e] vin[col_e]
+    template <bool COMBINE, class Epi>
+    __device__ __forceinline__ void spmv_staged(const Ell& A, const double* v0, const double* v1, double beta, Epi epi)
+    {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        unsigned char* slot_ = sh.ring + warp * RD_SPMV_SLOT_BYTES;
+        const double* sval = reinterpret_cast<const double*>(slot_);
+        const int32_t* scol = reinterpret_cast<const int32_t*>(slot_ + RD_SPMV_WD * 256);
+        uint64_t* bar = &sh.full[warp];
+        auto issue = [&](int64_t o, int wd) {
+            if (lane == 0) {
+                mbar_arrive_expect_tx(bar, (uint32_t)wd * 384u);
+                if (wd > 0) {
+                    bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
+                    bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
+                }
+            }
+        };
+        int64_t s = s0 + warp;
+        int64_t o = 0;
+        int wd = 0;
+        if (s < s1) {
+            o = A.off[s];
+            wd = (int)((A.off[s + 1] - o) >> 5);
+            if (wd <= RD_SPMV_WD) issue(o, wd);
+        }
+        for (; s < s1; s += 32) {
+            const int64_t sn = s + 32;
+            int64_t on = 0;
+            int wdn = 0;
+            if (sn < s1) {
+                on = A.off[sn];
+                wdn = (int)((A.off[sn + 1] - on) >> 5);
+            }
+            double acc = 0.0;
+            if (wd <= RD_SPMV_WD) {
+                mbar_wait(bar, ph);
+                ph ^= 1u;
+                int cc[RD_SPMV_WD];
+                double aa[RD_SPMV_WD];
+#pragma unroll
+                for (int q = 0; q < RD_SPMV_WD; ++q) {
+                    const bool ok = q < wd;
+                    cc[q] = ok ? scol[q * 32 + lane] : 0;
+                    aa[q] = ok ? sval[q * 32 + lane] : 0.0;
+                }
+                __syncwarp();
+                if (sn < s1 && wdn <= RD_SPMV_WD) issue(on, wdn);
+                double xx[RD_SPMV_WD];
+#pragma unroll
+                for (int q = 0; q < RD_SPMV_WD; ++q) xx[q] = (q < wd) ? v0[cc[q]] : 0.0;
+                if (COMBINE) {
+#pragma unroll
+                    for (int q = 0; q < RD_SPMV_WD; ++q)
+                        if (q < wd) xx[q] = fma(beta, v1[cc[q]], xx[q]);
+                }
+#pragma unroll
+                for (int q = 0; q < RD_SPMV_WD; ++q) acc = fma(aa[q], xx[q], acc);
+            } else {
+                if (sn < s1 && wdn <= RD_SPMV_WD) issue(on, wdn);
+                acc = ell_row_dot<COMBINE>(A, s, lane, v0, v1, beta);
+            }
+            epi(s * RD_SLICE + lane, acc);
+            o = on;
+            wd = wdn;
+        }
+    }
+
+    // stage A: t = M^{-1} K (v0 + beta v1), pnew = v0 + beta v1 on this CTA's rows  (Alg. 1 lines 23 + 9)
+    template <bool COMBINE>
+    __device__ void opK(const double* v0, const double* v1, double beta, double* pnew)
+    {
+        const int64_t N = P.N;
+        const double* minv = P.minv;
+        double* t = P.t;
+        spmv_staged<COMBINE>(P.K, v0, v1, beta, [&](int64_t row, double acc) {
+            if (row < N) {
+                t[row] = acc * ldg_f64(minv + row);
+                if (pnew) {
+                    double x = v0[row];
+                    if (COMBINE) x = fma(beta, v1[row], x);
+                    pnew[row] = x;
+                }
+            }
+        });
+    }
+    // stage B: w = chi_I (m.v + sigma K^T t); returns this thread's partial of v^T w  (Alg. 1 line 9)
+    __device__ double opKT(const double* v)
+    {
+        const int64_t N = P.N;
+        const double* m = P.m;
+        const uint8_t* act = P.act;
+        const double sigma = P.sigma;
+        double* w = P.w;
+        double dot = 0.0;
+        spmv_staged<false>(P.KT, P.t, nullptr, 0.0, [&](int64_t row, double acc) {
+            if (row < N) {
+                const double vi = v[row];
+                double wi = fma(sigma, acc, ldg_f64(m + row) * vi);
+                if (act && act[row]) wi = 0.0;
+                w[row] = wi;
+                dot = fma(vi, wi, dot);
+            }
+        });
+        return dot;
+    }
+
+    // Stage C without a coarse space (rank-zero execution = Jacobi-CG): two rows per thread in flight
+    __device__ void stage_update_plain(double a, const double* p)
+    {
+        double rr = 0.0, rho = 0.0;
+        __syncthreads();
+        const int64_t step = 2 * (int64_t)blockDim.x;
+        for (int64_t i0 = row0 + threadIdx.x; i0 < row1; i0 += step) {
+            const int64_t i1 = i0 + blockDim.x;
+            const bool in1 = i1 < row1;
+            const double w0 = P.w[i0], r0 = P.r[i0], d0 = ldg_f64(P.dinv + i0), p0 = p[i0], x0 = P.x[i0];
+            double w1 = 0.0, r1 = 0.0, d1 = 0.0, p1 = 0.0, x1 = 0.0;
+            if (in1) { w1 = P.w[i1]; r1 = P.r[i1]; d1 = ldg_f64(P.dinv + i1); p1 = p[i1]; x1 = P.x[i1]; }
+            const double rn0 = fma(-a, w0, r0), zn0 = rn0 * d0;
+            P.x[i0] = fma(a, p0, x0);
+            P.r[i0] = rn0;
+            P.z[i0] = zn0;
+            rr = fma(rn0, rn0, rr);
+            rho = fma(rn0, zn0, rho);
+            if (in1) {
+                const double rn1 = fma(-a, w1, r1), zn1 = rn1 * d1;
+                P.x[i1] = fma(a, p1, x1);
+                P.r[i1] = rn1;
+                P.z[i1] = zn1;
+                rr = fma(rn1, rn1, rr);
+                rho = fma(rn1, zn1, rho);
+            }
+        }
+        rr = block_sum(rr, sh.red);
+        rho = block_sum(rho, sh.red);
+        put(SL_RR, rr);
+        put(SL_RHO, rho);
+    }
+
+    // Stage C with a coarse space: one pass over HW_I through the shared-memory ring (header comment).
+    //   r_i  <- r_i - a w~_i + sum_j HW_ij (a nu_j)      x~_i <- x~_i + a p~_i      z~_i <- r_i / d_i
+    //   ||r||^2, r^T z~,  c_j = sum_i HW_ij z~_i                                      (eq. (18))
+    __device__ void stage_update_coarse(double a, const double* p)
+    {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const int kp = P.kp;
+        const uint32_t tile_bytes = 256u * (uint32_t)kp;
+        const int nst = min(32, (int)(RD_RING_BYTES / tile_bytes));
+        const int64_t ntiles = (row1 - row0 + 31) >> 5;
+        double rr = 0.0, rho = 0.0;
+        double acc[(RD_MAX_K + 31) / 32];
+#pragma unroll
+        for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) acc[q] = 0.0;
+        __syncthreads();  // w~ of this CTA's rows was written by other threads of the CTA; anu is in place
+        if (warp < nst) {
+            double* tile = reinterpret_cast<double*>(sh.ring + (size_t)warp * tile_bytes);
+            uint64_t* bar = &sh.full[warp];
+            double* zbw = sh.zb[warp];
+            const double* anu = sh.anu;
+            auto issue = [&](int64_t t) {
+                const double* src = P.HWm + row0 + 32 * t;
+                if (lane == 0) mbar_arrive_expect_tx(bar, tile_bytes);
+                __syncwarp();
+                for (int j = lane; j < kp; j += 32) bulk_g2s(tile + j * 32, src + (size_t)j * P.ldw, 256u, bar);
+            };
+            int64_t t = warp;
+            double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi = 0.0;
+            if (t < ntiles) {
+                issue(t);
+                const int64_t i = row0 + 32 * t + lane;
+                if (i < row1) { ri = P.r[i]; wi = P.w[i]; di = ldg_f64(P.dinv + i); pi = p[i]; xi = P.x[i]; }
+            }
+            for (; t < ntiles; t += nst) {
+                const int64_t i = row0 + 32 * t + lane;
+                const bool in = i < row1;
+                // next tile's row data: in flight while this tile is processed
+                const int64_t tn = t + nst;
+                const int64_t inx = row0 + 32 * tn + lane;
+                double rin = 0.0, win = 0.0, din = 0.0, pin = 0.0, xin = 0.0;
+                if (tn < ntiles && inx < row1) { rin = P.r[inx]; win = P.w[inx]; din = ldg_f64(P.dinv + inx); pin = p[inx]; xin = P.x[inx]; }
+                mbar_wait(bar, ph);
+                ph ^= 1u;
+                // pass 1: lane = row
+                double q0 = 0.0, q1 = 0.0, q2 = 0.0, q3 = 0.0;
+                const double* trow = tile + lane;
+#pragma unroll 2
+                for (int j = 0; j < kp; j += 4) {
+                    q0 = fma(trow[(j + 0) * 32], anu[j + 0], q0);
+                    q1 = fma(trow[(j + 1) * 32], anu[j + 1], q1);
+                    q2 = fma(trow[(j + 2) * 32], anu[j + 2], q2);
+                    q3 = fma(trow[(j + 3) * 32], anu[j + 3], q3);
+                }
+                const double rn = fma(-a, wi, ri) + ((q0 + q1) + (q2 + q3));
+                const double zn = in ? rn * di : 0.0;
+                if (in) {
+                    P.r[i] = rn;
+                    P.x[i] = fma(a, pi, xi);
+                    P.z[i] = zn;
+                    rr = fma(rn, rn, rr);
+                    rho = fma(rn, zn, rho);
+                }
+                zbw[lane] = zn;
+                __syncwarp();
+                // pass 2: lane = column, rows in the skewed order (ii + lane) mod 32
+#pragma unroll
+                for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) {
+                    const int j = lane + 32 * q;
+                    if (j < kp) {
+                        const double* tcol = tile + j * 32;
+                        double a0 = 0.0, a1 = 0.0;
+#pragma unroll 8
+                        for (int ii = 0; ii < 32; ii += 2) {
+                            const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
+                            a0 = fma(tcol[r0], zbw[r0], a0);
+                            a1 = fma(tcol[r1], zbw[r1], a1);
+                        }
+                        acc[q] += a0 + a1;
+                    }
+                }
+                __syncwarp();  // every lane has read the tile and zb
+                if (tn < ntiles) issue(tn);
+                ri = rin; wi = win; di = din; pi = pin; xi = xin;
+            }
+#pragma unroll
+            for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) {
+                const int j = lane + 32 * q;
+                if (j < kp) sh.cpart[warp * kp + j] = acc[q];
+            }
+        }
+        __syncthreads();
+        if ((int)threadIdx.x < kp) {
+            double v = 0.0;
+            for (int cw = 0; cw < nst; ++cw) v += sh.cpart[cw * kp + threadIdx.x];
+            slot(SL_NSCAL + threadIdx.x)[blockIdx.x] = v;
+        }
+        rr = block_sum(rr, sh.red);
+        rho = block_sum(rho, sh.red);
+        put(SL_RR, rr);
+        put(SL_RHO, rho);
+    }
+};
+
+__global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Cg3Shared& sh = *reinterpret_cast<Cg3Shared*>(smem_raw);
+    Cg3Cta cta(P, sh);
+    alg1_coeff_body(P, sh, cta);
+}
+
+}  // namespace rd

@@ -16,6 +16,7 @@
 #include "../../include/refdef.h"
 #include "cg.cuh"
 #include "cg2.cuh"
+#include "cg3.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
 #include "pdas.cuh"
@@ -337,8 +338,11 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
-    const bool v2 = ctx->opt.alg1_variant == 0;
-    if (v2)
+    const int variant = ctx->opt.alg1_variant;
+    const bool v2 = variant != 1;  // coefficient form: one n x r pass per iteration
+    if (variant == 0)
+        CU(cudaLaunchCooperativeKernel((const void*)k_alg1_v3, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, sizeof(Cg3Shared), ctx->stream));
+    else if (variant == 2)
         CU(cudaLaunchCooperativeKernel((const void*)k_alg1_v2, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, sizeof(Cg2Shared), ctx->stream));
     else
         CU(cudaLaunchCooperativeKernel((const void*)k_alg1, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, 0, ctx->stream));
@@ -353,6 +357,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     rep->status = ctx->h_cgrep->status;
     rep->rel_resid_verified = ctx->h_cgrep->rel_resid_verified;
     rep->t_iter_ms = ms;
+    for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = (variant == 0) ? ctx->h_cgrep->t_stage_us[q] : 0.0;
     // algorithmic HBM bytes of one loop iteration:
     // both ELL matrices once (8 B value + 4 B index per stored nonzero), t written and read on all N rows,
     // 14 vector passes over the n inactive rows, the two n x r passes over HW_I and W_I, the mask.
@@ -518,6 +523,9 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     CU(cudaFuncSetAttribute(k_alg1_v2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Cg2Shared)));
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1_v2, RD_CG_THREADS, sizeof(Cg2Shared)));
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v2 does not fit an SM (occupancy 0)");
+    CU(cudaFuncSetAttribute(k_alg1_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Cg3Shared)));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1_v3, RD_CG_THREADS, sizeof(Cg3Shared)));
+    if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v3 does not fit an SM (occupancy 0)");
     ctx->cg_grid = ctx->num_sms;
     RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
     // d = diag(H), dinv

@@ -268,3 +268,30 @@ def test_query_device_buffers_match_host_buffers(setup):
     assert np.array_equal(rdv["y"].cpu().numpy(), rh["y"])  # deterministic reductions: same bits
     assert rdv["hashes"] == rh["hashes"]
     assert [s["cg_iters"] for s in rdv["steps"]] == [s["cg_iters"] for s in rh["steps"]]
+
+
+@pytest.mark.parametrize("method", [0, 1])
+def test_alg1_kernel_variants_agree(setup, rd, method):
+    """The three persistent kernels (TMA-staged coefficient form, literal recurrence, register-staged coefficient
+    form) run the same Algorithm 1: same status and rank, iteration counts within a few, solutions equal at the
+    level of the 1e-8 stop."""
+    w, o, g, W = setup
+    rng = np.random.default_rng(16)
+    act = (rng.random(w.N) < 0.2).astype(np.uint8)
+    b = np.where(act == 0, w.m * rng.standard_normal(w.N), 0.0)
+    x0 = np.zeros(w.N)
+    out = {}
+    try:
+        for variant in (0, 1, 2):
+            g.set_options(rd.Options(pdas_cap=w.pdas_cap, alg1_variant=variant))
+            out[variant] = g.solve_inactive(method, act, b, x0)
+    finally:
+        g.set_options(rd.Options(pdas_cap=w.pdas_cap))
+    x_ref, r_ref = out[1]
+    for variant in (0, 2):
+        x, r = out[variant]
+        assert r["status"] == r_ref["status"] == 0 and r["rank_used"] == r_ref["rank_used"]
+        assert r["rel_resid_verified"] <= 1e-8
+        assert abs(r["iters"] - r_ref["iters"]) <= max(3, 0.05 * r_ref["iters"]), (variant, r["iters"], r_ref["iters"])
+        assert (x[act == 1] == 0).all()
+        assert np.linalg.norm(x - x_ref) <= 1e-6 * np.linalg.norm(x_ref)
