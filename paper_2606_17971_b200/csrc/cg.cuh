@@ -39,6 +39,7 @@ struct CgParams {
     const double* b;     // rhs, 0 on J
     double *x, *r, *p0, *p1, *z, *w, *t;
     const double *Wm, *HWm;  // chi_I W and chi_I H chi_I W, N x kp column-major (ld = ldw)
+    const double* HWt;       // HWm tile-major: (i, j) at (i / 32) * 32 kp + 32 j + i % 32 (k_alg1_v3)
     const double* C;         // kp x kp column-major
     const double* EW;        // W_I^T H_II W_I, kp x kp column-major (k_alg1_v2)
     double eps, eps_c;

@@ -227,11 +227,11 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[warp];
             double* zbw = sh.zb[warp];
             const double* anu = sh.anu;
-            auto issue = [&](int64_t t) {
-                const double* src = P.HWm + row0 + 32 * t;
-                if (lane == 0) mbar_arrive_expect_tx(bar, tile_bytes);
-                __syncwarp();
-                for (int j = lane; j < kp; j += 32) bulk_g2s(tile + j * 32, src + (size_t)j * P.ldw, 256u, bar);
+            auto issue = [&](int64_t t) {  // one contiguous 256 kp bytes of the tile-major copy
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(bar, tile_bytes);
+                    bulk_g2s(tile, P.HWt + ((size_t)(row0 >> 5) + t) * 32 * kp, tile_bytes, bar);
+                }
             };
             int64_t t = warp;
             double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi = 0.0;
@@ -271,21 +271,31 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
                 }
                 zbw[lane] = zn;
                 __syncwarp();
-                // pass 2: lane = column, rows in the skewed order (ii + lane) mod 32
-#pragma unroll
-                for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) {
-                    const int j = lane + 32 * q;
-                    if (j < kp) {
-                        const double* tcol = tile + j * 32;
-                        double a0 = 0.0, a1 = 0.0;
+                // pass 2: lane = column(s) lane and lane + 32, rows in the skewed order (ii + lane) mod 32
+                if (lane < kp) {
+                    const double* t0 = tile + lane * 32;
+                    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+                    if (lane + 32 < kp) {
+                        const double* t1 = t0 + 32 * 32;
 #pragma unroll 8
                         for (int ii = 0; ii < 32; ii += 2) {
                             const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
-                            a0 = fma(tcol[r0], zbw[r0], a0);
-                            a1 = fma(tcol[r1], zbw[r1], a1);
+                            const double z0 = zbw[r0], z1 = zbw[r1];
+                            a0 = fma(t0[r0], z0, a0);
+                            a1 = fma(t0[r1], z1, a1);
+                            b0 = fma(t1[r0], z0, b0);
+                            b1 = fma(t1[r1], z1, b1);
                         }
-                        acc[q] += a0 + a1;
+                    } else {
+#pragma unroll 8
+                        for (int ii = 0; ii < 32; ii += 2) {
+                            const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
+                            a0 = fma(t0[r0], zbw[r0], a0);
+                            a1 = fma(t0[r1], zbw[r1], a1);
+                        }
                     }
+                    acc[0] += a0 + a1;
+                    acc[1] += b0 + b1;
                 }
                 __syncwarp();  // every lane has read the tile and zb
                 if (tn < ntiles) issue(tn);

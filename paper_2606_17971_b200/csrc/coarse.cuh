@@ -59,8 +59,11 @@ __global__ void k_spmm_K(Ell K, int64_t N, int64_t ldv, const double* minv, cons
 
 template <int CB>
 __global__ void k_spmm_KT(Ell KT, int64_t N, int64_t ldv, const double* m, double sigma, const uint8_t* act,
-                          const double* V, int64_t ldt, const double* T, int64_t ldo, double* OUT)
+                          const double* V, int64_t ldt, const double* T, int64_t ldo, double* OUT, double* OUTT, int kp,
+                          int jbase)
 {
+    // OUTT (may be NULL): the same block written tile-major for k_alg1_v3's ring, element (i, j) of the N x kp
+    // matrix at (i / 32) * 32 kp + 32 j + i % 32, so that a 32-row x kp tile is one contiguous 256 kp bytes.
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
@@ -80,9 +83,13 @@ __global__ void k_spmm_KT(Ell KT, int64_t N, int64_t ldv, const double* m, doubl
         if (row < N) {
             const double mi = m[row];
             const bool zero = act && act[row];
+            double* ot = OUTT ? OUTT + (size_t)s * 32 * kp + (size_t)jbase * 32 + lane : nullptr;
 #pragma unroll
-            for (int q = 0; q < CB; ++q)
-                OUT[row + (size_t)q * ldo] = zero ? 0.0 : fma(sigma, acc[q], mi * V[row + (size_t)q * ldv]);
+            for (int q = 0; q < CB; ++q) {
+                const double o_ = zero ? 0.0 : fma(sigma, acc[q], mi * V[row + (size_t)q * ldv]);
+                OUT[row + (size_t)q * ldo] = o_;
+                if (ot) ot[q * 32] = o_;
+            }
         }
     }
 }

@@ -62,7 +62,7 @@ struct rd_ctx {
     int* h_nactive = nullptr;
     // reference
     int k = 0, kp = 0;
-    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *Tchunk = nullptr;
+    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *HWt = nullptr, *Tchunk = nullptr;
     double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;
     int gram_nparts = 0;
     CoarseInfo* d_cinfo = nullptr;
@@ -255,6 +255,7 @@ int alloc_reference(rd_ctx* ctx, int k)
     RDTRY(dalloc(ctx, &ctx->W, nk));
     RDTRY(dalloc(ctx, &ctx->Wm, nk));
     RDTRY(dalloc(ctx, &ctx->HWm, nk));
+    RDTRY(dalloc(ctx, &ctx->HWt, nk));  // tile-major copy of HWm (k_alg1_v3); pad rows stay zero
     RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
     ctx->gram_nparts = ctx->num_sms * 2;
     RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
@@ -282,7 +283,8 @@ int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse)
         const double* V = ctx->Wm + (size_t)j * ctx->ldw;
         k_spmm_K<8><<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->ldw, ctx->minv, V, ctx->ldw, ctx->Tchunk);
         k_spmm_KT<8><<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->ldw, ctx->m, ctx->sigma, ctx->act, V, ctx->ldw,
-                                                       ctx->Tchunk, ctx->ldw, ctx->HWm + (size_t)j * ctx->ldw);
+                                                       ctx->Tchunk, ctx->ldw, ctx->HWm + (size_t)j * ctx->ldw,
+                                                       ctx->opt.alg1_variant == 0 ? ctx->HWt : nullptr, kp, j);
         ctx->launches += 2;
     }
     dim3 gg(ctx->gram_nparts, (kp + 63) / 64, (kp + 63) / 64);
@@ -329,7 +331,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.m = ctx->m; P.minv = ctx->minv; P.dinv = ctx->dinv; P.sigma = ctx->sigma;
     P.act = ctx->act; P.b = ctx->b;
     P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
-    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.C = ctx->C; P.EW = ctx->EW;
+    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.HWt = ctx->HWt; P.C = ctx->C; P.EW = ctx->EW;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
     P.partial = ctx->partial; P.bar = ctx->bar; P.rep = ctx->d_cgrep;
     CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
