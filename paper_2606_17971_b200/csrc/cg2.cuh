@@ -266,6 +266,47 @@ struct Cg2CtaT {
         }
     }
 
+    // ---- the k x k coefficient recurrences of the header comment (replicated in every CTA)
+    // lines 7 / 20 / 22-23: mu = C c, rho = r^T z~ - s^T mu, beta, nu = mu + beta nu, g = c + beta g
+    __device__ void coef_direction(bool restart, double rho_prime, double& rho, double& beta)
+    {
+        const int kp = P.kp;
+        small_matvec(sh.C, sh.c, sh.mu);
+        if (restart) {
+            if ((int)threadIdx.x < kp) { sh.sv[threadIdx.x] = 0.0; }
+            __syncthreads();
+        }
+        small_dot2(sh.sv, sh.mu, sh.sv, sh.mu);
+        const double rho_new = rho_prime - sh.small[0];
+        beta = restart ? 0.0 : rho_new / rho;
+        rho = rho_new;
+        __syncthreads();
+        if ((int)threadIdx.x < kp) {
+            sh.nu[threadIdx.x] = fma(beta, sh.nu[threadIdx.x], sh.mu[threadIdx.x]);
+            sh.g[threadIdx.x] = fma(beta, sh.g[threadIdx.x], sh.c[threadIdx.x]);
+        }
+        __syncthreads();
+    }
+    // line 9: p^T B p = p~^T w~ - 2 nu^T g + nu^T E_W nu
+    __device__ double coef_curvature(double pw)
+    {
+        small_matvec(sh.EW, sh.nu, sh.e);
+        small_dot2(sh.nu, sh.g, sh.nu, sh.e);
+        return pw - 2.0 * sh.small[0] + sh.small[1];
+    }
+    // line 10 in coefficients: s = W_I^T r, a nu, xi
+    __device__ void coef_step(double a)
+    {
+        __syncthreads();
+        if ((int)threadIdx.x < P.kp) {
+            const int j = threadIdx.x;
+            sh.sv[j] = fma(-a, sh.g[j] - sh.e[j], sh.sv[j]);
+            sh.anu[j] = a * sh.nu[j];
+            sh.xi[j] = fma(a, sh.nu[j], sh.xi[j]);
+        }
+        __syncthreads();
+    }
+
     // the two SpMVs of S3 over this CTA's slices (operator.cuh)
     template <bool COMBINE>
     __device__ void opK(const double* v0, const double* v1, double beta, double* pnew)
@@ -340,21 +381,7 @@ __device__ __forceinline__ void alg1_coeff_body(const CgParams& P, SH& sh, CTA& 
     while (!done && iters < P.cap) {
         // ---- coefficient part of lines 7 / 20 / 22-23
         if (coarse) {
-            cta.small_matvec(sh.C, sh.c, sh.mu);  // mu = C c
-            if (restart) {
-                if ((int)threadIdx.x < kp) { sh.sv[threadIdx.x] = 0.0; }
-                __syncthreads();
-            }
-            cta.small_dot2(sh.sv, sh.mu, sh.sv, sh.mu);
-            const double rho_new = rho_prime - sh.small[0];  // rho = r^T z = r^T z~ - s^T mu
-            beta = restart ? 0.0 : rho_new / rho;
-            rho = rho_new;
-            __syncthreads();
-            if ((int)threadIdx.x < kp) {
-                sh.nu[threadIdx.x] = fma(beta, sh.nu[threadIdx.x], sh.mu[threadIdx.x]);
-                sh.g[threadIdx.x] = fma(beta, sh.g[threadIdx.x], sh.c[threadIdx.x]);
-            }
-            __syncthreads();
+            cta.coef_direction(restart, rho_prime, rho, beta);
         } else {
             beta = restart ? 0.0 : rho_prime / rho;
             rho = rho_prime;
@@ -380,23 +407,12 @@ __device__ __forceinline__ void alg1_coeff_body(const CgParams& P, SH& sh, CTA& 
         cta.tick(3);
         iters++;
         double pw = sh.scal[SL_DOT];
-        if (coarse) {
-            cta.small_matvec(sh.EW, sh.nu, sh.e);           // e = E_W nu
-            cta.small_dot2(sh.nu, sh.g, sh.nu, sh.e);       // nu^T g, nu^T E_W nu
-            pw = pw - 2.0 * sh.small[0] + sh.small[1];      // p^T B p
-        }
+        if (coarse) pw = cta.coef_curvature(pw);  // p^T B p
         if (!(pw > 0.0) || !(rho > 0.0)) { status = RD_ENOTSPD_DEV; break; }
         // line 10
         const double a = rho / pw;
         if (coarse) {
-            __syncthreads();
-            if ((int)threadIdx.x < kp) {
-                const int j = threadIdx.x;
-                sh.sv[j] = fma(-a, sh.g[j] - sh.e[j], sh.sv[j]);  // s = W_I^T r
-                sh.anu[j] = a * sh.nu[j];
-                sh.xi[j] = fma(a, sh.nu[j], sh.xi[j]);
-            }
-            __syncthreads();
+            cta.coef_step(a);
             x_split = true;
             cta.tick(4);
             cta.stage_update_coarse(a, pnew);

@@ -39,8 +39,15 @@ struct __align__(128) Cg3Shared {
     __align__(128) unsigned char ring[RD_RING_BYTES];  // written by the async proxy only
 };
 
+#ifdef RD_DEBUG_SKEW
+__device__ unsigned long long g_dbg[148 * 8];
+#endif
+
 struct Cg3Cta : Cg2CtaT<Cg3Shared> {
     using Base = Cg2CtaT<Cg3Shared>;
+#ifdef RD_DEBUG_SKEW
+    int dbg_it = 0, dbg_seen4 = 0;
+#endif
     uint32_t ph;  // phase parity of this warp's mbarrier (uniform in the warp)
 
     __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : Base(p, s), ph(0)
@@ -56,6 +63,12 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
 
     __device__ void tick(int slot)
     {
+#ifdef RD_DEBUG_SKEW
+        if (slot == 6) dbg_it++;
+        if (threadIdx.x == 0) {
+            if (dbg_it == 100 && slot < 7) g_dbg[blockIdx.x * 8 + (slot == 4 ? (dbg_seen4++ ? 7 : 4) : slot)] = global_timer_ns();
+        }
+#endif
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             const uint64_t t = global_timer_ns();
             sh.tacc[slot] += t - sh.tlast;
@@ -64,76 +77,231 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
     }
     __device__ void finish(CgDevReport* rep)
     {
+#ifdef RD_DEBUG_SKEW
+        unsigned long long t0 = ~0ull;
+        for (int b = 0; b < G; ++b) t0 = min(t0, g_dbg[b * 8 + 4]);
+        for (int b = 0; b < G; ++b)
+            printf("SKEW %d startA %lld endA %lld barA %lld endB %lld barB %lld coef %lld endC %lld\n", b, g_dbg[b * 8 + 4] - t0,
+                   g_dbg[b * 8 + 0] - t0, g_dbg[b * 8 + 1] - t0, g_dbg[b * 8 + 2] - t0, g_dbg[b * 8 + 3] - t0, g_dbg[b * 8 + 7] - t0,
+                   g_dbg[b * 8 + 5] - t0);
+#endif
         for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = 1e-3 * (double)sh.tacc[q];
     }
 
-    // ---- staged sliced-ELL product over this CTA's slices; epi(row, acc) consumes sum_e A[row,e] vin[col_e]
-    template <bool COMBINE, class Epi>
-    __device__ __forceinline__ void spmv_staged(const Ell& A, const double* v0, const double* v1, double beta, Epi epi)
+    // ---- grid barrier + all-reduce in one round trip.  Every CTA publishes its partials, then a release store of
+    // the barrier generation to its own flag; thread i of every CTA acquires flag i.  No central counter, no
+    // second "go" broadcast; the partials are then summed by every CTA in the same fixed order (deterministic).
+    __device__ void sync_fetch(bool want_scal, bool want_c)
+    {
+        const double* base = P.partial + (size_t)(nbar & 1u) * SL_NSLOT * G;
+        nbar++;
+        const unsigned int gen = nbar;
+        if (P.bar_mode == 0) {
+            grid_barrier_counter(reinterpret_cast<unsigned long long*>(P.bar), G, gen);
+        } else if (P.bar_mode == 1) {
+            grid_barrier(P.bar, G);
+        } else {
+            __syncthreads();  // this CTA's partials and vector writes are issued
+            if (threadIdx.x == 0) {
+                __threadfence();
+                st_release_u32(&P.flags[blockIdx.x], gen);
+            }
+            if (P.bar_mode == 3) {
+                if (threadIdx.x < 32) {
+                    for (int i = threadIdx.x; i < G; i += 32)
+                        while (ld_relaxed_u32(&P.flags[i]) < gen) {}
+                    __threadfence();  // acquire side; also drops this SM's stale L1 lines
+                }
+            } else {
+                for (int i = threadIdx.x; i < G; i += blockDim.x) {
+                    while (ld_relaxed_u32(&P.flags[i]) < gen) {}
+                    __threadfence();
+                }
+            }
+            __syncthreads();
+        }
+        if (!want_scal) return;
+        // all slots in one round: 8 lanes per slot (128 slot groups >= 4 + kp), fixed order => identical on all CTAs
+        const int nsl = want_c ? SL_NSCAL + P.kp : SL_NSCAL;
+        const int sl = threadIdx.x >> 3, sub = threadIdx.x & 7;
+        if ((sl & ~3) < nsl) {  // warp-uniform: some slot of this warp is live
+            double a0 = 0.0, a1 = 0.0;
+            if (sl < nsl) {
+                const double* q = base + (size_t)sl * G;
+#pragma unroll 4
+                for (int i = sub; i < G; i += 16) {
+                    a0 += __ldcg(q + i);
+                    if (i + 8 < G) a1 += __ldcg(q + i + 8);
+                }
+            }
+            double a = a0 + a1;
+            a += __shfl_xor_sync(0xffffffffu, a, 4);
+            a += __shfl_xor_sync(0xffffffffu, a, 2);
+            a += __shfl_xor_sync(0xffffffffu, a, 1);
+            if (sub == 0 && sl < nsl) {
+                if (sl < SL_NSCAL) sh.scal[sl] = a; else sh.c[sl - SL_NSCAL] = a;
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- k x k coefficient recurrences (cg2.cuh header), done by warp 0 alone: lane owns rows lane and lane + 32
+    // of the kp x kp matrices (column-major: conflict-free), vectors are broadcast reads.  One __syncthreads.
+    __device__ __forceinline__ void matvec_w0(const double* M, const double* v, int kp, int lane, double& o0, double& o1)
+    {
+        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+        const bool r0 = lane < kp, r1 = lane + 32 < kp;
+        const double* m0 = M + (r0 ? lane : 0);
+        const double* m1 = M + (r1 ? lane + 32 : 0);
+        for (int j = 0; j < kp; j += 2) {
+            const double v0 = v[j], v1 = v[j + 1];
+            a0 = fma(m0[(size_t)j * kp], v0, a0);
+            b0 = fma(m0[(size_t)(j + 1) * kp], v1, b0);
+            a1 = fma(m1[(size_t)j * kp], v0, a1);
+            b1 = fma(m1[(size_t)(j + 1) * kp], v1, b1);
+        }
+        o0 = r0 ? a0 + b0 : 0.0;
+        o1 = r1 ? a1 + b1 : 0.0;
+    }
+    // lines 7 / 20 / 22-23 and the curvature terms of line 9 that do not need p~^T w~:
+    //   mu = C c, rho = r^T z~ - s^T mu, beta, nu = mu + beta nu, g = c + beta g, e = E_W nu, nu^T g, nu^T e
+    __device__ void coef_direction(bool restart, double rho_prime, double& rho, double& beta)
+    {
+        const int kp = P.kp;
+        if (threadIdx.x < 32) {
+            const int lane = threadIdx.x;
+            const bool r0 = lane < kp, r1 = lane + 32 < kp;
+            double mu0, mu1;
+            matvec_w0(sh.C, sh.c, kp, lane, mu0, mu1);
+            const double s0_ = (restart || !r0) ? 0.0 : sh.sv[lane], s1_ = (restart || !r1) ? 0.0 : sh.sv[lane + 32];
+            const double smu = warp_sum(fma(s0_, mu0, s1_ * mu1));
+            const double rho_new = rho_prime - smu;
+            const double bt = restart ? 0.0 : rho_new / rho;
+            double nu0 = 0.0, nu1 = 0.0, g0 = 0.0, g1 = 0.0;
+            if (r0) { nu0 = fma(bt, sh.nu[lane], mu0); g0 = fma(bt, sh.g[lane], sh.c[lane]); sh.nu[lane] = nu0; sh.g[lane] = g0; sh.mu[lane] = mu0; if (restart) sh.sv[lane] = 0.0; }
+            if (r1) { nu1 = fma(bt, sh.nu[lane + 32], mu1); g1 = fma(bt, sh.g[lane + 32], sh.c[lane + 32]); sh.nu[lane + 32] = nu1; sh.g[lane + 32] = g1; sh.mu[lane + 32] = mu1; if (restart) sh.sv[lane + 32] = 0.0; }
+            __syncwarp();
+            double e0, e1;
+            matvec_w0(sh.EW, sh.nu, kp, lane, e0, e1);
+            if (r0) sh.e[lane] = e0;
+            if (r1) sh.e[lane + 32] = e1;
+            const double ng = warp_sum(fma(nu0, g0, nu1 * g1));
+            const double ne = warp_sum(fma(nu0, e0, nu1 * e1));
+            if (lane == 0) { sh.small[0] = rho_new; sh.small[1] = bt; sh.small[2] = ng; sh.small[3] = ne; }
+        }
+        __syncthreads();
+        rho = sh.small[0];
+        beta = sh.small[1];
+    }
+    __device__ double coef_curvature(double pw) { return pw - 2.0 * sh.small[2] + sh.small[3]; }
+    // line 10 in coefficients; the __syncthreads that opens stage_update_coarse publishes anu
+    __device__ void coef_step(double a)
+    {
+        if ((int)threadIdx.x < P.kp) {
+            const int j = threadIdx.x;
+            sh.sv[j] = fma(-a, sh.g[j] - sh.e[j], sh.sv[j]);
+            sh.anu[j] = a * sh.nu[j];
+            sh.xi[j] = fma(a, sh.nu[j], sh.xi[j]);
+        }
+    }
+
+    // values and column indices of one 32-row slice (wd entries per row) into this warp's slot
+    __device__ __forceinline__ void issue_slice(const Ell& A, int64_t o, int wd)
+    {
+        if ((threadIdx.x & 31) == 0) {
+            unsigned char* slot_ = sh.ring + (threadIdx.x >> 5) * RD_SPMV_SLOT_BYTES;
+            uint64_t* bar = &sh.full[threadIdx.x >> 5];
+            mbar_arrive_expect_tx(bar, (uint32_t)wd * 384u);
+            if (wd > 0) {
+                if (P.l2_mode & 12) {
+                    const uint64_t pol = (P.l2_mode & 4) ? l2_policy_evict_first() : l2_policy_evict_last();
+                    bulk_g2s_hint(slot_, A.val + o, (uint32_t)wd * 256u, bar, pol);
+                    bulk_g2s_hint(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar, pol);
+                } else {
+                    bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
+                    bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
+                }
+            }
+        }
+    }
+    // sum_e A[row,e] vin[col_e] for this lane's row of the slice staged in (sval, scol); WDC = register budget
+    // (entries per row).  All gathers are issued before the first use; `next` refills the slot in between.
+    template <bool COMBINE, int WDC, class Next>
+    __device__ __forceinline__ double staged_row_dot(const double* sval, const int32_t* scol, int wd, int lane,
+                                                     const double* v0, const double* v1, double beta, Next next)
+    {
+        int cc[WDC];
+        double aa[WDC], xx[WDC], yy[WDC];
+#pragma unroll
+        for (int q = 0; q < WDC; ++q) {
+            const bool ok = q < wd;
+            cc[q] = ok ? scol[q * 32 + lane] : 0;
+            aa[q] = ok ? sval[q * 32 + lane] : 0.0;
+        }
+        __syncwarp();
+        next();
+#pragma unroll
+        for (int q = 0; q < WDC; ++q) xx[q] = (q < wd) ? v0[cc[q]] : 0.0;
+        if (COMBINE) {
+#pragma unroll
+            for (int q = 0; q < WDC; ++q) yy[q] = (q < wd) ? v1[cc[q]] : 0.0;
+#pragma unroll
+            for (int q = 0; q < WDC; ++q) xx[q] = fma(beta, yy[q], xx[q]);
+        }
+        double acc = 0.0;
+#pragma unroll
+        for (int q = 0; q < WDC; ++q) acc = fma(aa[q], xx[q], acc);
+        return acc;
+    }
+
+    // ---- staged sliced-ELL product over this CTA's slices.  pre(row) loads what the epilogue needs of the row
+    // (issued before the wait on the slice, so it never adds a round trip); epi(row, acc, pre(row)) consumes
+    // sum_e A[row,e] vin[col_e].  A matrix of uniform slice width needs no extent lookups (Ell::uwd).
+    template <bool COMBINE, class Pre, class Epi>
+    __device__ __forceinline__ void spmv_staged(const Ell& A, const double* v0, const double* v1, double beta, Pre pre, Epi epi)
     {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         unsigned char* slot_ = sh.ring + warp * RD_SPMV_SLOT_BYTES;
         const double* sval = reinterpret_cast<const double*>(slot_);
         const int32_t* scol = reinterpret_cast<const int32_t*>(slot_ + RD_SPMV_WD * 256);
         uint64_t* bar = &sh.full[warp];
-        auto issue = [&](int64_t o, int wd) {
-            if (lane == 0) {
-                mbar_arrive_expect_tx(bar, (uint32_t)wd * 384u);
-                if (wd > 0) {
-                    bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
-                    bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
-                }
-            }
+        const int uwd = A.uwd;
+        auto extent = [&](int64_t s, int64_t& o, int& wd) {
+            if (uwd >= 0) { o = s * 32 * uwd; wd = uwd; }
+            else { o = A.off[s]; wd = (int)((A.off[s + 1] - o) >> 5); }
         };
         int64_t s = s0 + warp;
-        int64_t o = 0;
         int wd = 0;
         if (s < s1) {
-            o = A.off[s];
-            wd = (int)((A.off[s + 1] - o) >> 5);
-            if (wd <= RD_SPMV_WD) issue(o, wd);
+            int64_t o;
+            extent(s, o, wd);
+            if (wd <= RD_SPMV_WD) issue_slice(A, o, wd);
         }
         for (; s < s1; s += 32) {
             const int64_t sn = s + 32;
             int64_t on = 0;
             int wdn = 0;
-            if (sn < s1) {
-                on = A.off[sn];
-                wdn = (int)((A.off[sn + 1] - on) >> 5);
-            }
-            double acc = 0.0;
+            if (sn < s1) extent(sn, on, wdn);
+            const int64_t row = s * RD_SLICE + lane;
+            auto rowdata = pre(row);
+            auto next = [&]() { if (sn < s1 && wdn <= RD_SPMV_WD) issue_slice(A, on, wdn); };
+            double acc;
             if (wd <= RD_SPMV_WD) {
                 mbar_wait(bar, ph);
                 ph ^= 1u;
-                int cc[RD_SPMV_WD];
-                double aa[RD_SPMV_WD];
-#pragma unroll
-                for (int q = 0; q < RD_SPMV_WD; ++q) {
-                    const bool ok = q < wd;
-                    cc[q] = ok ? scol[q * 32 + lane] : 0;
-                    aa[q] = ok ? sval[q * 32 + lane] : 0.0;
-                }
-                __syncwarp();
-                if (sn < s1 && wdn <= RD_SPMV_WD) issue(on, wdn);
-                double xx[RD_SPMV_WD];
-#pragma unroll
-                for (int q = 0; q < RD_SPMV_WD; ++q) xx[q] = (q < wd) ? v0[cc[q]] : 0.0;
-                if (COMBINE) {
-#pragma unroll
-                    for (int q = 0; q < RD_SPMV_WD; ++q)
-                        if (q < wd) xx[q] = fma(beta, v1[cc[q]], xx[q]);
-                }
-#pragma unroll
-                for (int q = 0; q < RD_SPMV_WD; ++q) acc = fma(aa[q], xx[q], acc);
+                if (wd <= 5) acc = staged_row_dot<COMBINE, 5>(sval, scol, wd, lane, v0, v1, beta, next);
+                else acc = staged_row_dot<COMBINE, RD_SPMV_WD>(sval, scol, wd, lane, v0, v1, beta, next);
             } else {
-                if (sn < s1 && wdn <= RD_SPMV_WD) issue(on, wdn);
+                next();
                 acc = ell_row_dot<COMBINE>(A, s, lane, v0, v1, beta);
             }
-            epi(s * RD_SLICE + lane, acc);
-            o = on;
+            epi(row, acc, rowdata);
             wd = wdn;
         }
     }
+
+    struct RowK { double minv, x; };
+    struct RowKT { double v, m; bool act; };
 
     // stage A: t = M^{-1} K (v0 + beta v1), pnew = v0 + beta v1 on this CTA's rows  (Alg. 1 lines 23 + 9)
     template <bool COMBINE>
@@ -142,16 +310,25 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         const int64_t N = P.N;
         const double* minv = P.minv;
         double* t = P.t;
-        spmv_staged<COMBINE>(P.K, v0, v1, beta, [&](int64_t row, double acc) {
-            if (row < N) {
-                t[row] = acc * ldg_f64(minv + row);
-                if (pnew) {
-                    double x = v0[row];
-                    if (COMBINE) x = fma(beta, v1[row], x);
-                    pnew[row] = x;
+        spmv_staged<COMBINE>(
+            P.K, v0, v1, beta,
+            [&](int64_t row) {
+                RowK r{0.0, 0.0};
+                if (row < N) {
+                    r.minv = ldg_f64(minv + row);
+                    if (pnew) {
+                        r.x = v0[row];
+                        if (COMBINE) r.x = fma(beta, v1[row], r.x);
+                    }
                 }
-            }
-        });
+                return r;
+            },
+            [&](int64_t row, double acc, const RowK& r) {
+                if (row < N) {
+                    t[row] = acc * r.minv;
+                    if (pnew) pnew[row] = r.x;
+                }
+            });
     }
     // stage B: w = chi_I (m.v + sigma K^T t); returns this thread's partial of v^T w  (Alg. 1 line 9)
     __device__ double opKT(const double* v)
@@ -162,15 +339,25 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         const double sigma = P.sigma;
         double* w = P.w;
         double dot = 0.0;
-        spmv_staged<false>(P.KT, P.t, nullptr, 0.0, [&](int64_t row, double acc) {
-            if (row < N) {
-                const double vi = v[row];
-                double wi = fma(sigma, acc, ldg_f64(m + row) * vi);
-                if (act && act[row]) wi = 0.0;
-                w[row] = wi;
-                dot = fma(vi, wi, dot);
-            }
-        });
+        spmv_staged<false>(
+            P.KT, P.t, nullptr, 0.0,
+            [&](int64_t row) {
+                RowKT r{0.0, 0.0, false};
+                if (row < N) {
+                    r.v = v[row];
+                    r.m = ldg_f64(m + row);
+                    r.act = act && act[row];
+                }
+                return r;
+            },
+            [&](int64_t row, double acc, const RowKT& r) {
+                if (row < N) {
+                    double wi = fma(sigma, acc, r.m * r.v);
+                    if (r.act) wi = 0.0;
+                    w[row] = wi;
+                    dot = fma(r.v, wi, dot);
+                }
+            });
         return dot;
     }
 
@@ -207,6 +394,21 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         put(SL_RHO, rho);
     }
 
+    // one 32-row x kp tile of the tile-major copy of HW_I (contiguous 256 kp bytes) into this consumer warp's slot
+    __device__ __forceinline__ void issue_tile(int64_t t)
+    {
+        if ((threadIdx.x & 31) == 0) {
+            const int warp = threadIdx.x >> 5;
+            const uint32_t tile_bytes = 256u * (uint32_t)P.kp;
+            void* tile = sh.ring + (size_t)warp * tile_bytes;
+            uint64_t* bar = &sh.full[warp];
+            mbar_arrive_expect_tx(bar, tile_bytes);
+            const double* src = P.HWt + ((size_t)(row0 >> 5) + t) * 32 * P.kp;
+            if (P.l2_mode & 1) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_last());
+            else if (P.l2_mode & 2) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_first());
+            else bulk_g2s(tile, src, tile_bytes, bar);
+        }
+    }
     // Stage C with a coarse space: one pass over HW_I through the shared-memory ring (header comment).
     //   r_i  <- r_i - a w~_i + sum_j HW_ij (a nu_j)      x~_i <- x~_i + a p~_i      z~_i <- r_i / d_i
     //   ||r||^2, r^T z~,  c_j = sum_i HW_ij z~_i                                      (eq. (18))
@@ -227,12 +429,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[warp];
             double* zbw = sh.zb[warp];
             const double* anu = sh.anu;
-            auto issue = [&](int64_t t) {  // one contiguous 256 kp bytes of the tile-major copy
-                if (lane == 0) {
-                    mbar_arrive_expect_tx(bar, tile_bytes);
-                    bulk_g2s(tile, P.HWt + ((size_t)(row0 >> 5) + t) * 32 * kp, tile_bytes, bar);
-                }
-            };
+            auto issue = [&](int64_t t) { issue_tile(t); };
             int64_t t = warp;
             double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi = 0.0;
             if (t < ntiles) {

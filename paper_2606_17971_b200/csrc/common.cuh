@@ -66,6 +66,12 @@ __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p)
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p)
+{
+    unsigned int v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v)
 {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -75,6 +81,24 @@ __device__ __forceinline__ unsigned int atom_add_acqrel_u32(unsigned int* p, uns
     unsigned int old;
     asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
     return old;
+}
+
+// Single-hop variant: one monotone 64-bit arrival counter; CTA number `gen` (1, 2, ...) of this launch is through
+// when the counter reaches gen * nblocks.  Arrival is a release reduction without a return value (no round trip),
+// everybody polls the counter itself with acquire loads: one L2 round trip after the last arrival instead of
+// fence + atomic + reset + fence + release-store + poll.  The counter must be zero at launch.
+__device__ __forceinline__ void grid_barrier_counter(unsigned long long* counter, unsigned int nblocks, unsigned int gen)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned long long target = (unsigned long long)gen * nblocks;
+        asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(counter), "l"(1ull) : "memory");
+        unsigned long long seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(counter) : "memory");
+        } while (seen < target);
+    }
+    __syncthreads();
 }
 
 __device__ __forceinline__ void grid_barrier(GridBarrier* bar, unsigned int nblocks)

@@ -15,6 +15,7 @@ struct Ell {
     const double* val;
     const int64_t* off;  // nslices + 1, in entries
     int64_t nslices;
+    int32_t uwd;  // entries per row if every slice has the same width (off[s] = 32 uwd s, no lookup needed), else -1
 };
 
 // One row of a sliced-ELL product with an on-the-fly combined input  v0[c] + beta v1[c]  (v1 may be

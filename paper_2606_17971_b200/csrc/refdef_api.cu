@@ -35,7 +35,8 @@ struct EllStore {
     double* val = nullptr;
     int64_t* off = nullptr;
     int64_t nslices = 0, entries = 0;
-    Ell view() const { return Ell{col, val, off, nslices}; }
+    int32_t uwd = -1;
+    Ell view() const { return Ell{col, val, off, nslices, uwd}; }
 };
 
 }  // namespace
@@ -71,6 +72,7 @@ struct rd_ctx {
     int cg_grid = 0;
     double* partial = nullptr;
     GridBarrier* bar = nullptr;
+    unsigned int* flags = nullptr;
     CgDevReport* d_cgrep = nullptr;
     CgDevReport* h_cgrep = nullptr;
     PdasCounters* d_cnt = nullptr;
@@ -215,6 +217,13 @@ int upload_ell(rd_ctx* ctx, const HostEll& h, EllStore& d)
 {
     d.nslices = (int64_t)h.off.size() - 1;
     d.entries = h.off.back();
+    d.uwd = -1;
+    if (d.nslices > 0) {
+        const int64_t w0 = h.off[1] - h.off[0];
+        bool uniform = true;
+        for (int64_t s = 1; s < d.nslices && uniform; ++s) uniform = (h.off[s + 1] - h.off[s]) == w0;
+        if (uniform && w0 / RD_SLICE <= 64) d.uwd = (int32_t)(w0 / RD_SLICE);
+    }
     RDTRY(dalloc(ctx, &d.col, h.col.size(), false));
     RDTRY(dalloc(ctx, &d.val, h.val.size(), false));
     RDTRY(dalloc(ctx, &d.off, h.off.size(), false));
@@ -333,11 +342,14 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
     P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.HWt = ctx->HWt; P.C = ctx->C; P.EW = ctx->EW;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
-    P.partial = ctx->partial; P.bar = ctx->bar; P.rep = ctx->d_cgrep;
+    P.partial = ctx->partial; P.bar = ctx->bar; P.flags = ctx->flags;
+    { const char* e_ = getenv("RD_BAR_MODE"); P.bar_mode = e_ ? atoi(e_) : 0; }
+    { const char* e_ = getenv("RD_L2_MODE"); P.l2_mode = e_ ? atoi(e_) : 2; } P.rep = ctx->d_cgrep;
     CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->p1, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->z, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
+    CU(cudaMemsetAsync(ctx->flags, 0, sizeof(unsigned int) * ctx->cg_grid, ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
     const int variant = ctx->opt.alg1_variant;
@@ -530,6 +542,7 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v3 does not fit an SM (occupancy 0)");
     ctx->cg_grid = ctx->num_sms;
     RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
+    RDTRY(dalloc(ctx, &ctx->flags, (size_t)ctx->cg_grid));
     // d = diag(H), dinv
     k_diag_H<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
         ctx->KT.view(), N, ctx->m, ctx->minv, ctx->sigma, ctx->opt.jacobi, ctx->d, ctx->dinv);
