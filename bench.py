@@ -238,8 +238,7 @@ def run_ours(args):
         e1.synchronize()
         return e0.elapsed_time(e1), res
 
-    for _ in range(args.warmup):
-        one_step(False)
+    warm_ms = [one_step(False)[0] for _ in range(args.warmup)]
     sampler = ClockSampler(local_rank)
     barrier()
     sampler.start()
@@ -317,7 +316,11 @@ def run_ours(args):
             "breakdown": {"pdas_steps": n_steps, "query_status_counts": {str(k): v for k, v in statuses.items()},
                           "reference_builds_in_timed_region": ref_builds, "reference_ms": round(ref_ms, 1),
                           "alg1_ms": round(alg_ms, 1), "coarse_setup_ms": round(coarse_ms, 1), "update_ms": round(upd_ms, 1),
-                          "wall_ms_incl_host": round(wall_ms, 1)},
+                          "wall_ms_incl_host": round(wall_ms, 1),
+                          # the sequence so far, for the reader: the first query of a pass carries the reference build
+                          # (PAPER.md:352); warm-up queries are untimed for `value` but listed here
+                          "warmup_query_s": [round(x * 1e-3, 3) for x in warm_ms], "timed_query_s": [round(x * 1e-3, 3) for x in step_ms],
+                          "reference_build_s_before_timed_region": round(refms0 * 1e-3, 3)},
         }
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(args, w, g, method, iters / max(args.steps, 1), n_steps / max(args.steps, 1))

@@ -404,7 +404,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[warp];
             mbar_arrive_expect_tx(bar, tile_bytes);
             const double* src = P.HWt + ((size_t)(row0 >> 5) + t) * 32 * P.kp;
-            if (P.l2_mode & 1) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_last());
+            if ((P.l2_mode & 1) || t < P.hw_res_tiles) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_last());
             else if (P.l2_mode & 2) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_first());
             else bulk_g2s(tile, src, tile_bytes, bar);
         }

@@ -344,7 +344,17 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
     P.partial = ctx->partial; P.bar = ctx->bar; P.flags = ctx->flags;
     { const char* e_ = getenv("RD_BAR_MODE"); P.bar_mode = e_ ? atoi(e_) : 0; }
-    { const char* e_ = getenv("RD_L2_MODE"); P.l2_mode = e_ ? atoi(e_) : 2; } P.rep = ctx->d_cgrep;
+    { const char* e_ = getenv("RD_L2_MODE"); P.l2_mode = e_ ? atoi(e_) : 2; }
+    {   // Part of the H_II W_I stream is requested with L2 evict_last when the whole working set nearly fits the
+        // 126 MB L2 (config 2): what is left of a 60 MB budget after K, K^T and ten vectors, at most half the stream.
+        const char* e_ = getenv("RD_HW_RES_PCT");
+        const double hw_bytes = 8.0 * (double)ctx->ldw * ctx->kp;
+        const double other = 12.0 * (double)(ctx->K.entries + ctx->KT.entries) + 80.0 * (double)N;
+        double frac = hw_bytes > 0 ? std::min(0.5, std::max(0.0, (60e6 - other) / hw_bytes)) : 0.0;
+        if (e_) frac = atoi(e_) / 100.0;
+        const int64_t tiles_per_cta = ((ctx->K.nslices + ctx->cg_grid - 1) / ctx->cg_grid);
+        P.hw_res_tiles = (int32_t)((double)tiles_per_cta * frac);
+    } P.rep = ctx->d_cgrep;
     CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->p1, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->z, 0, ctx->ldw * sizeof(double), ctx->stream));
