@@ -238,7 +238,14 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             cc[q] = ok ? scol[q * 32 + lane] : 0;
             aa[q] = ok ? sval[q * 32 + lane] : 0.0;
         }
-        __syncwarp();
+        // The refill below is an asynchronous write into the slot just read.  Shared-memory loads complete out of
+        // program order with respect to it (they can queue behind this SM's global gathers for longer than a bulk
+        // copy takes to land: measured as rare wrong rows on config 5), so the loaded registers are CONSUMED by a
+        // real instruction first: the warp cannot issue the vote before every load has written back.
+        int chk = 0;
+#pragma unroll
+        for (int q = 0; q < WDC; ++q) chk ^= cc[q] ^ __double2hiint(aa[q]) ^ __double2loint(aa[q]);
+        if (__ballot_sync(0xffffffffu, chk == 0x5a5a5a5b)) __nanosleep(1);  // harmless if it ever fires
         next();
 #pragma unroll
         for (int q = 0; q < WDC; ++q) xx[q] = (q < wd) ? v0[cc[q]] : 0.0;

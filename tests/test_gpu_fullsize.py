@@ -104,3 +104,26 @@ def test_fullsize_longer_run_residual_is_true_residual(big):
     # CG minimises the energy norm of the error monotonically: the iterate must beat the start in that norm,
     # i.e. x^T H x - 2 b^T x < 0 for a zero start
     assert xg @ o.apply_H(xg) - 2.0 * (b @ xg) < 0.0
+
+
+@pytest.mark.parametrize("method", [0, 1])
+def test_fullsize_runs_are_bit_identical(big, method):
+    """All reductions have a fixed order, so repeated solves must agree to the last bit; a data race in the
+    asynchronous staging (shared-memory slots refilled by TMA while still being read) shows up here as a few
+    differing rows.  This caught exactly that on config 5 (see cg3.cuh, staged_row_dot)."""
+    w, o, g, W, pkg = big
+    rng = np.random.default_rng(3)
+    act = (rng.random(w.N) < 0.5).astype(np.uint8)
+    yd = w._target(1000 * w.config)
+    b = np.where(act == 0, w.m * yd, 0.0)
+    x0 = np.zeros(w.N)
+    g.set_options(pkg.Options(pdas_cap=w.pdas_cap, cg_cap=40))
+    try:
+        runs = [g.solve_inactive(method, act, b, x0) for _ in range(6)]
+    finally:
+        g.set_options(pkg.Options(pdas_cap=w.pdas_cap))
+    x_first, r_first = runs[0]
+    for x, r in runs[1:]:
+        assert r["iters"] == r_first["iters"] == 40
+        assert r["rel_resid_verified"] == r_first["rel_resid_verified"]
+        assert np.array_equal(x, x_first)
