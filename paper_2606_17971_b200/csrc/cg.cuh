@@ -46,10 +46,7 @@ struct CgParams {
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]
     GridBarrier* bar;
-    int32_t l2_mode;      // experiment switch: L2 eviction hints of the bulk copies (RD_L2_MODE)
     int32_t hw_res_tiles; // tiles per CTA of the H_II W_I stream requested with L2 evict_last (kept resident)
-    int32_t bar_mode;     // experiment switch of k_alg1_v3's grid barrier (RD_BAR_MODE)
-    unsigned int* flags;  // [gridDim.x] barrier generations, one per CTA (k_alg1_v3), zero at launch
     CgDevReport* rep;
 };
 

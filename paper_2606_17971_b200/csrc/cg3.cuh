@@ -39,15 +39,9 @@ struct __align__(128) Cg3Shared {
     __align__(128) unsigned char ring[RD_RING_BYTES];  // written by the async proxy only
 };
 
-#ifdef RD_DEBUG_SKEW
-__device__ unsigned long long g_dbg[148 * 8];
-#endif
 
 struct Cg3Cta : Cg2CtaT<Cg3Shared> {
     using Base = Cg2CtaT<Cg3Shared>;
-#ifdef RD_DEBUG_SKEW
-    int dbg_it = 0, dbg_seen4 = 0;
-#endif
     uint32_t ph;  // phase parity of this warp's mbarrier (uniform in the warp)
 
     __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : Base(p, s), ph(0)
@@ -63,12 +57,6 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
 
     __device__ void tick(int slot)
     {
-#ifdef RD_DEBUG_SKEW
-        if (slot == 6) dbg_it++;
-        if (threadIdx.x == 0) {
-            if (dbg_it == 100 && slot < 7) g_dbg[blockIdx.x * 8 + (slot == 4 ? (dbg_seen4++ ? 7 : 4) : slot)] = global_timer_ns();
-        }
-#endif
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             const uint64_t t = global_timer_ns();
             sh.tacc[slot] += t - sh.tlast;
@@ -77,49 +65,18 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
     }
     __device__ void finish(CgDevReport* rep)
     {
-#ifdef RD_DEBUG_SKEW
-        unsigned long long t0 = ~0ull;
-        for (int b = 0; b < G; ++b) t0 = min(t0, g_dbg[b * 8 + 4]);
-        for (int b = 0; b < G; ++b)
-            printf("SKEW %d startA %lld endA %lld barA %lld endB %lld barB %lld coef %lld endC %lld\n", b, g_dbg[b * 8 + 4] - t0,
-                   g_dbg[b * 8 + 0] - t0, g_dbg[b * 8 + 1] - t0, g_dbg[b * 8 + 2] - t0, g_dbg[b * 8 + 3] - t0, g_dbg[b * 8 + 7] - t0,
-                   g_dbg[b * 8 + 5] - t0);
-#endif
         for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = 1e-3 * (double)sh.tacc[q];
     }
 
-    // ---- grid barrier + all-reduce in one round trip.  Every CTA publishes its partials, then a release store of
-    // the barrier generation to its own flag; thread i of every CTA acquires flag i.  No central counter, no
-    // second "go" broadcast; the partials are then summed by every CTA in the same fixed order (deterministic).
+    // ---- grid barrier + all-reduce.  Every CTA has written one partial per reduced quantity; the barrier is the
+    // single-hop counter barrier of common.cuh (arrival = release reduction on one monotone counter, everybody polls
+    // that counter); then every CTA sums all partials in the same fixed order (deterministic, identical branches).
     __device__ void sync_fetch(bool want_scal, bool want_c)
     {
         const double* base = P.partial + (size_t)(nbar & 1u) * SL_NSLOT * G;
         nbar++;
         const unsigned int gen = nbar;
-        if (P.bar_mode == 0) {
-            grid_barrier_counter(reinterpret_cast<unsigned long long*>(P.bar), G, gen);
-        } else if (P.bar_mode == 1) {
-            grid_barrier(P.bar, G);
-        } else {
-            __syncthreads();  // this CTA's partials and vector writes are issued
-            if (threadIdx.x == 0) {
-                __threadfence();
-                st_release_u32(&P.flags[blockIdx.x], gen);
-            }
-            if (P.bar_mode == 3) {
-                if (threadIdx.x < 32) {
-                    for (int i = threadIdx.x; i < G; i += 32)
-                        while (ld_relaxed_u32(&P.flags[i]) < gen) {}
-                    __threadfence();  // acquire side; also drops this SM's stale L1 lines
-                }
-            } else {
-                for (int i = threadIdx.x; i < G; i += blockDim.x) {
-                    while (ld_relaxed_u32(&P.flags[i]) < gen) {}
-                    __threadfence();
-                }
-            }
-            __syncthreads();
-        }
+        grid_barrier_counter(reinterpret_cast<unsigned long long*>(P.bar), G, gen);
         if (!want_scal) return;
         // all slots in one round: 8 lanes per slot (128 slot groups >= 4 + kp), fixed order => identical on all CTAs
         const int nsl = want_c ? SL_NSCAL + P.kp : SL_NSCAL;
@@ -213,11 +170,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[threadIdx.x >> 5];
             mbar_arrive_expect_tx(bar, (uint32_t)wd * 384u);
             if (wd > 0) {
-                if (P.l2_mode & 12) {
-                    const uint64_t pol = (P.l2_mode & 4) ? l2_policy_evict_first() : l2_policy_evict_last();
-                    bulk_g2s_hint(slot_, A.val + o, (uint32_t)wd * 256u, bar, pol);
-                    bulk_g2s_hint(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar, pol);
-                } else {
+                {
                     bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
                     bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
                 }
@@ -411,9 +364,9 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[warp];
             mbar_arrive_expect_tx(bar, tile_bytes);
             const double* src = P.HWt + ((size_t)(row0 >> 5) + t) * 32 * P.kp;
-            if ((P.l2_mode & 1) || t < P.hw_res_tiles) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_last());
-            else if (P.l2_mode & 2) bulk_g2s_hint(tile, src, tile_bytes, bar, l2_policy_evict_first());
-            else bulk_g2s(tile, src, tile_bytes, bar);
+            // no reuse before the next iteration: evict_first keeps the gathered vectors and K in L2; when the working
+            // set nearly fits the L2 the first hw_res_tiles tiles of every CTA are kept instead (evict_last)
+            bulk_g2s_hint(tile, src, tile_bytes, bar, t < P.hw_res_tiles ? l2_policy_evict_last() : l2_policy_evict_first());
         }
     }
     // Stage C with a coarse space: one pass over HW_I through the shared-memory ring (header comment).

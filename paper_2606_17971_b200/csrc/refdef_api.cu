@@ -72,7 +72,6 @@ struct rd_ctx {
     int cg_grid = 0;
     double* partial = nullptr;
     GridBarrier* bar = nullptr;
-    unsigned int* flags = nullptr;
     CgDevReport* d_cgrep = nullptr;
     CgDevReport* h_cgrep = nullptr;
     PdasCounters* d_cnt = nullptr;
@@ -342,16 +341,12 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
     P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.HWt = ctx->HWt; P.C = ctx->C; P.EW = ctx->EW;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
-    P.partial = ctx->partial; P.bar = ctx->bar; P.flags = ctx->flags;
-    { const char* e_ = getenv("RD_BAR_MODE"); P.bar_mode = e_ ? atoi(e_) : 0; }
-    { const char* e_ = getenv("RD_L2_MODE"); P.l2_mode = e_ ? atoi(e_) : 2; }
+    P.partial = ctx->partial; P.bar = ctx->bar;
     {   // Part of the H_II W_I stream is requested with L2 evict_last when the whole working set nearly fits the
         // 126 MB L2 (config 2): what is left of a 60 MB budget after K, K^T and ten vectors, at most half the stream.
-        const char* e_ = getenv("RD_HW_RES_PCT");
         const double hw_bytes = 8.0 * (double)ctx->ldw * ctx->kp;
         const double other = 12.0 * (double)(ctx->K.entries + ctx->KT.entries) + 80.0 * (double)N;
         double frac = hw_bytes > 0 ? std::min(0.5, std::max(0.0, (60e6 - other) / hw_bytes)) : 0.0;
-        if (e_) frac = atoi(e_) / 100.0;
         const int64_t tiles_per_cta = ((ctx->K.nslices + ctx->cg_grid - 1) / ctx->cg_grid);
         P.hw_res_tiles = (int32_t)((double)tiles_per_cta * frac);
     } P.rep = ctx->d_cgrep;
@@ -359,7 +354,6 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     CU(cudaMemsetAsync(ctx->p1, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->z, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
-    CU(cudaMemsetAsync(ctx->flags, 0, sizeof(unsigned int) * ctx->cg_grid, ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
     const int variant = ctx->opt.alg1_variant;
@@ -552,7 +546,6 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v3 does not fit an SM (occupancy 0)");
     ctx->cg_grid = ctx->num_sms;
     RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
-    RDTRY(dalloc(ctx, &ctx->flags, (size_t)ctx->cg_grid));
     // d = diag(H), dinv
     k_diag_H<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
         ctx->KT.view(), N, ctx->m, ctx->minv, ctx->sigma, ctx->opt.jacobi, ctx->d, ctx->dinv);
