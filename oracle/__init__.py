@@ -8,6 +8,7 @@ from .oracle import (  # noqa: F401
     OracleOptions,
     build_oracle,
     reference_eigs,
+    sine_reference,
     JACOBI_CG,
     REFDEF,
     ZEROEXT,

@@ -9,6 +9,7 @@ PAPER.md:382), computed with a library eigensolver on the assembled matrix.
 from __future__ import annotations
 
 import ctypes as C
+import itertools
 import os
 import subprocess
 from dataclasses import dataclass
@@ -305,3 +306,46 @@ def reference_eigs(rowptr, colidx, val, m, sigma, k, dense_below: int = 1500):
     th, V = spla.eigsh((H / scale).tocsc(), k=k, sigma=0.0, which="LM", tol=1e-12)
     order = np.argsort(th)
     return th[order] * scale, np.asfortranarray(V[:, order])
+
+
+def sine_reference(dims, k):
+    """Analytical Cartesian spatial reference (NEXT-1 of SURVEY.md 8(f)): section 2.2.3, eq. (15),
+    restated for the cell-centred grids of workloads/ (the paper's grid is node-centred; pin P7 fixes the
+    cell-centred form against the assembled operator).
+
+    For axis a with n_a cells, the 1-D factors and Laplacian eigenvalues (h_a = 1/n_a) are
+        v_q(j) = sqrt(2/n_a) sin(pi q (j - 1/2)/n_a)   (sqrt(1/n_a) for q = n_a),     j, q = 1..n_a
+        mu_q   = 4 n_a^2 sin^2(pi q / (2 n_a)).
+    A product phi = v_{q_1} (x) ... (x) v_{q_d} (x fastest) has Laplacian eigenvalue mu = sum_a mu_{q_a}.  "We retain
+    the r lowest products.  Lexicographic ordering fixes the choice within repeated eigenvalues":
+    sorted by (mu, q_1, ..., q_d), where mu is summed over the per-axis terms in ascending order of the terms so that
+    permuted index tuples tie exactly (reading A18).
+
+    Returns (modes, mu, W): modes int (k, d), mu (k,), W (N, k) column-major with orthonormal columns."""
+    dims = [int(n) for n in dims]
+    d = len(dims)
+    N = int(np.prod(dims))
+    if not (1 <= k <= N):
+        raise ValueError("k out of range")
+    terms = [4.0 * n * n * np.sin(np.pi * np.arange(1, min(n, k) + 1) / (2.0 * n)) ** 2 for n in dims]
+    cand = []
+    for q in itertools.product(*[range(1, len(t) + 1) for t in terms]):  # q = (q_1, ..., q_d), q_1 = x index
+        parts = sorted(terms[a][q[a] - 1] for a in range(d))
+        mu = 0.0
+        for p in parts:
+            mu += p
+        cand.append((mu, q))
+    cand.sort()
+    cand = cand[:k]
+    modes = np.array([q for _, q in cand], dtype=np.int32).reshape(k, d)
+    mu = np.array([m for m, _ in cand])
+    W = np.empty((N, k), order="F")
+    for c in range(k):
+        col = np.ones(1)
+        for a in range(d):  # x fastest: kron(v_{q_d}, ..., v_{q_1})
+            n, q = dims[a], int(modes[c, a])
+            j = np.arange(1, n + 1)
+            v = np.sqrt((1.0 if q == n else 2.0) / n) * np.sin(np.pi * q * (j - 0.5) / n)
+            col = np.kron(v, col)
+        W[:, c] = col
+    return modes, mu, W

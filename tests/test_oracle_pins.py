@@ -475,3 +475,57 @@ def test_golden_config1_unchanged(oracle_mod):
         assert [f"{s['active_hash']:016x}" for s in r["steps"]] == gm["active_hash"]
         assert [s["n_inactive"] for s in r["steps"]] == gm["n_inactive"]
         assert abs(np.sqrt((w.m * r["y"] ** 2).sum()) - gm["y_Mnorm"]) <= 1e-9 * gm["y_Mnorm"]
+
+
+# ------------------------------------------------------------------ NEXT-1: analytical Cartesian reference, eq. (15)
+def test_sine_reference_is_the_spectrum_of_the_homogeneous_operator(oracle_mod):
+    """PAPER.md:186-192 (cell-centred form): for uniform kappa and zero velocity the sine products ARE the lowest
+    eigenvectors of H, with theta = h^d + sigma (h^(d-2) mu h^2)^2 / h^d, in the order of the library eigensolver."""
+    n, k = 9, 7
+    w = make_steady_2d(n=n, channels=[], vel=0.0, alpha=1e-4, k=k, n_queries=1, n_bumps=1, psi_factor=0.6,
+                       pdas_cap=5, config=1)
+    o = oracle_mod.Oracle.from_workload(w)
+    modes, mu, W = oracle_mod.sine_reference((n, n), k)
+    assert np.allclose(W.T @ W, np.eye(k), atol=1e-13)
+    h = 1.0 / n
+    theta = h ** 2 + w.alpha * (mu * h ** 2) ** 2 / h ** 2  # K-eigenvalue = h^(d-2) * (mu h^2), d = 2
+    for c in range(k):
+        assert np.allclose(o.apply_H(W[:, c]), theta[c] * W[:, c], rtol=1e-11, atol=1e-13 * theta[c])
+    th, _ = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, k)
+    assert np.allclose(np.sort(theta), th, rtol=1e-9)
+    # selection and order: (mu, q_1, q_2) lexicographic; (1,2) before (2,1), which tie exactly
+    assert modes.tolist()[:4] == [[1, 1], [1, 2], [2, 1], [2, 2]]
+    assert mu[1] == mu[2] and (np.diff(mu) >= 0).all()
+    # the x index is the fastest: column of mode (2, 1) changes sign along x, not along y
+    col = W[:, 2].reshape(n, n)  # (y, x)
+    assert (np.sign(col[:, 0]) != np.sign(col[:, -1])).all() and (np.sign(col[0, :]) == np.sign(col[-1, :])).all()
+
+
+def test_sine_reference_3d_and_highest_mode(oracle_mod):
+    n, k = 4, 64  # every product of the 4^3 grid: a complete orthonormal basis, including q = n (norm sqrt(1/n))
+    modes, mu, W = oracle_mod.sine_reference((n, n, n), k)
+    assert np.allclose(W.T @ W, np.eye(k), atol=1e-13)
+    assert sorted(map(tuple, modes.tolist())) == sorted(itertools.product(range(1, n + 1), repeat=3))
+    w3 = make_steady_3d(n=n, bores=[], R=0.1, vpeak=0.0, alpha=1e-5, k=4, n_queries=1, n_bumps=1, psi_factor=0.6,
+                        pdas_cap=5, config=3)
+    o3 = oracle_mod.Oracle.from_workload(w3)
+    h = 1.0 / n
+    for c in (0, 5, 63):
+        theta = h ** 3 + w3.alpha * (h * mu[c] * h ** 2) ** 2 / h ** 3  # K-eigenvalue = h^(d-2) mu h^2, d = 3
+        assert np.allclose(o3.apply_H(W[:, c]), theta * W[:, c], rtol=1e-11, atol=1e-14 * theta)
+
+
+def test_sine_reference_deflates_the_heterogeneous_problem(oracle_mod):
+    """The reference is homogeneous, the CHT matrix keeps the conductivity interface and the transport
+    (PAPER.md:192): Algorithm 1 with it must still converge to the same solution, in fewer iterations than
+    Jacobi-CG on the twin of config 2."""
+    w = make_config(twin="c2_48")
+    o = oracle_mod.Oracle.from_workload(w)
+    _, _, W = oracle_mod.sine_reference(w.dims, w.k)
+    idx = np.arange(w.N)
+    b = w.m * w._target(1000 * w.config)
+    xj, rj = o.alg1(idx, b, np.zeros(w.N), None)
+    xs, rs = o.alg1(idx, b, np.zeros(w.N), W)
+    assert rj["status"] == rs["status"] == 0 and rs["rank_used"] == w.k
+    assert rs["iters"] < rj["iters"]
+    assert np.linalg.norm(xs - xj) <= 1e-5 * np.linalg.norm(xj)
