@@ -160,8 +160,8 @@ def load_profile():
 class Sequence:
     """The config's query sequence on one context: warm starts inside a pass, reset + reference rebuild on wrap."""
 
-    def __init__(self, g, w, method, ref_tol, qids):
-        self.g, self.w, self.method, self.ref_tol, self.qids = g, w, method, ref_tol, qids
+    def __init__(self, g, w, method, ref_tol, qids, reference="eig"):
+        self.g, self.w, self.method, self.ref_tol, self.qids, self.reference = g, w, method, ref_tol, qids, reference
         self.pos = 0
         self.ref_builds = 0
         self.ref_ms = 0.0
@@ -175,7 +175,11 @@ class Sequence:
     def begin_pass(self):
         self.g.reset_sequence()
         if self.method != 0:
-            _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
+            if self.reference == "sine":  # analytical Cartesian reference, PAPER.md:186-192 (steady grids only)
+                self.g.build_reference_sine(self.w.k, self.w.dims)
+                st = 0
+            else:
+                _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
             info = self.g.reference_info()
             self.ref_builds += 1
             self.ref_ms += info["build_ms"]
@@ -212,7 +216,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant), stream=stream.cuda_stream)
     tall = 2 if args.alg1_variant == 1 else 1
-    seq = Sequence(g, w, method, args.ref_tol, shard_queries(rank, world, w.n_queries))
+    seq = Sequence(g, w, method, args.ref_tol, shard_queries(rank, world, w.n_queries), args.reference)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
@@ -306,7 +310,7 @@ def run_ours(args):
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(mx_total / args.steps, 3),
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": f"replicas x{world}",
-                       "alg1_variant": args.alg1_variant, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
+                       "alg1_variant": args.alg1_variant, "reference": args.reference, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
                        "l2": "flushed between steps (256 MiB write); the deflated working set (W, HW, K, K^T) exceeds L2"},
             "e2e": {"value": round(e2e_value, 4), "unit": "s/query", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
@@ -353,8 +357,12 @@ def run_loop(args):
     tall = 2 if args.alg1_variant == 1 else 1
     ref = None
     if method != 0:
-        _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
-        ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
+        if args.reference == "sine":
+            g.build_reference_sine(w.k, w.dims)
+            ref = dict(g.reference_info(), kind="sine (PAPER.md:186-192)")
+        else:
+            _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
+            ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
     yd = w._target(1000 * w.config)
     b = torch.from_numpy(w.m * yd).to(dev)
     act = torch.zeros(w.N, dtype=torch.uint8, device=dev)
@@ -496,6 +504,9 @@ def main(argv=None):
     ap.add_argument("--twin", default=None)
     ap.add_argument("--method", default="refdef", choices=list(METHODS))
     ap.add_argument("--ref-tol", type=float, default=1e-3)
+    ap.add_argument("--reference", default="eig", choices=["eig", "sine"],
+                    help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
+                         "Cartesian reference (rd_build_reference_sine, steady configs 1, 2, 3, 5)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -145,6 +145,16 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
 /* Facts about the last rd_build_reference: block size b, total Chebyshev degree (each degree = one application
  * of H to all b columns), wall milliseconds.  Any pointer may be NULL. */
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms);
+/* The analytical Cartesian spatial reference of the paper (section 2.2.3, eq. (15)) for steady
+ * problems on a Cartesian grid of dims[0] x ... x dims[ndim-1] cells (ndim <= 3, x = dims[0] fastest, product = N,
+ * else RD_EINVAL): the k lowest products of the 1-D sine modes of the constant-coefficient Dirichlet Laplacian,
+ * v_q(j) = sqrt(2/n) sin(pi q (j + 1/2)/n) for the cell-centred grids used here (the paper's grid is node-centred),
+ * ordered by (mu, q_1, ..., q_d), mu = sum_a 4 n_a^2 sin^2(pi q_a/(2 n_a)) ("Lexicographic ordering fixes the choice
+ * within repeated eigenvalues").  The reference is homogeneous; the operator keeps its interfaces and transport.
+ * O(N k) work: replaces rd_build_reference when the grid is Cartesian.  mu_out: host, k doubles, may be NULL.
+ * modes_out: host, k x ndim int32 (row c = q_1..q_d of column c), may be NULL.  The build time is charged to the next
+ * query like rd_build_reference's. */
+int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, double* mu_out, int32_t* modes_out);
 /* Inject a reference (e.g. the oracle's): W is N x k column-major with leading dimension N. */
 int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W);
 /* Copy the stored reference out: W_out N x k column-major (ld N); returns k via k_out (0 if none). */

@@ -17,6 +17,7 @@
 #include "cg.cuh"
 #include "cg2.cuh"
 #include "cg3.cuh"
+#include "sine.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
 #include "pdas.cuh"
@@ -817,6 +818,86 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     if (status != RD_OK) fail(ctx, status, "reference not converged to tol %g in %d sweeps (worst residual %g)", tol, sweeps,
                               *std::max_element(resid.begin(), resid.begin() + k));
     return status;
+}
+
+int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, double* mu_out, int32_t* modes_out)
+{
+    if (!ctx || !dims || k < 1 || k > RD_MAX_K || ndim < 1 || ndim > 3) return RD_EINVAL;
+    int64_t prod = 1;
+    for (int a = 0; a < ndim; ++a) {
+        if (dims[a] < 1 || dims[a] > (1 << 20)) return fail(ctx, RD_EINVAL, "dims[%d] = %lld", a, (long long)dims[a]);
+        prod *= dims[a];
+    }
+    if (prod != ctx->N) return fail(ctx, RD_EINVAL, "product of dims %lld is not N = %lld (steady Cartesian grids only)", (long long)prod, (long long)ctx->N);
+    if (k > ctx->N) return fail(ctx, RD_EINVAL, "k = %d exceeds N = %lld", k, (long long)ctx->N);
+    const auto t_begin = std::chrono::steady_clock::now();
+    // ---- selection on the host: the k lowest products, ordered by (mu, q_1, ..., q_d); mu is summed over the
+    // per-axis terms in ascending order so that permuted tuples tie exactly (reading A18)
+    int qmax = 1;
+    std::vector<std::vector<double>> terms(ndim);
+    for (int a = 0; a < ndim; ++a) {
+        const int64_t n = dims[a];
+        const int qa = (int)std::min<int64_t>(n, k);
+        qmax = std::max(qmax, qa);
+        terms[a].resize(qa);
+        for (int q = 1; q <= qa; ++q) {
+            const double s = std::sin(M_PI * q / (2.0 * n));
+            terms[a][q - 1] = 4.0 * n * n * (s * s);
+        }
+    }
+    struct Cand { double mu; int q[3]; };
+    std::vector<Cand> cand;
+    const int q0n = (int)terms[0].size(), q1n = ndim > 1 ? (int)terms[1].size() : 1, q2n = ndim > 2 ? (int)terms[2].size() : 1;
+    cand.reserve((size_t)q0n * q1n * q2n);
+    for (int q0 = 1; q0 <= q0n; ++q0)
+        for (int q1 = 1; q1 <= q1n; ++q1)
+            for (int q2 = 1; q2 <= q2n; ++q2) {
+                double p[3] = {terms[0][q0 - 1], ndim > 1 ? terms[1][q1 - 1] : 0.0, ndim > 2 ? terms[2][q2 - 1] : 0.0};
+                std::sort(p, p + ndim);
+                double mu = 0.0;
+                for (int a = 0; a < ndim; ++a) mu += p[a];
+                cand.push_back(Cand{mu, {q0, q1, q2}});
+            }
+    std::sort(cand.begin(), cand.end(), [](const Cand& x, const Cand& y) {
+        if (x.mu != y.mu) return x.mu < y.mu;
+        if (x.q[0] != y.q[0]) return x.q[0] < y.q[0];
+        if (x.q[1] != y.q[1]) return x.q[1] < y.q[1];
+        return x.q[2] < y.q[2];
+    });
+    std::vector<int32_t> modes((size_t)k * 3);
+    for (int c = 0; c < k; ++c) {
+        for (int a = 0; a < 3; ++a) modes[(size_t)c * 3 + a] = cand[c].q[a];
+        if (mu_out) mu_out[c] = cand[c].mu;
+        if (modes_out) for (int a = 0; a < ndim; ++a) modes_out[(size_t)c * ndim + a] = cand[c].q[a];
+    }
+    // ---- tables and the product on the device
+    RDTRY(alloc_reference(ctx, k));
+    int nmax = 1;
+    for (int a = 0; a < ndim; ++a) nmax = std::max<int>(nmax, (int)dims[a]);
+    int32_t* d_modes = nullptr;
+    double* d_tab = nullptr;
+    const size_t tab_count = (size_t)ndim * qmax * nmax;
+    if (cudaMalloc(&d_modes, modes.size() * sizeof(int32_t)) != cudaSuccess || cudaMalloc(&d_tab, tab_count * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        if (d_modes) cudaFree(d_modes);
+        return fail(ctx, RD_ENOMEM, "cudaMalloc of the sine tables");
+    }
+    cudaError_t e = cudaMemcpyAsync(d_modes, modes.data(), modes.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream);
+    const int n0 = (int)dims[0], n1 = ndim > 1 ? (int)dims[1] : 1, n2 = ndim > 2 ? (int)dims[2] : 1;
+    k_sine_tables<<<grid_for((int64_t)tab_count, kThreads, 1024), kThreads, 0, ctx->stream>>>(ndim, qmax, nmax, n0, n1, n2, d_tab);
+    k_sine_product<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->N, ctx->ldw, ndim, qmax, nmax, n0, n1, k,
+                                                                                           ctx->kp, d_modes, d_tab, ctx->W);
+    ctx->launches += 2;
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_modes);
+    cudaFree(d_tab);
+    if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "sine reference: %s", cudaGetErrorString(e));
+    ctx->ref_degree = 0;
+    ctx->ref_block = k;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    return RD_OK;
 }
 
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms)

@@ -1,0 +1,89 @@
+"""GPU parity of the analytical Cartesian reference (NEXT-1; eq. (15), cell-centred form):
+rd_build_reference_sine against oracle.sine_reference, and RefDef queries driven by it against the oracle
+driven by the same reference."""
+import numpy as np
+import pytest
+
+from workloads import make_config, make_steady_2d
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def rd():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_17971_b200 as pkg
+
+    pkg.load_library()
+    return pkg
+
+
+CASES = {
+    "config1": lambda: make_config(1),
+    "c2_48": lambda: make_config(twin="c2_48"),
+    "c3_16": lambda: make_config(twin="c3_16"),
+    # ragged: N = 37^2 is not a multiple of 32
+    "ragged37": lambda: make_steady_2d(n=37, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-4, k=5, n_queries=2, n_bumps=3,
+                                       psi_factor=0.6, pdas_cap=60, config=1, name="ragged37"),
+}
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_sine_reference_matches_oracle(rd, oracle_mod, case):
+    w = CASES[case]()
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        mu, modes = g.build_reference_sine(w.k, w.dims)
+        modes_o, mu_o, W_o = oracle_mod.sine_reference(w.dims, w.k)
+        assert np.array_equal(modes, modes_o)  # integer work: the same products in the same order
+        assert np.allclose(mu, mu_o, rtol=1e-14, atol=0)
+        W = g.get_reference()
+        assert W.shape == (w.N, w.k)
+        assert np.abs(W - W_o).max() <= 1e-14  # entries are O(1/sqrt(N)) products of sines; sinpi vs sin(pi x)
+        assert np.allclose(W.T @ W, np.eye(w.k), atol=1e-12)
+    finally:
+        g.close()
+
+
+def test_sine_reference_rejects_wrong_grids(rd):
+    w = make_config(1)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        with pytest.raises(rd.RefDefError):
+            g.build_reference_sine(w.k, (31, 32))  # product != N
+        with pytest.raises(rd.RefDefError):
+            g.build_reference_sine(w.k, (4, 4, 8, 8))  # more than three axes
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("case", ["config1", "c2_48", "c3_16"])
+def test_query_parity_with_sine_reference(rd, oracle_mod, case):
+    """The whole path (S1-S7) with the analytical reference: same active-set sequence, y and u within 1e-6 (M-norm),
+    iteration counts within 5 % of the oracle run with oracle.sine_reference."""
+    w = CASES[case]()
+    o = oracle_mod.Oracle.from_workload(w)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        g.build_reference_sine(w.k, w.dims)
+        _, _, W_o = oracle_mod.sine_reference(w.dims, w.k)
+        yd, psi = w.target(0)
+        ro = o.solve_query(1, yd, psi, W_o, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        rg = g.solve_query(1, yd, psi)
+        assert rg["status"] == ro["status"] and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"])
+        for sg, so in zip(rg["steps"], ro["steps"]):
+            assert sg["status"] == so["status"] == 0 and sg["rel_resid_verified"] <= 1e-8
+            assert sg["rank_used"] == so["rank_used"]
+            assert abs(sg["cg_iters"] - so["cg_iters"]) <= max(3, 0.05 * so["cg_iters"])
+
+        def rel_m(a, b):
+            return float(np.sqrt((w.m * (a - b) ** 2).sum() / (w.m * b * b).sum()))
+
+        assert rel_m(rg["y"], ro["y"]) <= 1e-6 and rel_m(rg["u"], ro["u"]) <= 1e-6
+        assert rg["t_reference_ms"] > 0.0  # the build is charged to this first query
+    finally:
+        g.close()
