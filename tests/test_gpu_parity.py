@@ -295,3 +295,38 @@ def test_alg1_kernel_variants_agree(setup, rd, method):
         assert abs(r["iters"] - r_ref["iters"]) <= max(3, 0.05 * r_ref["iters"]), (variant, r["iters"], r_ref["iters"])
         assert (x[act == 1] == 0).all()
         assert np.linalg.norm(x - x_ref) <= 1e-6 * np.linalg.norm(x_ref)
+
+
+@pytest.mark.parametrize("k", [1, 9, 17, 24, 33, 41, 57, 64])
+def test_alg1_every_tile_width(rd, oracle_mod, k):
+    """Every padded rank kp = 8..64 changes the geometry of the TMA ring (tile = 256 kp bytes, min(32, 512/kp) slots,
+    one or two columns per lane in the transposed pass): a seeded random reference of k columns, GPU against oracle
+    (iterations, rank, solution) and against the literal-recurrence kernel."""
+    w = make_steady_2d(n=61, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-4, k=8, n_queries=1, n_bumps=3, psi_factor=0.6,
+                       pdas_cap=20, config=1, name="n61")  # N = 3721: 117 slices, ragged tail
+    o = oracle_mod.Oracle.from_workload(w)
+    rng = np.random.default_rng(1000 + k)
+    W = rng.standard_normal((w.N, k))
+    act = (rng.random(w.N) < 0.3).astype(np.uint8)
+    idx = np.flatnonzero(act == 0)
+    b = np.where(act == 0, w.m * rng.standard_normal(w.N), 0.0)
+    x0 = np.zeros(w.N)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        g.set_reference(W)
+        xg, rg = g.solve_inactive(1, act, b, x0)
+        g.set_options(rd.Options(pdas_cap=w.pdas_cap, alg1_variant=1))
+        xl, rl = g.solve_inactive(1, act, b, x0)
+    finally:
+        g.close()
+    xo, ro = o.alg1(idx, b[idx], x0[idx], W[idx])
+    assert rg["status"] == ro["status"] == rl["status"] == 0
+    assert rg["rank_used"] == ro["rank_used"] == k
+    assert rg["rel_resid_verified"] <= 1e-8
+    assert abs(rg["iters"] - ro["iters"]) <= max(3, 0.05 * ro["iters"]), (rg["iters"], ro["iters"])
+    assert (xg[act == 1] == 0).all()
+    xt, _ = o.alg1(idx, b[idx], x0[idx], W[idx], eps=1e-13)
+    ref_err = np.linalg.norm(xo - xt) / np.linalg.norm(xt)
+    got_err = np.linalg.norm(xg[idx] - xt) / np.linalg.norm(xt)
+    assert got_err <= max(10 * ref_err, 1e-9), (got_err, ref_err)
+    assert np.linalg.norm(xg - xl) <= 1e-6 * np.linalg.norm(xl)
