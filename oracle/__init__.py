@@ -9,6 +9,7 @@ from .oracle import (  # noqa: F401
     build_oracle,
     reference_eigs,
     sine_reference,
+    spacetime_reference,
     JACOBI_CG,
     REFDEF,
     ZEROEXT,

@@ -349,3 +349,52 @@ def sine_reference(dims, k):
             col = np.kron(v, col)
         W[:, c] = col
     return modes, mu, W
+
+
+def temporal_sign(q):
+    """Fixed sign of a temporal eigenvector: the component of largest magnitude (lowest index on ties) is positive."""
+    j = int(np.argmax(np.abs(q)))
+    return q if q[j] > 0 else -q
+
+
+def spacetime_reference(dims, nt, dt, k):
+    """Mode-dependent temporal reference (NEXT-2 of SURVEY.md 8(f)): section 2.2.4, eq. (16)-(17),
+    for the backward-Euler all-at-once operator of workloads/ (K_st = I (x) K_s + L (x) M_s, L lower bidiagonal with
+    1/dt and -1/dt, capacity c_0 = 1, W_t = I).
+
+    Homogeneous reference operator: A_0 = I (x) L_s + L (x) I with L_s the constant-coefficient Dirichlet Laplacian
+    (eq. (16)); for a spatial sine mode phi_i with Laplacian eigenvalue mu_i (sine_reference), eq. (17) reads
+        H_i = W_t + alpha (mu_i I + L)^T W_t (mu_i I + L),   H_i q_{i,j} = nu_{i,j} q_{i,j},
+    and q_{i,j} (x) phi_i is an eigenvector of eq. (16).  H_i and S_i = (mu_i I + L)^T (mu_i I + L) share eigenvectors
+    and nu = h^d (1 + alpha s) is increasing in s, so candidates are ordered by s (no alpha needed).  "The
+    construction considers the first min(r, N_s) spatial modes ... We order the candidate pairs by nu and retain a
+    total space-time rank r.  A fixed ordering resolves repeated eigenvalues": sorted by
+    (s, i, j), i the position of the spatial mode in sine_reference's order, j the index of s within S_i ascending.
+
+    Layout id = space + N_s * t: column = kron(q, phi).  Returns (pairs, s, W): pairs int (k, d + 1) = (q_1..q_d, j),
+    s (k,), W (N_s nt, k) column-major, orthonormal columns."""
+    dims = [int(n) for n in dims]
+    Ns = int(np.prod(dims))
+    rs = min(k, Ns)
+    modes, mu, Phi = sine_reference(dims, rs)
+    L = (np.eye(nt) - np.eye(nt, k=-1)) / dt
+    cand = []
+    Q = []
+    for i in range(rs):
+        B = mu[i] * np.eye(nt) + L
+        s, V = np.linalg.eigh(B.T @ B)
+        Q.append(V)
+        for j in range(nt):
+            cand.append((s[j], i, j))
+    cand.sort()
+    cand = cand[:k]
+    d = len(dims)
+    pairs = np.zeros((k, d + 1), dtype=np.int32)
+    svals = np.zeros(k)
+    W = np.empty((Ns * nt, k), order="F")
+    for c, (s, i, j) in enumerate(cand):
+        pairs[c, :d] = modes[i]
+        pairs[c, d] = j
+        svals[c] = s
+        W[:, c] = np.kron(temporal_sign(Q[i][:, j]), Phi[:, i])
+    return pairs, svals, W

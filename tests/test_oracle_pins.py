@@ -529,3 +529,42 @@ def test_sine_reference_deflates_the_heterogeneous_problem(oracle_mod):
     assert rj["status"] == rs["status"] == 0 and rs["rank_used"] == w.k
     assert rs["iters"] < rj["iters"]
     assert np.linalg.norm(xs - xj) <= 1e-5 * np.linalg.norm(xj)
+
+
+# ------------------------------------------------------------------ NEXT-2: mode-dependent temporal reference, eq. (16)-(17)
+def test_spacetime_reference_is_the_spectrum_of_the_homogeneous_operator(oracle_mod):
+    """q (x) phi are eigenvectors of the homogeneous all-at-once reduced Hessian with
+    nu = h^d (1 + alpha s); the k retained pairs are its k lowest eigenpairs (library eigensolver on the assembled H)."""
+    from workloads import make_spacetime_2d
+
+    n, nt, T, k = 6, 5, 1.0, 9
+    w = make_spacetime_2d(n=n, nt=nt, T=T, channels=[], vel=0.0, alpha=1e-4, k=k, n_queries=1, n_bumps=1,
+                          psi_factor=0.6, pdas_cap=5, config=4)
+    o = oracle_mod.Oracle.from_workload(w)
+    pairs, s, W = oracle_mod.spacetime_reference((n, n), nt, T / nt, k)
+    assert W.shape == (n * n * nt, k) and np.allclose(W.T @ W, np.eye(k), atol=1e-12)
+    hd = (1.0 / n) ** 2
+    nu = hd * (1.0 + w.alpha * s)
+    for c in range(k):
+        assert np.allclose(o.apply_H(W[:, c]), nu[c] * W[:, c], rtol=1e-10, atol=1e-12 * nu[c])
+    th, _ = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, k)
+    assert np.allclose(nu, th, rtol=1e-9) and (np.diff(s) >= 0).all()
+    # the temporal vector depends on the spatial eigenvalue (PAPER.md:200): same j, different mode, different q
+    assert pairs[0].tolist() == [1, 1, 0]
+    # sign convention and layout: time is the slow index
+    col = W[:, 0].reshape(nt, n * n)
+    q = col[:, 0] / col[0, 0] * abs(col[0, 0])
+    assert np.abs(q).argmax() == np.abs(col).sum(axis=1).argmax() and col[np.abs(q).argmax()].sum() > 0
+
+
+def test_spacetime_reference_deflates_the_twin_of_config4(oracle_mod):
+    w = make_config(twin="c4_32x8")
+    o = oracle_mod.Oracle.from_workload(w)
+    _, _, W = oracle_mod.spacetime_reference(w.dims, w.nt, 1.0 / w.nt, w.k)
+    idx = np.arange(w.N)
+    b = w.m * w._target(1000 * w.config)
+    xj, rj = o.alg1(idx, b, np.zeros(w.N), None)
+    xs, rs = o.alg1(idx, b, np.zeros(w.N), W)
+    assert rj["status"] == rs["status"] == 0 and rs["rank_used"] == w.k
+    assert rs["iters"] < rj["iters"]
+    assert np.linalg.norm(xs - xj) <= 1e-5 * np.linalg.norm(xj)
