@@ -149,6 +149,15 @@ def workload_name(args, w):
            f", N={w.N}, k={w.k}, {w.n_queries} queries/sequence, PDAS cap {w.pdas_cap}"
 
 
+def build_analytical_reference(g, w):
+    """The paper's closed-form references: sine products on steady Cartesian grids (section 2.2.3), sine products
+    paired with per-mode temporal eigenvectors on the all-at-once transient grid (section 2.2.4; horizon T = 1)."""
+    if w.nt > 1:
+        g.build_reference_spacetime(w.k, w.dims, w.nt, 1.0 / w.nt)
+    else:
+        g.build_reference_sine(w.k, w.dims)
+
+
 def load_profile():
     p = os.path.join(ROOT, "profiles", "bench_workload_profile.json")
     if os.path.exists(p):
@@ -175,8 +184,8 @@ class Sequence:
     def begin_pass(self):
         self.g.reset_sequence()
         if self.method != 0:
-            if self.reference == "sine":  # analytical Cartesian reference, PAPER.md:186-192 (steady grids only)
-                self.g.build_reference_sine(self.w.k, self.w.dims)
+            if self.reference == "sine":  # analytical references of the paper: PAPER.md:186-192 (steady), :194-208 (transient)
+                build_analytical_reference(self.g, self.w)
                 st = 0
             else:
                 _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
@@ -358,8 +367,8 @@ def run_loop(args):
     ref = None
     if method != 0:
         if args.reference == "sine":
-            g.build_reference_sine(w.k, w.dims)
-            ref = dict(g.reference_info(), kind="sine (PAPER.md:186-192)")
+            build_analytical_reference(g, w)
+            ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
         else:
             _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
             ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
@@ -506,7 +515,7 @@ def main(argv=None):
     ap.add_argument("--ref-tol", type=float, default=1e-3)
     ap.add_argument("--reference", default="eig", choices=["eig", "sine"],
                     help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
-                         "Cartesian reference (rd_build_reference_sine, steady configs 1, 2, 3, 5)")
+                         "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

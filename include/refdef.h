@@ -155,6 +155,17 @@ int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, 
  * modes_out: host, k x ndim int32 (row c = q_1..q_d of column c), may be NULL.  The build time is charged to the next
  * query like rd_build_reference's. */
 int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, double* mu_out, int32_t* modes_out);
+/* The mode-dependent temporal reference of the paper (section 2.2.4, eq. (16)-(17)) for the
+ * backward-Euler all-at-once operator K_st = I (x) K_s + L (x) M_s on a Cartesian grid of dims cells (ndim <= 3) and nt
+ * uniform slabs of length dt (product of dims x nt = N, ordering space + N_s * time, else RD_EINVAL; nt <= 256).
+ * For each of the first min(k, N_s) spatial sine modes phi_i (Laplacian eigenvalue mu_i, rd_build_reference_sine's
+ * order) the temporal matrix S_i = (mu_i I + L)^T (mu_i I + L) is diagonalised (it shares its eigenvectors with H_i of
+ * eq. (17); capacity c_0 = 1, W_t = I); the candidate pairs are ordered by (s, i, j) and the k lowest retained;
+ * column c of the reference is q_{i,j} (x) phi_i, each q with its largest-magnitude component positive.
+ * s_out: host, k doubles (reference eigenvalue nu = h^d (1 + sigma s)), may be NULL.  pairs_out: host, k x (ndim + 1)
+ * int32 (q_1..q_d of the spatial mode, then j), may be NULL.  Build time charged to the next query. */
+int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt,
+                                 double* s_out, int32_t* pairs_out);
 /* Inject a reference (e.g. the oracle's): W is N x k column-major with leading dimension N. */
 int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W);
 /* Copy the stored reference out: W_out N x k column-major (ld N); returns k via k_out (0 if none). */

@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_sine", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
 
 
@@ -100,6 +100,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
     lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
+    lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
     lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
     lib.rd_set_reference.argtypes = [vp, i32, vp]
     lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
@@ -221,6 +222,16 @@ class RefDef:
                                                       modes.ctypes.data), "rd_build_reference_sine")
         self.k = k
         return mu, modes
+
+    def build_reference_spacetime(self, k, dims, nt, dt):
+        """Mode-dependent temporal reference.  Returns (s, pairs): pairs k x (d + 1) = (q_1..q_d, j)."""
+        dims = np.ascontiguousarray(dims, dtype=np.int64)
+        s = np.zeros(k)
+        pairs = np.zeros((k, len(dims) + 1), dtype=np.int32)
+        self._check(self._lib.rd_build_reference_spacetime(self._h, k, len(dims), dims.ctypes.data, nt, dt, s.ctypes.data,
+                                                           pairs.ctypes.data), "rd_build_reference_spacetime")
+        self.k = k
+        return s, pairs
 
     def reference_info(self):
         b, deg, ms = C.c_int32(0), C.c_int64(0), C.c_double(0)

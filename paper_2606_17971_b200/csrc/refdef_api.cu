@@ -387,6 +387,45 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     return RD_OK;
 }
 
+// The count lowest products of 1-D sine modes, ordered by (mu, q_1, ..., q_d); mu is summed over the per-axis terms in
+// ascending order so that permuted tuples tie exactly (reading A18).
+struct SineCand { double mu; int q[3]; };
+void select_sine_modes(int ndim, const int64_t* dims, int count, std::vector<SineCand>& cand, int* qmax_out)
+{
+    const int k = count;
+    int qmax = 1;
+    std::vector<std::vector<double>> terms(ndim);
+    for (int a = 0; a < ndim; ++a) {
+        const int64_t n = dims[a];
+        const int qa = (int)std::min<int64_t>(n, k);
+        qmax = std::max(qmax, qa);
+        terms[a].resize(qa);
+        for (int q = 1; q <= qa; ++q) {
+            const double s = std::sin(M_PI * q / (2.0 * n));
+            terms[a][q - 1] = 4.0 * n * n * (s * s);
+        }
+    }
+    const int q0n = (int)terms[0].size(), q1n = ndim > 1 ? (int)terms[1].size() : 1, q2n = ndim > 2 ? (int)terms[2].size() : 1;
+    cand.reserve((size_t)q0n * q1n * q2n);
+    for (int q0 = 1; q0 <= q0n; ++q0)
+        for (int q1 = 1; q1 <= q1n; ++q1)
+            for (int q2 = 1; q2 <= q2n; ++q2) {
+                double p[3] = {terms[0][q0 - 1], ndim > 1 ? terms[1][q1 - 1] : 0.0, ndim > 2 ? terms[2][q2 - 1] : 0.0};
+                std::sort(p, p + ndim);
+                double mu = 0.0;
+                for (int a = 0; a < ndim; ++a) mu += p[a];
+                cand.push_back(SineCand{mu, {q0, q1, q2}});
+            }
+    std::sort(cand.begin(), cand.end(), [](const SineCand& x, const SineCand& y) {
+        if (x.mu != y.mu) return x.mu < y.mu;
+        if (x.q[0] != y.q[0]) return x.q[0] < y.q[0];
+        if (x.q[1] != y.q[1]) return x.q[1] < y.q[1];
+        return x.q[2] < y.q[2];
+    });
+    cand.resize(std::min<size_t>(cand.size(), (size_t)count));
+    if (qmax_out) *qmax_out = qmax;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -834,36 +873,8 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
     // ---- selection on the host: the k lowest products, ordered by (mu, q_1, ..., q_d); mu is summed over the
     // per-axis terms in ascending order so that permuted tuples tie exactly (reading A18)
     int qmax = 1;
-    std::vector<std::vector<double>> terms(ndim);
-    for (int a = 0; a < ndim; ++a) {
-        const int64_t n = dims[a];
-        const int qa = (int)std::min<int64_t>(n, k);
-        qmax = std::max(qmax, qa);
-        terms[a].resize(qa);
-        for (int q = 1; q <= qa; ++q) {
-            const double s = std::sin(M_PI * q / (2.0 * n));
-            terms[a][q - 1] = 4.0 * n * n * (s * s);
-        }
-    }
-    struct Cand { double mu; int q[3]; };
-    std::vector<Cand> cand;
-    const int q0n = (int)terms[0].size(), q1n = ndim > 1 ? (int)terms[1].size() : 1, q2n = ndim > 2 ? (int)terms[2].size() : 1;
-    cand.reserve((size_t)q0n * q1n * q2n);
-    for (int q0 = 1; q0 <= q0n; ++q0)
-        for (int q1 = 1; q1 <= q1n; ++q1)
-            for (int q2 = 1; q2 <= q2n; ++q2) {
-                double p[3] = {terms[0][q0 - 1], ndim > 1 ? terms[1][q1 - 1] : 0.0, ndim > 2 ? terms[2][q2 - 1] : 0.0};
-                std::sort(p, p + ndim);
-                double mu = 0.0;
-                for (int a = 0; a < ndim; ++a) mu += p[a];
-                cand.push_back(Cand{mu, {q0, q1, q2}});
-            }
-    std::sort(cand.begin(), cand.end(), [](const Cand& x, const Cand& y) {
-        if (x.mu != y.mu) return x.mu < y.mu;
-        if (x.q[0] != y.q[0]) return x.q[0] < y.q[0];
-        if (x.q[1] != y.q[1]) return x.q[1] < y.q[1];
-        return x.q[2] < y.q[2];
-    });
+    std::vector<SineCand> cand;
+    select_sine_modes(ndim, dims, k, cand, &qmax);
     std::vector<int32_t> modes((size_t)k * 3);
     for (int c = 0; c < k; ++c) {
         for (int a = 0; a < 3; ++a) modes[(size_t)c * 3 + a] = cand[c].q[a];
@@ -893,6 +904,97 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
     cudaFree(d_modes);
     cudaFree(d_tab);
     if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "sine reference: %s", cudaGetErrorString(e));
+    ctx->ref_degree = 0;
+    ctx->ref_block = k;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    return RD_OK;
+}
+
+int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt, double* s_out,
+                                 int32_t* pairs_out)
+{
+    if (!ctx || !dims || k < 1 || k > RD_MAX_K || ndim < 1 || ndim > 3 || nt < 1 || nt > RD_DENSE_MAXN || !(dt > 0.0)) return RD_EINVAL;
+    int64_t Ns = 1;
+    for (int a = 0; a < ndim; ++a) {
+        if (dims[a] < 1 || dims[a] > (1 << 20)) return fail(ctx, RD_EINVAL, "dims[%d] = %lld", a, (long long)dims[a]);
+        Ns *= dims[a];
+    }
+    if (Ns * nt != ctx->N) return fail(ctx, RD_EINVAL, "product of dims x nt = %lld is not N = %lld", (long long)(Ns * nt), (long long)ctx->N);
+    if (k > ctx->N) return fail(ctx, RD_EINVAL, "k = %d exceeds N = %lld", k, (long long)ctx->N);
+    const auto t_begin = std::chrono::steady_clock::now();
+    // ---- the first min(k, N_s) spatial modes and their Laplacian eigenvalues
+    const int rs = (int)std::min<int64_t>(k, Ns);
+    int qmax = 1;
+    std::vector<SineCand> cand;
+    select_sine_modes(ndim, dims, rs, cand, &qmax);
+    std::vector<int32_t> modes((size_t)rs * 3);
+    std::vector<double> mu(rs);
+    for (int i = 0; i < rs; ++i) {
+        for (int a = 0; a < 3; ++a) modes[(size_t)i * 3 + a] = cand[i].q[a];
+        mu[i] = cand[i].mu;
+    }
+    RDTRY(alloc_reference(ctx, k));
+    int nmax = 1;
+    for (int a = 0; a < ndim; ++a) nmax = std::max<int>(nmax, (int)dims[a]);
+    const size_t tab_count = (size_t)ndim * qmax * nmax, tt = (size_t)rs * nt * nt;
+    struct Scratch {
+        std::vector<void*> p;
+        ~Scratch() { for (void* q : p) cudaFree(q); }
+    } scratch;
+    auto salloc = [&](void** out, size_t bytes) -> int {
+        if (cudaMalloc(out, std::max<size_t>(bytes, 16)) != cudaSuccess) { cudaGetLastError(); return fail(ctx, RD_ENOMEM, "cudaMalloc(%zu)", bytes); }
+        scratch.p.push_back(*out);
+        return RD_OK;
+    };
+    int32_t *d_modes = nullptr, *d_sel = nullptr;
+    double *d_tab = nullptr, *d_mu = nullptr, *d_A = nullptr, *d_V = nullptr, *d_s = nullptr, *d_Q = nullptr;
+    RDTRY(salloc((void**)&d_modes, modes.size() * sizeof(int32_t)));
+    RDTRY(salloc((void**)&d_sel, (size_t)2 * k * sizeof(int32_t)));
+    RDTRY(salloc((void**)&d_tab, tab_count * sizeof(double)));
+    RDTRY(salloc((void**)&d_mu, rs * sizeof(double)));
+    RDTRY(salloc((void**)&d_A, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_V, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_s, (size_t)rs * nt * sizeof(double)));
+    RDTRY(salloc((void**)&d_Q, tt * sizeof(double)));
+    CU(cudaMemcpyAsync(d_modes, modes.data(), modes.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d_mu, mu.data(), rs * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    const int n0 = (int)dims[0], n1 = ndim > 1 ? (int)dims[1] : 1, n2 = ndim > 2 ? (int)dims[2] : 1;
+    k_sine_tables<<<grid_for((int64_t)tab_count, kThreads, 1024), kThreads, 0, ctx->stream>>>(ndim, qmax, nmax, n0, n1, n2, d_tab);
+    // ---- temporal eigenproblems of eq. (17), one CTA per spatial mode
+    k_temporal_eigs<<<rs, 256, 0, ctx->stream>>>(nt, 1.0 / dt, d_mu, d_A, d_V, d_s, d_Q);
+    ctx->launches += 2;
+    std::vector<double> s_all((size_t)rs * nt);
+    CU(cudaMemcpyAsync(s_all.data(), d_s, s_all.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    // ---- ordered selection of the k lowest pairs: (s, i, j) ("order the candidate pairs by nu ... A
+    // fixed ordering resolves repeated eigenvalues"; nu = h^d (1 + alpha s) is increasing in s)
+    struct Pair { double s; int i, j; };
+    std::vector<Pair> pr;
+    pr.reserve(s_all.size());
+    for (int i = 0; i < rs; ++i)
+        for (int j = 0; j < nt; ++j) pr.push_back(Pair{s_all[(size_t)i * nt + j], i, j});
+    std::sort(pr.begin(), pr.end(), [](const Pair& x, const Pair& y) {
+        if (x.s != y.s) return x.s < y.s;
+        if (x.i != y.i) return x.i < y.i;
+        return x.j < y.j;
+    });
+    std::vector<int32_t> sel((size_t)2 * k);
+    for (int c = 0; c < k; ++c) {
+        sel[2 * c] = pr[c].i;
+        sel[2 * c + 1] = pr[c].j;
+        if (s_out) s_out[c] = pr[c].s;
+        if (pairs_out) {
+            for (int a = 0; a < ndim; ++a) pairs_out[(size_t)c * (ndim + 1) + a] = modes[(size_t)pr[c].i * 3 + a];
+            pairs_out[(size_t)c * (ndim + 1) + ndim] = pr[c].j;
+        }
+    }
+    CU(cudaMemcpyAsync(d_sel, sel.data(), sel.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    k_kron_product<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(Ns, nt, ctx->ldw, ndim, qmax, nmax, n0, n1, k, ctx->kp,
+                                                                                           d_modes, d_sel, d_tab, d_Q, ctx->W);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
     ctx->ref_degree = 0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();

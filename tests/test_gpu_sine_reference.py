@@ -87,3 +87,77 @@ def test_query_parity_with_sine_reference(rd, oracle_mod, case):
         assert rg["t_reference_ms"] > 0.0  # the build is charged to this first query
     finally:
         g.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: mode-dependent temporal reference
+ST_CASES = {
+    "c4_32x8": lambda: make_config(twin="c4_32x8"),
+}
+
+
+def _st_small():
+    from workloads import make_spacetime_2d
+
+    # ragged: N = 13 * 13 * 5 = 845 is not a multiple of 32; nt odd (a bye round in the Jacobi ordering)
+    return make_spacetime_2d(n=13, nt=5, T=1.0, channels=[(0.4, 0.6)], vel=20.0, alpha=1e-4, k=11, n_queries=1, n_bumps=2,
+                             psi_factor=0.6, pdas_cap=40, config=4, name="st13x5")
+
+
+ST_CASES["st13x5"] = _st_small
+
+
+@pytest.mark.parametrize("case", list(ST_CASES))
+def test_spacetime_reference_matches_oracle(rd, oracle_mod, case):
+    w = ST_CASES[case]()
+    dt = 1.0 / w.nt
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        s, pairs = g.build_reference_spacetime(w.k, w.dims, w.nt, dt)
+        pairs_o, s_o, W_o = oracle_mod.spacetime_reference(w.dims, w.nt, dt, w.k)
+        assert np.array_equal(pairs, pairs_o)  # the same (spatial mode, temporal index) pairs in the same order
+        assert np.allclose(s, s_o, rtol=1e-12, atol=0)
+        W = g.get_reference()
+        # Jacobi (device) against LAPACK (oracle) eigenvectors of well-separated 5..32-dimensional problems
+        assert np.abs(W - W_o).max() <= 1e-11
+        assert np.allclose(W.T @ W, np.eye(w.k), atol=1e-11)
+    finally:
+        g.close()
+
+
+def test_spacetime_reference_rejects_wrong_sizes(rd):
+    w = ST_CASES["st13x5"]()
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        with pytest.raises(rd.RefDefError):
+            g.build_reference_spacetime(w.k, w.dims, w.nt + 1, 0.2)
+        with pytest.raises(rd.RefDefError):
+            g.build_reference_spacetime(w.k, w.dims, w.nt, 0.0)
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("case", list(ST_CASES))
+def test_query_parity_with_spacetime_reference(rd, oracle_mod, case):
+    w = ST_CASES[case]()
+    dt = 1.0 / w.nt
+    o = oracle_mod.Oracle.from_workload(w)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        g.build_reference_spacetime(w.k, w.dims, w.nt, dt)
+        _, _, W_o = oracle_mod.spacetime_reference(w.dims, w.nt, dt, w.k)
+        yd, psi = w.target(0)
+        ro = o.solve_query(1, yd, psi, W_o, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        rg = g.solve_query(1, yd, psi)
+        assert rg["status"] == ro["status"] and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"])
+        for sg, so in zip(rg["steps"], ro["steps"]):
+            assert sg["status"] == so["status"] == 0 and sg["rel_resid_verified"] <= 1e-8
+            assert sg["rank_used"] == so["rank_used"]
+            assert abs(sg["cg_iters"] - so["cg_iters"]) <= max(3, 0.05 * so["cg_iters"])
+
+        def rel_m(a, b):
+            return float(np.sqrt((w.m * (a - b) ** 2).sum() / (w.m * b * b).sum()))
+
+        assert rel_m(rg["y"], ro["y"]) <= 1e-6 and rel_m(rg["u"], ro["u"]) <= 1e-6
+    finally:
+        g.close()
