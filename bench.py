@@ -414,6 +414,67 @@ def run_loop(args):
     return out
 
 
+def run_replay(args):
+    """--mode replay: the matched-replay protocol of the paper (Table 3 :438-451; NEXT-4 of SURVEY.md 8(f)).
+    A query sequence is run once with RefDef under the warm-start policy and every inactive system it meets is
+    recorded (active set and right-hand side b = l_I - H_IJ psi_J).  The SAME systems are then solved again from zero
+    initial guesses with direct restriction (eq. (12)), with zero-extension (eq. (13), history accumulating in replay
+    order) and with Jacobi-CG, all from the same reference: iterations, retained rank and seconds per transfer."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    import paper_2606_17971_b200 as pkg
+
+    pkg.load_library()
+    w = make_workload(args)
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant))
+    if args.reference == "sine":
+        build_analytical_reference(g, w)
+    else:
+        g.build_reference(w.k, tol=args.ref_tol, max_block_iters=60)
+    ref = g.reference_info()
+    systems = []
+    nq = min(w.n_queries, args.steps)
+    for q in range(nq):
+        yd, psi = w.target(q)
+        res = g.solve_query(1, yd, psi, want_sets=True)
+        ell = w.m * yd
+        nbytes = (w.N + 7) // 8
+        for st in range(res["n_steps"]):
+            bits = np.asarray(res["J_bits"][st * nbytes:(st + 1) * nbytes] if res["J_bits"].ndim == 1 else res["J_bits"][st], dtype=np.uint8)
+            act = np.unpackbits(bits, bitorder="little")[:w.N].astype(np.uint8)
+            if act.all():
+                continue  # empty inactive set: nothing to solve
+            b = np.where(act == 0, ell - g.apply_H(np.where(act == 1, psi, 0.0)), 0.0)
+            systems.append((act, b))
+    out_methods = {}
+    x0 = np.zeros(w.N)
+    for name in ("refdef", "zeroext", "jacobi"):
+        g.reset_sequence()
+        iters = ranks = 0
+        ms = 0.0
+        worst = 0.0
+        for act, b in systems:
+            _, r = g.solve_inactive(METHODS[name], act, b, x0)
+            iters += r["iters"]
+            ranks += r["rank_used"]
+            ms += r["t_iter_ms"]
+            worst = max(worst, r["rel_resid_verified"])
+        out_methods[name] = {"cg_iters": iters, "alg1_s": round(ms * 1e-3, 4), "mean_rank": round(ranks / max(len(systems), 1), 2),
+                             "worst_rel_resid": worst}
+    g.close()
+    base = out_methods["zeroext"]["cg_iters"]
+    return {"metric": "matched replay of the inactive systems of a sequence (PAPER.md:168, Table 3): CG iterations per transfer",
+            "value": out_methods["refdef"]["cg_iters"], "unit": "CG iterations (direct restriction)", "n_gpus": 1, "steps": nq, "warmup": 0,
+            "higher_is_better": False, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args, w), "mode": "replay", "queries": nq, "systems": len(systems),
+                       "reference": args.reference, "reference_build_ms": ref["build_ms"]},
+            "methods": out_methods,
+            "iteration_ratio_zeroext_over_direct": round(base / max(out_methods["refdef"]["cg_iters"], 1), 3)}
+
+
 # ----------------------------------------------------------------------------------------------- oracle legs
 def oracle_sample(w, method, W, iters_per_query, steps_per_query, budget_s, seed_qid=0):
     """Times the oracle, as it stands (single thread), on a bounded sample of one query of the workload: Algorithm 1
@@ -519,7 +580,8 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mode", default="query", choices=["query", "loop"], help="query: the metric; loop: the CG loop alone")
+    ap.add_argument("--mode", default="query", choices=["query", "loop", "replay"],
+                    help="query: the metric; loop: the CG loop alone; replay: matched replay of a sequence's inactive systems")
     ap.add_argument("--cg-cap", type=int, default=500000, help="--mode loop: iteration cap of each solve")
     ap.add_argument("--alg1-variant", type=int, default=0, help="rd_options.alg1_variant (0: default kernel; 1: literal recurrence)")
     ap.add_argument("--ref-sweeps", type=int, default=60, help="--mode loop: filter sweeps of the reference build")
@@ -528,6 +590,8 @@ def main(argv=None):
         out = run_reference(args)
     elif args.mode == "loop":
         out = run_loop(args)
+    elif args.mode == "replay":
+        out = run_replay(args)
     else:
         out = run_ours(args)
     if out is not None:

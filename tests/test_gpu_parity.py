@@ -330,3 +330,36 @@ def test_alg1_every_tile_width(rd, oracle_mod, k):
     got_err = np.linalg.norm(xg[idx] - xt) / np.linalg.norm(xt)
     assert got_err <= max(10 * ref_err, 1e-9), (got_err, ref_err)
     assert np.linalg.norm(xg - xl) <= 1e-6 * np.linalg.norm(xl)
+
+
+def test_operator_change_keeps_the_reference(rd, oracle_mod):
+    """Algorithm 2 steps 6-8: when the flow scale changes the operator is reassembled but the
+    reference is kept.  Here: reference built on the nominal operator (velocity 50), injected into a context of the
+    off-design operator (velocity 75) through rd_get_reference / rd_set_reference; the query on the new operator
+    must match the oracle run with the same retained reference, and deflation must still pay against Jacobi-CG."""
+    from workloads.cht import CH2
+
+    mk = lambda vel: make_steady_2d(n=48, channels=CH2, vel=vel, alpha=1e-4, k=16, n_queries=2, n_bumps=5,
+                                    psi_factor=0.55, pdas_cap=100, config=2, name=f"c2_48_v{vel:g}")
+    w_nom, w_off = mk(50.0), mk(75.0)
+    g_nom = rd.RefDef.from_workload(w_nom, rd.Options(pdas_cap=w_nom.pdas_cap))
+    g_off = rd.RefDef.from_workload(w_off, rd.Options(pdas_cap=w_off.pdas_cap))
+    try:
+        _, _, _, st = g_nom.build_reference(w_nom.k, tol=1e-6)
+        assert st == 0
+        W = g_nom.get_reference()
+        g_off.set_reference(W)
+        o = oracle_mod.Oracle.from_workload(w_off)
+        yd, psi = w_off.target(0)
+        ro = o.solve_query(1, yd, psi, W, oracle_mod.OracleOptions(pdas_cap=w_off.pdas_cap))
+        rg = g_off.solve_query(1, yd, psi)
+        assert rg["status"] == ro["status"] == 0 and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"])
+        assert _rel_m(w_off, rg["y"], ro["y"]) <= 1e-6 and _rel_m(w_off, rg["u"], ro["u"]) <= 1e-6
+        g_off.reset_sequence()
+        rj = g_off.solve_query(0, yd, psi)
+        assert rj["status"] == 0 and np.array_equal(rj["J_bits"], rg["J_bits"])
+        assert rg["total_cg_iters"] < rj["total_cg_iters"]
+    finally:
+        g_nom.close()
+        g_off.close()
