@@ -441,10 +441,8 @@ def run_replay(args):
         yd, psi = w.target(q)
         res = g.solve_query(1, yd, psi, want_sets=True)
         ell = w.m * yd
-        nbytes = (w.N + 7) // 8
         for st in range(res["n_steps"]):
-            bits = np.asarray(res["J_bits"][st * nbytes:(st + 1) * nbytes] if res["J_bits"].ndim == 1 else res["J_bits"][st], dtype=np.uint8)
-            act = np.unpackbits(bits, bitorder="little")[:w.N].astype(np.uint8)
+            act = np.unpackbits(res["J_bits"][st], bitorder="little")[:w.N].astype(np.uint8)  # packed LSB first
             if act.all():
                 continue  # empty inactive set: nothing to solve
             b = np.where(act == 0, ell - g.apply_H(np.where(act == 1, psi, 0.0)), 0.0)

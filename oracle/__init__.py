@@ -8,6 +8,7 @@ from .oracle import (  # noqa: F401
     OracleOptions,
     build_oracle,
     reference_eigs,
+    reference_eigs_scaled,
     sine_reference,
     spacetime_reference,
     JACOBI_CG,

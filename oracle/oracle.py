@@ -398,3 +398,32 @@ def spacetime_reference(dims, nt, dt, k):
         svals[c] = s
         W[:, c] = np.kron(temporal_sign(Q[i][:, j]), Phi[:, i])
     return pairs, svals, W
+
+
+def reference_eigs_scaled(rowptr, colidx, val, m, sigma, k, dense_below: int = 1500):
+    """Jacobi-scaled reference (NEXT-3 of SURVEY.md 8(f)): the k lowest pairs of the generalized problem
+    H w = mu D w, D = diag(H) -- the paper's "M_c phi_j = mu_j D_c phi_j supplies low modes in Jacobi-scaled
+    coordinates", each column then "normalized in the Euclidean norm", here on the fine operator (A13).
+
+    Returns (mu, W): mu ascending, W (N x k, column-major) with unit columns (not orthogonal: they are D-orthogonal
+    before the normalisation).  A library eigensolver on the assembled matrices."""
+    import scipy.linalg as sla
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+
+    N = len(m)
+    K = sp.csr_matrix((val, colidx, rowptr), shape=(N, N))
+    H = (sp.diags(m) + sigma * (K.T @ sp.diags(1.0 / np.asarray(m)) @ K)).tocsc()
+    H = 0.5 * (H + H.T)
+    d = H.diagonal()
+    if N <= dense_below:
+        mu, V = sla.eigh(H.toarray(), np.diag(d))
+        mu, V = mu[:k], V[:, :k]
+    else:
+        s = 1.0 / np.sqrt(d)
+        Hs = (sp.diags(s) @ H @ sp.diags(s)).tocsc()
+        mu, Vs = spla.eigsh(Hs, k=k, sigma=0.0, which="LM", tol=1e-12)
+        order = np.argsort(mu)
+        mu, V = mu[order], s[:, None] * Vs[:, order]
+    V = V / np.linalg.norm(V, axis=0)
+    return mu.copy(), np.asfortranarray(V)
