@@ -187,6 +187,8 @@ class Sequence:
             if self.reference == "sine":  # analytical references of the paper: PAPER.md:186-192 (steady), :194-208 (transient)
                 build_analytical_reference(self.g, self.w)
                 st = 0
+            elif self.reference == "eig-scaled":  # Jacobi-scaled generalized problem
+                _, _, _, st = self.g.build_reference_scaled(self.w.k, tol=self.ref_tol, max_block_iters=60)
             else:
                 _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
             info = self.g.reference_info()
@@ -370,7 +372,8 @@ def run_loop(args):
             build_analytical_reference(g, w)
             ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
         else:
-            _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
+            build = g.build_reference_scaled if args.reference == "eig-scaled" else g.build_reference
+            _, resid, sweeps, st = build(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
             ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
     yd = w._target(1000 * w.config)
     b = torch.from_numpy(w.m * yd).to(dev)
@@ -432,6 +435,8 @@ def run_replay(args):
     g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant))
     if args.reference == "sine":
         build_analytical_reference(g, w)
+    elif args.reference == "eig-scaled":
+        g.build_reference_scaled(w.k, tol=args.ref_tol, max_block_iters=60)
     else:
         g.build_reference(w.k, tol=args.ref_tol, max_block_iters=60)
     ref = g.reference_info()
@@ -572,7 +577,7 @@ def main(argv=None):
     ap.add_argument("--twin", default=None)
     ap.add_argument("--method", default="refdef", choices=list(METHODS))
     ap.add_argument("--ref-tol", type=float, default=1e-3)
-    ap.add_argument("--reference", default="eig", choices=["eig", "sine"],
+    ap.add_argument("--reference", default="eig", choices=["eig", "eig-scaled", "sine"],
                     help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
                          "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4)")
     ap.add_argument("--e2e-steps", type=int, default=1)

@@ -145,6 +145,14 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
 /* Facts about the last rd_build_reference: block size b, total Chebyshev degree (each degree = one application
  * of H to all b columns), wall milliseconds.  Any pointer may be NULL. */
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms);
+/* The Jacobi-scaled variant of rd_build_reference (the paper's "generalized eigenproblem M_c phi = mu D_c phi supplies
+ * low modes in Jacobi-scaled coordinates ... each column is normalized in the Euclidean norm", here on the
+ * fine operator): the k lowest pairs of H w = mu D w, D = diag(H), by the same block method applied to
+ * D^{-1/2} H D^{-1/2}; the stored reference has unit columns (D-orthogonal up to that scaling, not orthogonal: the
+ * coarse setup orthogonalises the restricted basis anyway).  Arguments and statuses as rd_build_reference; mu_out
+ * receives the generalized eigenvalues, the residual test is ||H w - mu D w|| in the scaled coordinates. */
+int rd_build_reference_scaled(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* mu_out,
+                              double* resid_out, int32_t* iters_out);
 /* The analytical Cartesian spatial reference of the paper (section 2.2.3, eq. (15)) for steady
  * problems on a Cartesian grid of dims[0] x ... x dims[ndim-1] cells (ndim <= 3, x = dims[0] fastest, product = N,
  * else RD_EINVAL): the k lowest products of the 1-D sine modes of the constant-coefficient Dirichlet Laplacian,

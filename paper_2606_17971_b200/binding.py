@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
 
 
@@ -99,6 +99,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_kernel_launches.restype = i64
     lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
     lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
+    lib.rd_build_reference_scaled.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
     lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
@@ -212,6 +213,17 @@ class RefDef:
                                                       resid.ctypes.data, C.byref(it)), "rd_build_reference", soft_ok=True)
         self.k = k
         return theta, resid, it.value, st
+
+    def build_reference_scaled(self, k, tol=1e-3, max_block_iters=200):
+        """Jacobi-scaled reference H w = mu D w.  Returns (mu, relative residuals, sweeps, status)."""
+        mu = np.zeros(k)
+        resid = np.zeros(k)
+        it = C.c_int32(0)
+        st = self._check(self._lib.rd_build_reference_scaled(self._h, k, tol, max_block_iters, mu.ctypes.data,
+                                                             resid.ctypes.data, C.byref(it)), "rd_build_reference_scaled",
+                         soft_ok=True)
+        self.k = k
+        return mu, resid, it.value, st
 
     def build_reference_sine(self, k, dims):
         """Analytical Cartesian reference: dims = cells per axis, x first.  Returns (mu, modes)."""

@@ -244,4 +244,45 @@ __global__ void __launch_bounds__(1024) k_rr_small(int b, const double* Ain, dou
     for (int j = threadIdx.x; j < b; j += blockDim.x) theta[j] = A[perm[j] + (size_t)perm[j] * b];
 }
 
+// ---- NEXT-3: Jacobi-scaled reference.  S H S with S = diag(H)^{-1/2} has the structure of H itself:
+// S H S = (S M S) + sigma (K S)^T M^{-1} (K S), so the eigensolver above runs unchanged on column-scaled copies of the
+// values of K (K S), row-scaled copies of the values of K^T (S K^T) and the diagonal m / d.
+__global__ void k_scale_ell(Ell A, int64_t N, const double* d, int by_row, double* val_out)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t s = gw; s < A.nslices; s += nwt) {
+        const int64_t row = s * RD_SLICE + lane;
+        const int64_t o = A.off[s];
+        const int wd = (int)((A.off[s + 1] - o) >> 5);
+        for (int e = 0; e < wd; ++e) {
+            const int64_t pos = o + e * 32 + lane;
+            const double a = A.val[pos];
+            double sc = 0.0;
+            if (row < N && a != 0.0) sc = rsqrt(by_row ? d[row] : d[A.col[pos]]);
+            val_out[pos] = a * sc;
+        }
+    }
+}
+__global__ void k_div(int64_t N, const double* a, const double* b, double* out)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) out[i] = a[i] / b[i];
+}
+// W[:, j] <- (d^{-1/2} . W[:, j]) / || d^{-1/2} . W[:, j] ||_2, one CTA per column (fixed-order reduction)
+__global__ void __launch_bounds__(1024) k_unscale_normalize(int64_t N, int64_t ld, const double* d, double* W)
+{
+    __shared__ double red[32];
+    double* col = W + (size_t)blockIdx.x * ld;
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += blockDim.x) {
+        const double v = col[i] * rsqrt(d[i]);
+        col[i] = v;
+        acc = fma(v, v, acc);
+    }
+    acc = block_sum(acc, red);
+    const double inv = acc > 0.0 ? rsqrt(acc) : 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += blockDim.x) col[i] *= inv;
+}
+
 }  // namespace rd

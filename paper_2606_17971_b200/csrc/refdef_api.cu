@@ -1002,6 +1002,49 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     return RD_OK;
 }
 
+int rd_build_reference_scaled(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* mu_out, double* resid_out,
+                              int32_t* iters_out)
+{
+    if (!ctx || k < 1 || k > RD_MAX_K || !(tol > 0.0) || max_block_iters < 1) return RD_EINVAL;
+    const int64_t N = ctx->N;
+    const auto t_begin = std::chrono::steady_clock::now();
+    double *kval = nullptr, *ktval = nullptr, *ms = nullptr;
+    auto release = [&]() { if (kval) cudaFree(kval); if (ktval) cudaFree(ktval); if (ms) cudaFree(ms); };
+    if (cudaMalloc(&kval, std::max<int64_t>(ctx->K.entries, 1) * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&ktval, std::max<int64_t>(ctx->KT.entries, 1) * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&ms, ctx->ldw * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        release();
+        return fail(ctx, RD_ENOMEM, "cudaMalloc of the scaled operator copies");
+    }
+    cudaMemsetAsync(ms, 0, ctx->ldw * sizeof(double), ctx->stream);
+    const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    k_scale_ell<<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->d, 0, kval);    // K S
+    k_scale_ell<<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->d, 1, ktval);  // S K^T
+    k_div<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(N, ctx->m, ctx->d, ms);  // S M S
+    ctx->launches += 3;
+    // the eigensolver of rd_build_reference on the scaled operator (same structure, see eigs.cuh)
+    double* const kval0 = ctx->K.val;
+    double* const ktval0 = ctx->KT.val;
+    double* const m0 = ctx->m;
+    ctx->K.val = kval; ctx->KT.val = ktval; ctx->m = ms;
+    const int rc = rd_build_reference(ctx, k, tol, max_block_iters, mu_out, resid_out, iters_out);
+    ctx->K.val = kval0; ctx->KT.val = ktval0; ctx->m = m0;
+    cudaError_t e = cudaSuccess;
+    if (rc == RD_OK || rc == RD_ECAP) {
+        // w = S v, each column normalised in the Euclidean norm
+        k_unscale_normalize<<<k, 1024, 0, ctx->stream>>>(N, ctx->ldw, ctx->d, ctx->W);
+        ctx->launches++;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    release();
+    if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "scaled reference: %s", cudaGetErrorString(e));
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    return rc;
+}
+
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms)
 {
     if (!ctx) return RD_EINVAL;

@@ -161,3 +161,57 @@ def test_query_parity_with_spacetime_reference(rd, oracle_mod, case):
         assert rel_m(rg["y"], ro["y"]) <= 1e-6 and rel_m(rg["u"], ro["u"]) <= 1e-6
     finally:
         g.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: Jacobi-scaled reference
+@pytest.mark.parametrize("case", ["config1", "c2_48", "ragged37"])
+def test_scaled_reference_matches_oracle(rd, oracle_mod, case):
+    w = CASES[case]()
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        mu, resid, sweeps, st = g.build_reference_scaled(w.k, tol=1e-7)
+        assert st == 0 and resid.max() <= 1e-7
+        mu_o, W_o = oracle_mod.reference_eigs_scaled(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+        assert np.allclose(mu, mu_o, rtol=1e-9)
+        W = g.get_reference()
+        assert np.allclose(np.linalg.norm(W, axis=0), 1.0, atol=1e-12)
+        # W is unique only up to rotation inside clusters: compare the subspaces of complete clusters (principal
+        # angles), cutting where the spectrum has a relative gap
+        cut = w.k
+        while cut > 1 and (mu_o[cut - 1] - mu_o[cut - 2]) < 1e-6 * mu_o[cut - 1]:
+            cut -= 1
+        cut -= 1 if cut == w.k and w.k > 1 else 0  # the last retained pair may share a cluster with the first dropped
+        Qa, _ = np.linalg.qr(W[:, :cut])
+        Qb, _ = np.linalg.qr(W_o[:, :cut])
+        sv = np.linalg.svd(Qa.T @ Qb, compute_uv=False)
+        assert sv.min() >= 1.0 - 1e-8
+        # generalized residual of every column against the oracle's operator
+        o = oracle_mod.Oracle.from_workload(w)
+        d = o.diag_H()
+        for c in range(w.k):
+            r = o.apply_H(W[:, c]) - mu[c] * d * W[:, c]
+            assert np.linalg.norm(r) <= 1e-6 * mu[c] * np.linalg.norm(d * W[:, c])
+    finally:
+        g.close()
+
+
+def test_query_parity_with_scaled_reference(rd, oracle_mod):
+    w = CASES["c2_48"]()
+    o = oracle_mod.Oracle.from_workload(w)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        _, _, _, st = g.build_reference_scaled(w.k, tol=1e-6)
+        assert st == 0
+        W = g.get_reference()
+        yd, psi = w.target(0)
+        ro = o.solve_query(1, yd, psi, W, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        rg = g.solve_query(1, yd, psi)
+        assert rg["status"] == ro["status"] == 0 and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"])
+        for sg, so in zip(rg["steps"], ro["steps"]):
+            assert sg["rank_used"] == so["rank_used"]
+            assert abs(sg["cg_iters"] - so["cg_iters"]) <= max(3, 0.05 * so["cg_iters"])
+        rel_m = lambda a, b: float(np.sqrt((w.m * (a - b) ** 2).sum() / (w.m * b * b).sum()))
+        assert rel_m(rg["y"], ro["y"]) <= 1e-6 and rel_m(rg["u"], ro["u"]) <= 1e-6
+    finally:
+        g.close()
