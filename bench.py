@@ -322,7 +322,7 @@ def run_ours(args):
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": f"replicas x{world}",
                        "alg1_variant": args.alg1_variant, "reference": args.reference, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
-                       "l2": "flushed between steps (256 MiB write); the deflated working set (W, HW, K, K^T) exceeds L2"},
+                       "l2": "flushed between steps (256 MiB write); the loop's working set (HW, K, K^T, vectors: about 120 MB) is the size of the L2"},
             "e2e": {"value": round(e2e_value, 4), "unit": "s/query", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps},
             "gpu_launches": int(launches),
