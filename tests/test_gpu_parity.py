@@ -363,3 +363,63 @@ def test_operator_change_keeps_the_reference(rd, oracle_mod):
     finally:
         g_nom.close()
         g_off.close()
+
+
+OPTION_SETS = {
+    "all_inactive_start": dict(init=2),
+    "given_start": dict(init=3),
+    "c_is_diag": dict(c_is_diag=1),
+    "scheduled_replacement": dict(replace_period=25),
+    "no_jacobi": dict(jacobi=0),
+    "paper_tolerances": dict(eps=1e-10, eps_c=1e-11),
+}
+
+
+@pytest.mark.parametrize("name", list(OPTION_SETS))
+def test_query_parity_under_options(rd, oracle_mod, name):
+    """Every rd_options field that changes the path (readings A3, A5, A8, A11 of DESIGN.md; PAPER.md:267, :273, :339,
+    :341) against the oracle run with the same option."""
+    kw = OPTION_SETS[name]
+    w = make_config(twin="c2_48")
+    o = oracle_mod.Oracle.from_workload(w)
+    _, W = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap, **kw))
+    try:
+        g.set_reference(W)
+        yd, psi = w.target(0)
+        J0 = None
+        if kw.get("init") == 3:
+            J0 = (np.random.default_rng(11).random(w.N) < 0.4).astype(np.uint8)
+        ro = o.solve_query(1, yd, psi, W, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap, **kw), J0=J0)
+        rg = g.solve_query(1, yd, psi, J0=J0)
+        assert rg["status"] == ro["status"] and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"]), [s["margin"] for s in ro["steps"]]
+        tol = kw.get("eps", 1e-8)
+        for sg, so in zip(rg["steps"], ro["steps"]):
+            assert sg["status"] == so["status"] == 0 and sg["rel_resid_verified"] <= tol
+            assert sg["rank_used"] == so["rank_used"]
+            assert abs(sg["cg_iters"] - so["cg_iters"]) <= max(3, 0.05 * so["cg_iters"])
+            if kw.get("replace_period"):
+                assert sg["replacements"] >= sg["cg_iters"] // kw["replace_period"]
+        assert _rel_m(w, rg["y"], ro["y"]) <= 1e-6 and _rel_m(w, rg["u"], ro["u"]) <= 1e-6
+    finally:
+        g.close()
+
+
+def test_query_parity_with_sigma_one_over_alpha(rd, oracle_mod):
+    """BASELINE.json's literal text H = M + (1/alpha) K^T M^{-1} K (reading A1, sigma_is_alpha = 0): runnable and in
+    parity with the oracle given sigma = 1/alpha."""
+    w = make_config(1)
+    o = oracle_mod.Oracle(w.rowptr, w.colidx, w.val, w.m, 1.0 / w.alpha)
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap, sigma_is_alpha=0.0))
+    try:
+        yd, psi = w.target(0)
+        ro = o.solve_query(0, yd, psi, None, oracle_mod.OracleOptions(pdas_cap=w.pdas_cap))
+        rg = g.solve_query(0, yd, psi)
+        # (from the all-active start PDAS may still be releasing DOFs when it reaches config 1's cap of 20 steps:
+        # the status, whatever it is, and the whole sequence must agree)
+        assert rg["status"] == ro["status"] and rg["n_steps"] == ro["n_steps"]
+        assert np.array_equal(rg["J_bits"], ro["J_bits"])
+        assert _rel_m(w, rg["y"], ro["y"]) <= 1e-6 and _rel_m(w, rg["u"], ro["u"]) <= 1e-6
+    finally:
+        g.close()
