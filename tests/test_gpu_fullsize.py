@@ -1,5 +1,6 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (the default persistent
-kernel, one CTA per SM): configs 2 (512x512, k = 32) and 5 (160^3, k = 64).
+kernel, one CTA per SM): configs 2 (512x512, k = 32), 3 (96^3, k = 48), 4 (256x256 x 32 slabs, k = 64) and 5 (160^3,
+k = 64).
 
 The oracle cannot run a complete solve at these sizes (22 ms and 0.4 s per iteration), so the checks are
   * operator applies element by element (one oracle apply is milliseconds),
@@ -19,7 +20,7 @@ from workloads import make_config
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module", params=[2, 5])
+@pytest.fixture(scope="module", params=[2, 3, 4, 5])
 def big(request, oracle_mod):
     import torch
 
@@ -59,9 +60,9 @@ def test_fullsize_operator(big):
 def test_fullsize_capped_loop_matches_oracle(big, method):
     w, o, g, W, pkg = big
     rng = np.random.default_rng(2)
-    # config 5: 90 % of the DOFs active (an early PDAS step) keeps the oracle's QR of the 64 restricted columns to
+    # configs 3-5: 90 % of the DOFs active (an early PDAS step) keeps the oracle's QR of the 64 restricted columns to
     # seconds; the kernel's launch configuration, tile size and full-length vectors do not depend on |I|
-    frac = 0.1 if w.N < 1_000_000 else 0.9
+    frac = 0.1 if w.N < 500_000 else 0.9
     act = (rng.random(w.N) < frac).astype(np.uint8)
     idx = np.flatnonzero(act == 0)
     yd = w._target(1000 * w.config)
