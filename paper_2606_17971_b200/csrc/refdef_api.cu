@@ -743,7 +743,6 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     std::vector<double> theta(b), res2(b), resid(b, INFINITY);
 
     const int gs = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
-    const dim3 gblk(std::max(1, gs / std::min(nchunk, 4)), nchunk);
     const dim3 ggram(nparts, (b + 63) / 64, (b + 63) / 64);
     const int64_t bb = (int64_t)b * b;
 
@@ -757,9 +756,14 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     if (!(beta > 0.0) || !std::isfinite(beta)) return fail(ctx, RD_ENOTSPD, "spectrum bound %g", beta);
     beta *= 1.0 + 1e-10;
 
-    auto block_apply = [&](const double* Y, double c1, double cshift, double c2, const double* Yprev, double* Ynext) {
-        k_blk_K<<<gblk, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y, T);
-        k_blk_KT<<<gblk, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y, T, Yprev, Ynext);
+    // columns [col0, b) of the block (col0 a multiple of the chunk width): the leading col0 columns are locked
+    auto block_apply = [&](const double* Y, double c1, double cshift, double c2, const double* Yprev, double* Ynext, int col0 = 0) {
+        const int nch = nchunk - col0 / RD_EIG_CB;
+        const dim3 gb(std::max(1, gs / std::min(nch, 4)), nch);
+        const size_t o = (size_t)col0 * ld;
+        k_blk_K<<<gb, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y + o, T + o);
+        k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o,
+                                                   Yprev ? Yprev + o : nullptr, Ynext + o);
         ctx->launches += 2;
     };
     auto gram = [&](const double* A, const double* B, double* out) {
@@ -832,13 +836,22 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
         double* Y0 = P[cur];
         double* Y1 = P[(cur + 1) & 3];
         double* Y2 = P[(cur + 2) & 3];
-        block_apply(Y0, sg / e, c, 0.0, nullptr, Y1);
+        // Locking: the leading Ritz vectors that already pass the residual test (whole chunks of them) skip the filter
+        // and are carried over unchanged; orthonormalisation and Rayleigh-Ritz of the next sweep still see the whole
+        // block, and a locked vector that drifts above the tolerance is simply filtered again.
+        int nlock = 0;
+        while (nlock < k && resid[nlock] <= tol) ++nlock;
+        nlock = std::min((nlock / RD_EIG_CB) * RD_EIG_CB, b - RD_EIG_CB);
+        const double* Xlocked = Y0;
+        block_apply(Y0, sg / e, c, 0.0, nullptr, Y1, nlock);
         for (int j = 2; j <= deg; ++j) {
             const double sn = 1.0 / (tau - sg);
-            block_apply(Y1, 2.0 * sn / e, c, -sg * sn, Y0, Y2);
+            block_apply(Y1, 2.0 * sn / e, c, -sg * sn, Y0, Y2, nlock);
             double* tmp = Y0; Y0 = Y1; Y1 = Y2; Y2 = tmp;
             sg = sn;
         }
+        if (nlock > 0 && Y1 != Xlocked)
+            CU(cudaMemcpyAsync(Y1, Xlocked, (size_t)nlock * ld * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
         CU(cudaGetLastError());
         for (int q = 0; q < 4; ++q) if (P[q] == Y1) cur = q;
     }
