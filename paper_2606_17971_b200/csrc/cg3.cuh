@@ -250,6 +250,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
                 mbar_wait(bar, ph);
                 ph ^= 1u;
                 if (wd <= 5) acc = staged_row_dot<COMBINE, 5>(sval, scol, wd, lane, v0, v1, beta, next);
+                else if (wd <= 7) acc = staged_row_dot<COMBINE, 7>(sval, scol, wd, lane, v0, v1, beta, next);
                 else acc = staged_row_dot<COMBINE, RD_SPMV_WD>(sval, scol, wd, lane, v0, v1, beta, next);
             } else {
                 next();
