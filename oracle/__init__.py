@@ -11,6 +11,8 @@ from .oracle import (  # noqa: F401
     reference_eigs_scaled,
     sine_reference,
     spacetime_reference,
+    prolong_p1,
+    prolonged_reference,
     JACOBI_CG,
     REFDEF,
     ZEROEXT,

@@ -427,3 +427,72 @@ def reference_eigs_scaled(rowptr, colidx, val, m, sigma, k, dense_below: int = 1
         mu, V = mu[order], s[:, None] * Vs[:, order]
     V = V / np.linalg.norm(V, axis=0)
     return mu.copy(), np.asfortranarray(V)
+
+
+def prolong_p1(Vc, dims_c, dims_f):
+    """P1 prolongation of coarse vectors to the fine grid (NEXT-1(ii) of SURVEY.md 8(f)): "P1 prolongation maps these
+    vectors to the full fine mesh" (section 2.2.2), restated for the cell-centred Cartesian grids of
+    workloads/ (reading A19): the continuous d-linear interpolant of the coarse cell-centre values, extended
+    by the homogeneous Dirichlet value 0 on the boundary of the unit box, evaluated at the fine cell centres.
+
+    Per axis with n_c coarse and n_f fine cells the interpolation nodes are xi_0 = 0, xi_j = (j - 1/2)/n_c (j = 1..n_c),
+    xi_{n_c+1} = 1 with nodal values (0, v_1, ..., v_{n_c}, 0); the fine centre x_i = (i - 1/2)/n_f lies in one interval
+    [xi_j, xi_{j+1}] and takes (1 - t) v_j + t v_{j+1}, t = (x_i - xi_j)/(xi_{j+1} - xi_j).  In d dimensions the value at
+    a fine cell is the sum over the 2^d corners of the enclosing box of the product of the per-axis weights times the
+    corner value (x fastest ordering on both grids).  No normalisation here.
+
+    Vc: (N_c, k).  Returns (N_f, k) column-major.  Plain loops: small cases only."""
+    dims_c = [int(n) for n in dims_c]
+    dims_f = [int(n) for n in dims_f]
+    d = len(dims_c)
+    assert d == len(dims_f) and 1 <= d <= 3
+    Vc = np.asarray(Vc, dtype=np.float64)
+    if Vc.ndim == 1:
+        Vc = Vc[:, None]
+    Nc, Nf = int(np.prod(dims_c)), int(np.prod(dims_f))
+    assert Vc.shape[0] == Nc
+    k = Vc.shape[1]
+    # per axis: for each fine index the two node numbers (0 and n_c + 1 are the boundary nodes) and the weight t
+    axis = []
+    for a in range(d):
+        nc, nf = dims_c[a], dims_f[a]
+        xi = np.concatenate(([0.0], (np.arange(1, nc + 1) - 0.5) / nc, [1.0]))
+        ent = []
+        for i in range(1, nf + 1):
+            x = (i - 0.5) / nf
+            j = 0
+            while j + 1 <= nc and xi[j + 1] <= x:  # last node not to the right of x
+                j += 1
+            t = (x - xi[j]) / (xi[j + 1] - xi[j])
+            ent.append((j, t))
+        axis.append(ent)
+    strides_c = [int(np.prod(dims_c[:a])) for a in range(d)]
+    out = np.zeros((Nf, k), order="F")
+    for fi, idx in enumerate(itertools.product(*[range(n) for n in reversed(dims_f)])):
+        idx = idx[::-1]  # (i_x, i_y, i_z) with x fastest in fi
+        acc = np.zeros(k)
+        for corner in itertools.product((0, 1), repeat=d):
+            wgt, cid, inside = 1.0, 0, True
+            for a in range(d):
+                j, t = axis[a][idx[a]]
+                node = j + corner[a]
+                wgt *= t if corner[a] else (1.0 - t)
+                if node == 0 or node == dims_c[a] + 1:
+                    inside = False  # boundary node: value 0
+                else:
+                    cid += (node - 1) * strides_c[a]
+            if inside:
+                acc += wgt * Vc[cid]
+        out[fi] = acc
+    return out
+
+
+def prolonged_reference(coarse, dims_c, dims_f, k):
+    """The paper's coarse-mesh reference: the k lowest pairs of the coarse generalized problem
+    H_c phi = mu D_c phi (`reference_eigs_scaled` on the coarse operator `coarse` = (rowptr, colidx, val, m, sigma)),
+    P1-prolonged to the fine grid, "each column is normalized in the Euclidean norm".
+    Returns (mu, Wc, W): Wc the coarse vectors (unit columns), W (N_f, k) column-major with unit columns."""
+    mu, Wc = reference_eigs_scaled(*coarse, k)
+    W = prolong_p1(Wc, dims_c, dims_f)
+    W = np.asfortranarray(W / np.linalg.norm(W, axis=0))
+    return mu, Wc, W

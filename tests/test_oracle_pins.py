@@ -599,3 +599,93 @@ def test_scaled_reference_solves_the_generalized_problem(oracle_mod):
     _, r_sc = o.alg1(idx, b, np.zeros(w.N), W)
     assert r_std["status"] == r_sc["status"] == 0
     assert r_sc["iters"] <= 1.02 * r_std["iters"], (r_sc["iters"], r_std["iters"])
+
+
+# ------------------------------------------------------------------ NEXT-1(ii): coarse eigenproblem + P1 prolongation
+def _interp_axiswise(Vc, dims_c, dims_f):
+    """Library pin: numpy.interp along one axis after the other (nodes = boundary 0, coarse centres, boundary 1)."""
+    T = np.asarray(Vc, dtype=float).reshape(tuple(reversed(dims_c)))  # C order: slowest axis first, x last
+    d = len(dims_c)
+    for a in range(d):
+        ax = d - 1 - a  # position of grid axis a in the array
+        nc, nf = dims_c[a], dims_f[a]
+        xi = np.concatenate(([0.0], (np.arange(nc) + 0.5) / nc, [1.0]))
+        xf = (np.arange(nf) + 0.5) / nf
+        T = np.apply_along_axis(lambda v: np.interp(xf, xi, np.concatenate(([0.0], v, [0.0]))), ax, T)
+    return T.reshape(-1)
+
+
+@pytest.mark.parametrize("dims_c,dims_f", [((5,), (10,)), ((4,), (12,)), ((4,), (7,)), ((3, 5), (6, 15)),
+                                            ((2, 3, 4), (4, 9, 8)), ((6, 4), (6, 4))])
+def test_prolong_p1_matches_library_interpolation(oracle_mod, dims_c, dims_f):
+    """Non-square grids with different ratios per axis: a transposed axis or a wrong stride fails."""
+    rng = np.random.default_rng(17)
+    Vc = rng.standard_normal((int(np.prod(dims_c)), 3))
+    P = oracle_mod.prolong_p1(Vc, dims_c, dims_f)
+    assert P.shape == (int(np.prod(dims_f)), 3)
+    for c in range(3):
+        assert np.allclose(P[:, c], _interp_axiswise(Vc[:, c], dims_c, dims_f), rtol=0, atol=1e-14)
+    if tuple(dims_c) == tuple(dims_f):  # same grid: the identity
+        assert np.array_equal(P, Vc)
+
+
+def test_prolong_p1_closed_forms(oracle_mod):
+    """(a) A function that is d-linear between the coarse nodes and 0 on the boundary is reproduced exactly: the
+    product of 1-D hats h(s) = 1 - |2s - 1|, whose kink 1/2 is a coarse node for odd n_c.  (b) Dependence on x only
+    stays on x only (axis order).  (c) Interpolating the coarse sine mode stays within the P1 error bound
+    h_c^2 max|f''|/8 of the continuous mode, and a refinement ratio 2 puts the weights at 1/4, 3/4."""
+    hat = lambda s: 1.0 - np.abs(2.0 * s - 1.0)
+    nc, nf = (5, 7), (20, 21)
+    xc = [(np.arange(n) + 0.5) / n for n in nc]
+    xf = [(np.arange(n) + 0.5) / n for n in nf]
+    Vc = np.kron(hat(xc[1]), hat(xc[0]))  # x fastest
+    P = oracle_mod.prolong_p1(Vc, nc, nf)[:, 0]
+    assert np.allclose(P, np.kron(hat(xf[1]), hat(xf[0])), rtol=0, atol=1e-15)
+    Vx = np.kron(np.ones(nc[1]), hat(xc[0]))
+    Px = oracle_mod.prolong_p1(Vx, nc, nf)[:, 0].reshape(nf[1], nf[0])
+    # rows strictly between the first and last coarse centres in y see the constant 1 in y
+    inner = (xf[1] >= xc[1][0]) & (xf[1] <= xc[1][-1])
+    assert np.allclose(Px[inner], hat(xf[0])[None, :], rtol=0, atol=1e-15)
+    q, n = 3, 16
+    f = lambda s: np.sin(np.pi * q * s)
+    P1 = oracle_mod.prolong_p1(f((np.arange(n) + 0.5) / n), (n,), (2 * n,))[:, 0]
+    s_f = (np.arange(2 * n) + 0.5) / (2 * n)
+    assert np.abs(P1 - f(s_f)).max() <= (1.0 / n) ** 2 * (np.pi * q) ** 2 / 8 + 1e-15
+    v = np.arange(1.0, n + 1)
+    P2 = oracle_mod.prolong_p1(v, (n,), (2 * n,))[:, 0]
+    assert np.allclose(P2[1:-1:2], 0.75 * v[:-1] + 0.25 * v[1:], rtol=0, atol=1e-14)   # fine cell 2j: 3/4, 1/4
+    assert np.allclose(P2[2:-1:2], 0.25 * v[:-1] + 0.75 * v[1:], rtol=0, atol=1e-14)
+    assert abs(P2[0] - 0.5 * v[0]) <= 1e-15 and abs(P2[-1] - 0.5 * v[-1]) <= 1e-15     # half-way to the Dirichlet 0
+
+
+def test_prolonged_reference_deflates_the_fine_problem(oracle_mod):
+    """Coarse generalized eigenproblem (24^2) -> P1 prolongation -> unit columns on the 48^2 twin of
+    config 2: "The prolonged candidates are approximate fine-mesh modes": small Rayleigh quotients in
+    the Jacobi-scaled fine operator, fewer iterations than Jacobi-CG, same solution."""
+    w = make_config(twin="c2_48")
+    wc = make_config(config=2, n=24, k=w.k)
+    o = oracle_mod.Oracle.from_workload(w)
+    mu_c, Wc, W = oracle_mod.prolonged_reference((wc.rowptr, wc.colidx, wc.val, wc.m, wc.alpha), wc.dims, w.dims, w.k)
+    assert W.shape == (w.N, w.k) and np.allclose(np.linalg.norm(W, axis=0), 1.0, atol=1e-13)
+    assert np.allclose(np.linalg.norm(Wc, axis=0), 1.0, atol=1e-13)
+    d = o.diag_H()
+    mu_f, _ = oracle_mod.reference_eigs_scaled(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    # Rayleigh quotient of the lowest prolonged vector in the fine generalized problem: above the fine mu_1 (min-max),
+    # and an approximation of it
+    rq = lambda v: float(v @ o.apply_H(v)) / float(v @ (d * v))
+    assert mu_f[0] * (1 - 1e-10) <= rq(W[:, 0]) <= 1.5 * mu_f[0]
+    # every prolonged column stays in the low end of the fine Jacobi-scaled spectrum (which reaches up to about 2)
+    assert max(rq(W[:, c]) for c in range(w.k)) <= 10.0 * mu_f[-1] < 0.01
+    # the coarse generalized eigenvalues are the fine ones times about (h_c/h_f)^4 = 16 (H is M + sigma * fourth order)
+    assert 8.0 <= (mu_c / mu_f).min() and (mu_c / mu_f).max() <= 17.0
+    idx = np.arange(w.N)
+    b = w.m * w._target(1000 * w.config)
+    xj, rj = o.alg1(idx, b, np.zeros(w.N), None)
+    xp, rp = o.alg1(idx, b, np.zeros(w.N), W)
+    assert rj["status"] == rp["status"] == 0 and rp["rank_used"] == w.k
+    assert rp["iters"] < 0.6 * rj["iters"], (rp["iters"], rj["iters"])
+    assert np.linalg.norm(xp - xj) <= 1e-5 * np.linalg.norm(xj)
+    # nearly as good as the exact fine modes of the same generalized problem
+    _, W_f = oracle_mod.reference_eigs_scaled(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    _, rf = o.alg1(idx, b, np.zeros(w.N), W_f)
+    assert rf["iters"] <= rp["iters"] <= 1.25 * rf["iters"], (rp["iters"], rf["iters"])
