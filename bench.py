@@ -158,6 +158,35 @@ def build_analytical_reference(g, w):
         g.build_reference_sine(w.k, w.dims)
 
 
+_COARSE = {}
+
+
+def build_coarse_reference(g, w, ref_tol, coarsen=2):
+    """The paper's coarse-mesh reference (section 2.2.2): Jacobi-scaled low modes of the operator on a grid
+    with 1/coarsen of the cells per axis (a second context, rd_build_reference_scaled), P1 prolongation and column
+    normalisation on the fine grid (rd_build_reference_prolonged).  The coarse operator is an input like the fine one
+    (assembled once on the host, cached); the coarse eigensolve and the prolongation are timed.  Returns (status of
+    the coarse eigensolve, its milliseconds)."""
+    import paper_2606_17971_b200 as pkg
+    from workloads import make_config
+
+    if w.nt > 1:
+        raise SystemExit("bench.py: --reference coarse covers the steady configs (config 4: --reference sine)")
+    key = (w.config, tuple(w.dims), w.k, coarsen)
+    if key not in _COARSE:
+        _COARSE[key] = make_config(w.config, n=max(2, w.dims[0] // coarsen), k=w.k)
+    wc = _COARSE[key]
+    gc = pkg.RefDef.from_workload(wc)
+    try:
+        _, _, _, st = gc.build_reference_scaled(w.k, tol=ref_tol, max_block_iters=60)
+        ms_c = gc.reference_info()["build_ms"]
+        Wc = gc.get_reference()
+    finally:
+        gc.close()
+    g.build_reference_prolonged(Wc, wc.dims, w.dims)
+    return st, ms_c
+
+
 def load_profile():
     p = os.path.join(ROOT, "profiles", "bench_workload_profile.json")
     if os.path.exists(p):
@@ -184,16 +213,19 @@ class Sequence:
     def begin_pass(self):
         self.g.reset_sequence()
         if self.method != 0:
+            extra_ms = 0.0
             if self.reference == "sine":  # analytical references of the paper: PAPER.md:186-192 (steady), :194-208 (transient)
                 build_analytical_reference(self.g, self.w)
                 st = 0
+            elif self.reference == "coarse":  # coarse generalized eigenproblem + P1 prolongation
+                st, extra_ms = build_coarse_reference(self.g, self.w, self.ref_tol)
             elif self.reference == "eig-scaled":  # Jacobi-scaled generalized problem
                 _, _, _, st = self.g.build_reference_scaled(self.w.k, tol=self.ref_tol, max_block_iters=60)
             else:
                 _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
             info = self.g.reference_info()
             self.ref_builds += 1
-            self.ref_ms += info["build_ms"]
+            self.ref_ms += info["build_ms"] + extra_ms
             self.ref_status = st
 
     def next_inputs(self):
@@ -371,6 +403,9 @@ def run_loop(args):
         if args.reference == "sine":
             build_analytical_reference(g, w)
             ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
+        elif args.reference == "coarse":
+            st, ms_c = build_coarse_reference(g, w, args.ref_tol)
+            ref = dict(g.reference_info(), kind="coarse eigenproblem + P1 prolongation (PAPER.md:176)", status=st, coarse_eig_ms=ms_c)
         else:
             build = g.build_reference_scaled if args.reference == "eig-scaled" else g.build_reference
             _, resid, sweeps, st = build(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
@@ -435,6 +470,8 @@ def run_replay(args):
     g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant))
     if args.reference == "sine":
         build_analytical_reference(g, w)
+    elif args.reference == "coarse":
+        build_coarse_reference(g, w, args.ref_tol)
     elif args.reference == "eig-scaled":
         g.build_reference_scaled(w.k, tol=args.ref_tol, max_block_iters=60)
     else:
@@ -577,9 +614,10 @@ def main(argv=None):
     ap.add_argument("--twin", default=None)
     ap.add_argument("--method", default="refdef", choices=list(METHODS))
     ap.add_argument("--ref-tol", type=float, default=1e-3)
-    ap.add_argument("--reference", default="eig", choices=["eig", "eig-scaled", "sine"],
+    ap.add_argument("--reference", default="eig", choices=["eig", "eig-scaled", "sine", "coarse"],
                     help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
-                         "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4)")
+                         "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4); "
+                         "coarse: Jacobi-scaled modes of the half-resolution operator, P1-prolonged (PAPER.md:176)")
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -174,6 +174,18 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
  * int32 (q_1..q_d of the spatial mode, then j), may be NULL.  Build time charged to the next query. */
 int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt,
                                  double* s_out, int32_t* pairs_out);
+/* The paper's coarse-mesh reference (section 2.2.2): "P1 prolongation maps these vectors to the full
+ * fine mesh, where each column is normalized in the Euclidean norm."  Wc: N_c x k column-major (ld N_c), host or
+ * device: vectors on a coarser Cartesian grid of dims_c cells of the same unit box, typically the Jacobi-scaled low
+ * modes of the coarse operator (rd_build_reference_scaled on a context created from the coarse K, then
+ * rd_get_reference).  dims_f: the fine grid (ndim <= 3, x = dims[0] fastest on both grids, product of dims_f = N else
+ * RD_EINVAL; any ratio dims_f[a]/dims_c[a], also non-integer).  P1 on the cell-centred grids used here = the d-linear
+ * interpolant of the coarse cell-centre values, extended by the Dirichlet value 0 on the boundary, evaluated at the
+ * fine cell centres (reading A20).  norms_out: host, k doubles, the Euclidean norms of the prolonged columns
+ * before the normalisation, may be NULL; a zero or non-finite column is RD_EINVAL and leaves no reference.
+ * The time of this call is charged to the next query (the coarse eigensolve ran elsewhere: the caller adds it). */
+int rd_build_reference_prolonged(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims_c, const int64_t* dims_f,
+                                 const double* Wc, double* norms_out);
 /* Inject a reference (e.g. the oracle's): W is N x k column-major with leading dimension N. */
 int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W);
 /* Copy the stored reference out: W_out N x k column-major (ld N); returns k via k_out (0 if none). */

@@ -432,7 +432,7 @@ def reference_eigs_scaled(rowptr, colidx, val, m, sigma, k, dense_below: int = 1
 def prolong_p1(Vc, dims_c, dims_f):
     """P1 prolongation of coarse vectors to the fine grid (NEXT-1(ii) of SURVEY.md 8(f)): "P1 prolongation maps these
     vectors to the full fine mesh" (section 2.2.2), restated for the cell-centred Cartesian grids of
-    workloads/ (reading A19): the continuous d-linear interpolant of the coarse cell-centre values, extended
+    workloads/ (reading A20): the continuous d-linear interpolant of the coarse cell-centre values, extended
     by the homogeneous Dirichlet value 0 on the boundary of the unit box, evaluated at the fine cell centres.
 
     Per axis with n_c coarse and n_f fine cells the interpolation nodes are xi_0 = 0, xi_j = (j - 1/2)/n_c (j = 1..n_c),

@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
 
 
@@ -102,6 +102,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_build_reference_scaled.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
+    lib.rd_build_reference_prolonged.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
     lib.rd_set_reference.argtypes = [vp, i32, vp]
     lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
@@ -244,6 +245,26 @@ class RefDef:
                                                            pairs.ctypes.data), "rd_build_reference_spacetime")
         self.k = k
         return s, pairs
+
+    def build_reference_prolonged(self, Wc, dims_c, dims_f):
+        """Coarse-mesh reference: P1 prolongation of Wc (N_c x k numpy, or a column-major device tensor of
+        shape (k, N_c)) from the grid dims_c to the grid dims_f, unit columns.  Returns the norms before normalisation."""
+        dims_c = np.ascontiguousarray(dims_c, dtype=np.int64)
+        dims_f = np.ascontiguousarray(dims_f, dtype=np.int64)
+        if len(dims_c) != len(dims_f):
+            raise ValueError("dims_c and dims_f differ in length")
+        if isinstance(Wc, np.ndarray):
+            Wc = np.asfortranarray(Wc, dtype=np.float64)
+            nc, k = Wc.shape
+        else:
+            k, nc = Wc.shape
+        if nc != int(np.prod(dims_c)):
+            raise ValueError("Wc does not have prod(dims_c) rows")
+        norms = np.zeros(k)
+        self._check(self._lib.rd_build_reference_prolonged(self._h, k, len(dims_c), dims_c.ctypes.data, dims_f.ctypes.data,
+                                                           _ptr(Wc), norms.ctypes.data), "rd_build_reference_prolonged")
+        self.k = k
+        return norms
 
     def reference_info(self):
         b, deg, ms = C.c_int32(0), C.c_int64(0), C.c_double(0)

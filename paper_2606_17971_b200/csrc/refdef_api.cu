@@ -18,6 +18,7 @@
 #include "cg2.cuh"
 #include "cg3.cuh"
 #include "sine.cuh"
+#include "prolong.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
 #include "pdas.cuh"
@@ -673,6 +674,59 @@ int rd_diag_H(rd_ctx* ctx, double* d_out)
     if (!ctx || !d_out) return RD_EINVAL;
     RDTRY(out_host(ctx, d_out, ctx->d, ctx->N));
     CU(cudaStreamSynchronize(ctx->stream));
+    return RD_OK;
+}
+
+int rd_build_reference_prolonged(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims_c, const int64_t* dims_f,
+                                 const double* Wc, double* norms_out)
+{
+    if (!ctx || !dims_c || !dims_f || !Wc || k < 1 || k > RD_MAX_K || ndim < 1 || ndim > 3) return RD_EINVAL;
+    int64_t Nc = 1, Nf = 1;
+    for (int a = 0; a < ndim; ++a) {
+        if (dims_c[a] < 1 || dims_c[a] > (1 << 20)) return fail(ctx, RD_EINVAL, "dims_c[%d] = %lld", a, (long long)dims_c[a]);
+        if (dims_f[a] < 1 || dims_f[a] > (1 << 20)) return fail(ctx, RD_EINVAL, "dims_f[%d] = %lld", a, (long long)dims_f[a]);
+        Nc *= dims_c[a];
+        Nf *= dims_f[a];
+    }
+    if (Nf != ctx->N) return fail(ctx, RD_EINVAL, "product of dims_f %lld is not N = %lld (steady Cartesian grids only)", (long long)Nf, (long long)ctx->N);
+    const auto t_begin = std::chrono::steady_clock::now();
+    RDTRY(alloc_reference(ctx, k));
+    const int kp = ctx->kp, nparts = ctx->num_sms;
+    // scratch of this call: a device copy of the coarse block (Wc may be a host pointer), partial sums, norms
+    double *d_Wc = nullptr, *d_parts = nullptr, *d_norms = nullptr;
+    std::vector<double> norms(k, 0.0);
+    cudaError_t e = cudaMalloc(&d_Wc, (size_t)Nc * k * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_parts, (size_t)nparts * k * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&d_norms, (size_t)k * sizeof(double));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(d_Wc), cudaFree(d_parts), cudaFree(d_norms);
+        return fail(ctx, RD_ENOMEM, "cudaMalloc of the coarse block (%lld x %d)", (long long)Nc, k);
+    }
+    e = cudaMemcpyAsync(d_Wc, Wc, (size_t)Nc * k * sizeof(double), cudaMemcpyDefault, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->W, 0, (size_t)ctx->ldw * kp * sizeof(double), ctx->stream);  // pad rows stay zero
+    const int c0 = (int)dims_c[0], c1 = ndim > 1 ? (int)dims_c[1] : 1, c2 = ndim > 2 ? (int)dims_c[2] : 1;
+    const int f0 = (int)dims_f[0], f1 = ndim > 1 ? (int)dims_f[1] : 1, f2 = ndim > 2 ? (int)dims_f[2] : 1;
+    const int g = grid_for(ctx->N, kThreads, big_grid(ctx));
+    k_prolong_p1<<<g, kThreads, 0, ctx->stream>>>(ctx->N, ctx->ldw, ndim, c0, c1, c2, f0, f1, f2, k, kp, d_Wc, Nc, ctx->W);
+    k_col_sumsq_parts<<<dim3(nparts, k), kThreads, 0, ctx->stream>>>(ctx->N, ctx->ldw, ctx->W, d_parts);
+    k_col_normalise<<<dim3(std::max(1, g / 8), k), kThreads, 0, ctx->stream>>>(ctx->N, ctx->ldw, nparts, d_parts, ctx->W, d_norms);
+    ctx->launches += 3;
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(norms.data(), d_norms, (size_t)k * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_Wc), cudaFree(d_parts), cudaFree(d_norms);
+    if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "prolonged reference: %s", cudaGetErrorString(e));
+    if (norms_out) for (int c = 0; c < k; ++c) norms_out[c] = norms[c];
+    for (int c = 0; c < k; ++c)
+        if (!(norms[c] > 0.0) || !std::isfinite(norms[c])) {
+            ctx->k = 0;  // no usable reference
+            return fail(ctx, RD_EINVAL, "column %d of the prolonged reference has norm %g", c, norms[c]);
+        }
+    ctx->ref_degree = 0;
+    ctx->ref_block = k;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
     return RD_OK;
 }
 
