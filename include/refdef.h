@@ -224,6 +224,18 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
 int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C,
                     int32_t* rank_used, double* cond_E, int32_t* fallback);
 
+/* Energy fraction removed by the coarse correction, eq. (24): for an independent solution
+ * x_* of B x = b (B = H_II on the inactive set of `active`) and a zero initial guess,
+ *     chi = ||Q b||_B^2 / ||x_*||_B^2,   ||v||_B^2 = v^T B v,   Q = Z E^{-1} Z^T (Algorithm 1 line 2)
+ * with the basis of `method` on this active set (S1 + S2 are run; rank zero and RD_JACOBI_CG give chi = 0;
+ * the zero-extension history is read, not advanced).  Computed as c^T C c with c = W_I^T b and C of
+ * rd_coarse_setup (Q = W_I C W_I^T and C E_W C = C), and x_*^T (B x_*) from one masked operator apply.
+ * active: N bytes; b, x_star: N doubles in full-domain indexing (entries on J ignored), host or device.
+ * chi, qb_energy (= ||Qb||_B^2), xs_energy (= ||x_*||_B^2): host doubles out; the last two may be NULL.
+ * The complementary fraction ||x_* - Qb||_B^2 / ||x_*||_B^2 equals 1 - chi when x_* solves the system. */
+int rd_energy_fraction(rd_ctx* ctx, int32_t method, const uint8_t* active, const double* b, const double* x_star,
+                       double* chi, double* qb_energy, double* xs_energy);
+
 #ifdef __cplusplus
 }
 #endif

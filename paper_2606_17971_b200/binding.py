@@ -23,7 +23,7 @@ SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
            "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
-           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup"]
+           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction"]
 
 
 class RefDefError(RuntimeError):
@@ -114,6 +114,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_diag_H.argtypes = [vp, vp]
     lib.rd_solve_inactive.argtypes = [vp, i32, vp, vp, vp, C.POINTER(_SolveReport)]
     lib.rd_coarse_setup.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl), C.POINTER(i32)]
+    lib.rd_energy_fraction.argtypes = [vp, i32, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
     _lib = lib
     return lib
 
@@ -330,6 +331,13 @@ class RefDef:
         self._check(self._lib.rd_coarse_setup(self._h, method, _ptr(active), G.ctypes.data, EW.ctypes.data,
                                               Cm.ctypes.data, C.byref(rank), C.byref(cond), C.byref(fb)), "rd_coarse_setup")
         return dict(G=G, EW=EW, C=Cm, rank=rank.value, cond_E=cond.value, fallback=fb.value)
+
+    def energy_fraction(self, method, active, b, x_star):
+        """eq. (24): chi = ||Qb||_B^2 / ||x_*||_B^2 on the inactive system of `active`.  Returns (chi, ||Qb||_B^2, ||x_*||_B^2)."""
+        chi, qb, xs = C.c_double(0), C.c_double(0), C.c_double(0)
+        self._check(self._lib.rd_energy_fraction(self._h, method, _ptr(active), _ptr(b), _ptr(x_star), C.byref(chi),
+                                                 C.byref(qb), C.byref(xs)), "rd_energy_fraction")
+        return chi.value, qb.value, xs.value
 
     # ---- the query
     def solve_query(self, method, y_d, psi, J0=None, y=None, u=None, lam=None, want_sets=True):

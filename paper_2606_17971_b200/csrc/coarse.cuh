@@ -250,4 +250,43 @@ __global__ void __launch_bounds__(1024) k_coarse_small(int kp, const double* G, 
     if (threadIdx.x == 0) { info->rank = r; info->fallback = 0; info->cond_E = cond; }
 }
 
+// ---------------------------------------------------------------- eq. (24): energy fraction of the coarse correction
+// parts[blockIdx.x * (kp + 1) + j] = sum over this block's rows of Wm[i, j] * b[i]  (j < kp: c = W_I^T b) and, at
+// j = kp, of x[i] * Hx[i]  (||x_*||_B^2; x and Hx are zero on J).  Wm column-major with leading dimension ldw:
+// each column is a contiguous stream, rows split evenly over the blocks, fixed summation order.
+__global__ void __launch_bounds__(256) k_energy_parts(int64_t N, int64_t ldw, int kp, const double* Wm, const double* b,
+                                                      const double* x, const double* Hx, double* parts)
+{
+    __shared__ double scratch[32];
+    const int64_t chunk = (N + gridDim.x - 1) / gridDim.x;
+    const int64_t i0 = (int64_t)blockIdx.x * chunk, i1 = (i0 + chunk < N) ? i0 + chunk : N;
+    for (int j = 0; j <= kp; ++j) {
+        const double* u = (j < kp) ? Wm + (size_t)j * ldw : x;
+        const double* v = (j < kp) ? b : Hx;
+        double a = 0.0;
+        for (int64_t i = i0 + threadIdx.x; i < i1; i += blockDim.x) a = fma(ldg_f64(u + i), ldg_f64(v + i), a);
+        a = block_sum(a, scratch);
+        if (threadIdx.x == 0) parts[(size_t)blockIdx.x * (kp + 1) + j] = a;
+    }
+}
+
+// One CTA: out[0] = c^T C c = ||Qb||_B^2 (Q = W_I C W_I^T, C E_W C = C), out[1] = ||x_*||_B^2, out[2] = chi = out[0] / out[1].
+// v = the reduced vector of k_energy_parts (kp + 1 entries); use_coarse = 0 for rank zero (Q = 0).
+__global__ void __launch_bounds__(64) k_energy_fraction(int kp, int use_coarse, const double* C, const double* v, double* out)
+{
+    __shared__ double scratch[32];
+    double a = 0.0;
+    if (use_coarse && (int)threadIdx.x < kp) {
+        double s = 0.0;
+        for (int l = 0; l < kp; ++l) s = fma(C[(size_t)l * kp + threadIdx.x], v[l], s);
+        a = v[threadIdx.x] * s;
+    }
+    a = block_sum(a, scratch);
+    if (threadIdx.x == 0) {
+        out[0] = a;
+        out[1] = v[kp];
+        out[2] = v[kp] > 0.0 ? a / v[kp] : 0.0;
+    }
+}
+
 }  // namespace rd

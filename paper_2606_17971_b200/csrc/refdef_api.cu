@@ -1172,6 +1172,51 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
     return rep->status;
 }
 
+int rd_energy_fraction(rd_ctx* ctx, int32_t method, const uint8_t* active, const double* b, const double* x_star, double* chi,
+                       double* qb_energy, double* xs_energy)
+{
+    if (!ctx || !active || !b || !x_star || !chi) return RD_EINVAL;
+    if (method < RD_JACOBI_CG || method > RD_ZEROEXT) return RD_EINVAL;
+    const int64_t N = ctx->N;
+    int use_coarse = 0;
+    if (method != RD_JACOBI_CG && (!ctx->W || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
+    const uint8_t* da;
+    const double *db, *dx;
+    RDTRY(in_dev(ctx, active, N, ctx->act_stage, &da));
+    RDTRY(in_dev(ctx, b, N, ctx->in0, &db));
+    RDTRY(in_dev(ctx, x_star, N, ctx->in1, &dx));
+    CU(cudaMemcpyAsync(ctx->act, da, N, cudaMemcpyDeviceToDevice, ctx->stream));
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    k_mask_copy<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, db, ctx->b);
+    k_mask_copy<<<g, kThreads, 0, ctx->stream>>>(N, ctx->act, dx, ctx->x);
+    ctx->launches += 2;
+    if (method != RD_JACOBI_CG) {
+        RDTRY(coarse_setup(ctx, method, nullptr, nullptr));  // the history of RD_ZEROEXT is read, not advanced
+        use_coarse = ctx->h_cinfo->rank > 0;
+    }
+    RDTRY(launch_apply_H(ctx, ctx->x, ctx->act, ctx->w));  // w = B x_* on I, 0 on J
+    const int kp = use_coarse ? ctx->kp : 0;
+    const int nparts = ctx->gram_parts ? ctx->gram_nparts : 0;
+    double *parts = ctx->gram_parts, *red = ctx->cwork;
+    if (!nparts) {  // no reference was ever allocated (Jacobi-CG only): the CG reduction slots serve
+        parts = ctx->partial;
+        red = ctx->partial + ctx->cg_grid;
+    }
+    const int np = nparts ? nparts : ctx->cg_grid;
+    k_energy_parts<<<np, 256, 0, ctx->stream>>>(N, ctx->ldw, kp, ctx->Wm, ctx->b, ctx->x, ctx->w, parts);
+    k_reduce_parts<<<1, 128, 0, ctx->stream>>>(np, kp + 1, parts, red);
+    k_energy_fraction<<<1, 64, 0, ctx->stream>>>(kp, use_coarse, ctx->C, red, red + kp + 1);
+    ctx->launches += 3;
+    CU(cudaGetLastError());
+    double h[3];
+    CU(cudaMemcpyAsync(h, red + kp + 1, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (qb_energy) *qb_energy = h[0];
+    if (xs_energy) *xs_energy = h[1];
+    *chi = h[2];
+    return RD_OK;
+}
+
 int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double* psi, const uint8_t* J0, double* y, double* u,
                    double* lambda, rd_step_report* steps, uint8_t* J_bits, rd_query_report* rep)
 {

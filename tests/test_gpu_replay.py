@@ -24,3 +24,8 @@ def test_matched_replay_direct_restriction_beats_zero_extension():
     assert m["refdef"]["cg_iters"] <= m["zeroext"]["cg_iters"] <= 1.02 * m["jacobi"]["cg_iters"]
     assert m["refdef"]["mean_rank"] >= m["zeroext"]["mean_rank"]
     assert out["iteration_ratio_zeroext_over_direct"] >= 1.0
+    # eq. (24): a fraction; zero for rank zero; direct restriction keeps the larger coarse space here
+    assert m["jacobi"]["mean_chi"] == 0.0
+    assert 0.0 < m["zeroext"]["min_chi"] <= m["zeroext"]["mean_chi"] < 1.0
+    assert 0.0 < m["refdef"]["min_chi"] <= m["refdef"]["mean_chi"] < 1.0
+    assert m["refdef"]["mean_chi"] >= m["zeroext"]["mean_chi"]
