@@ -13,6 +13,7 @@ from .oracle import (  # noqa: F401
     spacetime_reference,
     prolong_p1,
     prolonged_reference,
+    transient_reference,
     JACOBI_CG,
     REFDEF,
     ZEROEXT,

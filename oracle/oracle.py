@@ -496,3 +496,54 @@ def prolonged_reference(coarse, dims_c, dims_f, k):
     W = prolong_p1(Wc, dims_c, dims_f)
     W = np.asfortranarray(W / np.linalg.norm(W, axis=0))
     return mu, Wc, W
+
+
+def transient_reference(Phi, st, nt, k):
+    """Transient variant of the coarse-mesh reference, eq. (14) (section 2.2.2): every spatial
+    vector phi_i (column of Phi, N_s x r_s: "each prolonged vector") defines the small temporal matrices
+        H_i = (I (x) phi_i)^T H (I (x) phi_i),   D_i = (I (x) phi_i)^T diag(H) (I (x) phi_i),   H_i q = nu D_i q,
+    with H the all-at-once reduced Hessian `st` = (rowptr, colidx, val, m, sigma) of N_s nt DOFs in the layout
+    id = space + N_s * t (so I (x) phi_i has the nt columns e_t (x) phi_i).  "The construction selects the requested
+    total rank from these spatial-temporal candidates" (:182): reading A21 of DESIGN.md -- all r_s nt pairs ordered
+    by (nu, i, j), j the index of nu within its own problem ascending; column = kron(q, phi_i) with the sign of
+    `temporal_sign`, normalised in the Euclidean norm like the steady columns (:176).
+
+    Written as the definition: H assembled by the library's sparse products, the Kronecker factor formed explicitly,
+    a library generalized symmetric eigensolver per i.  Returns (pairs, nu, W): pairs int (k, 2) = (i, j), nu (k,),
+    W (N_s nt, k) column-major with unit columns."""
+    import scipy.linalg as sla
+    import scipy.sparse as sp
+
+    rowptr, colidx, val, m, sigma = st
+    N = len(m)
+    Phi = np.asarray(Phi, dtype=np.float64)
+    Ns, rs = Phi.shape
+    if Ns * nt != N:
+        raise ValueError("Phi has %d rows, the operator %d = N_s * %d DOFs expected" % (Ns, N, nt))
+    if k > rs * nt:
+        raise ValueError("rank %d exceeds the %d candidates" % (k, rs * nt))
+    K = sp.csr_matrix((val, colidx, rowptr), shape=(N, N))
+    H = (sp.diags(m) + sigma * (K.T @ sp.diags(1.0 / np.asarray(m)) @ K)).tocsr()
+    d = H.diagonal()
+    cand = []
+    Q = []
+    for i in range(rs):
+        V = np.kron(np.eye(nt), Phi[:, i:i + 1])          # I (x) phi_i : (N_s nt) x nt
+        Hi = V.T @ (H @ V)
+        Hi = 0.5 * (Hi + Hi.T)
+        Di = V.T @ (d[:, None] * V)
+        nu, Qi = sla.eigh(Hi, Di)
+        Q.append(Qi)
+        for j in range(nt):
+            cand.append((nu[j], i, j))
+    cand.sort()
+    cand = cand[:k]
+    pairs = np.zeros((k, 2), dtype=np.int32)
+    nus = np.zeros(k)
+    W = np.empty((N, k), order="F")
+    for c, (nu, i, j) in enumerate(cand):
+        pairs[c] = (i, j)
+        nus[c] = nu
+        col = np.kron(temporal_sign(Q[i][:, j]), Phi[:, i])
+        W[:, c] = col / np.linalg.norm(col)
+    return pairs, nus, W
