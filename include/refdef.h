@@ -224,6 +224,18 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
 int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C,
                     int32_t* rank_used, double* cond_E, int32_t* fallback);
 
+/* Transient variant of the coarse-mesh reference, eq. (14) (section 2.2.2; reading A21).
+ * The context holds the all-at-once operator of N = N_s * nt DOFs in the layout id = space + N_s * t.  Phi: N_s x rs
+ * spatial vectors, column-major, host or device (e.g. prolonged coarse vectors, or the reference of a steady
+ * context read with rd_get_reference), none zero.  For every column phi_i the nt x nt matrices
+ *     H_i = (I (x) phi_i)^T H (I (x) phi_i),   D_i = (I (x) phi_i)^T diag(H) (I (x) phi_i),   H_i q = nu D_i q
+ * are formed (nt operator applies per vector) and solved on the device; the k lowest of the rs * nt candidates in
+ * the order (nu, i, j) become the reference: column = q (x) phi_i, the component of q of largest magnitude
+ * positive, unit Euclidean norm.  nu_out: k host doubles or NULL; pairs_out: 2k host int32 (i, j) or NULL.
+ * RD_EINVAL: k > rs * nt, k or rs > 64, nt > the dense limit, N not a multiple of nt; RD_ENOTSPD: a zero vector. */
+int rd_build_reference_transient(rd_ctx* ctx, int32_t k, int32_t rs, int32_t nt, const double* Phi, double* nu_out,
+                                 int32_t* pairs_out);
+
 /* Energy fraction removed by the coarse correction, eq. (24): for an independent solution
  * x_* of B x = b (B = H_II on the inactive set of `active`) and a zero initial guess,
  *     chi = ||Q b||_B^2 / ||x_*||_B^2,   ||v||_B^2 = v^T B v,   Q = Z E^{-1} Z^T (Algorithm 1 line 2)

@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction"]
 
 
@@ -103,6 +103,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
     lib.rd_build_reference_prolonged.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    lib.rd_build_reference_transient.argtypes = [vp, i32, i32, i32, vp, vp, vp]
     lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
     lib.rd_set_reference.argtypes = [vp, i32, vp]
     lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
@@ -266,6 +267,23 @@ class RefDef:
                                                            _ptr(Wc), norms.ctypes.data), "rd_build_reference_prolonged")
         self.k = k
         return norms
+
+    def build_reference_transient(self, k, Phi, nt):
+        """Transient coarse-mesh reference, eq. (14): Phi = N_s x rs spatial vectors (numpy, or a
+        column-major device tensor of shape (rs, N_s)).  Returns (pairs (k, 2) = (i, j), nu (k,))."""
+        if isinstance(Phi, np.ndarray):
+            Phi = np.asfortranarray(Phi, dtype=np.float64)
+            ns, rs = Phi.shape
+        else:
+            rs, ns = Phi.shape
+        if ns * nt != self.N:
+            raise ValueError("Phi does not have N / nt rows")
+        nu = np.zeros(k)
+        pairs = np.zeros((k, 2), dtype=np.int32)
+        self._check(self._lib.rd_build_reference_transient(self._h, k, rs, nt, _ptr(Phi), nu.ctypes.data, pairs.ctypes.data),
+                    "rd_build_reference_transient")
+        self.k = k
+        return pairs, nu
 
     def reference_info(self):
         b, deg, ms = C.c_int32(0), C.c_int64(0), C.c_double(0)

@@ -19,6 +19,7 @@
 #include "cg3.cuh"
 #include "sine.cuh"
 #include "prolong.cuh"
+#include "transient.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
 #include "pdas.cuh"
@@ -1060,6 +1061,96 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     k_kron_product<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(Ns, nt, ctx->ldw, ndim, qmax, nmax, n0, n1, k, ctx->kp,
                                                                                            d_modes, d_sel, d_tab, d_Q, ctx->W);
     ctx->launches++;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->ref_degree = 0;
+    ctx->ref_block = k;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    return RD_OK;
+}
+
+int rd_build_reference_transient(rd_ctx* ctx, int32_t k, int32_t rs, int32_t nt, const double* Phi, double* nu_out, int32_t* pairs_out)
+{
+    if (!ctx || !Phi || k < 1 || k > RD_MAX_K || rs < 1 || rs > RD_MAX_K || nt < 1 || nt > RD_DENSE_MAXN) return RD_EINVAL;
+    if (ctx->N % nt != 0) return fail(ctx, RD_EINVAL, "N = %lld is not a multiple of nt = %d", (long long)ctx->N, nt);
+    if ((int64_t)k > (int64_t)rs * nt) return fail(ctx, RD_EINVAL, "k = %d exceeds the %d x %d candidates", k, rs, nt);
+    const int64_t N = ctx->N, Ns = N / nt;
+    const auto t_begin = std::chrono::steady_clock::now();
+    RDTRY(alloc_reference(ctx, k));
+    struct Scratch {
+        std::vector<void*> p;
+        ~Scratch() { for (void* q : p) cudaFree(q); }
+    } scratch;
+    auto salloc = [&](void** out, size_t bytes) -> int {
+        if (cudaMalloc(out, std::max<size_t>(bytes, 16)) != cudaSuccess) { cudaGetLastError(); return fail(ctx, RD_ENOMEM, "cudaMalloc(%zu)", bytes); }
+        scratch.p.push_back(*out);
+        return RD_OK;
+    };
+    const size_t tt = (size_t)rs * nt * nt;
+    int32_t* d_sel = nullptr;
+    double *d_Phi = nullptr, *d_H = nullptr, *d_D = nullptr, *d_A = nullptr, *d_V = nullptr, *d_nu = nullptr, *d_Q = nullptr, *d_parts = nullptr,
+           *d_norms = nullptr;
+    const int nparts = 64;
+    RDTRY(salloc((void**)&d_sel, (size_t)2 * k * sizeof(int32_t)));
+    RDTRY(salloc((void**)&d_Phi, (size_t)Ns * rs * sizeof(double)));
+    RDTRY(salloc((void**)&d_H, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_D, (size_t)rs * nt * sizeof(double)));
+    RDTRY(salloc((void**)&d_A, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_V, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_nu, (size_t)rs * nt * sizeof(double)));
+    RDTRY(salloc((void**)&d_Q, tt * sizeof(double)));
+    RDTRY(salloc((void**)&d_parts, (size_t)nparts * k * sizeof(double)));
+    RDTRY(salloc((void**)&d_norms, (size_t)k * sizeof(double)));
+    CU(cudaMemcpyAsync(d_Phi, Phi, (size_t)Ns * rs * sizeof(double), cudaMemcpyDefault, ctx->stream));
+    // ---- the small temporal matrices of eq. (14): column t of H_i from one operator apply on e_t (x) phi_i
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    for (int i = 0; i < rs; ++i) {
+        const double* phi = d_Phi + (size_t)i * Ns;
+        for (int t = 0; t < nt; ++t) {
+            k_slab_vector<<<g, kThreads, 0, ctx->stream>>>(Ns, nt, t, phi, ctx->in0);
+            ctx->launches++;
+            RDTRY(launch_apply_H(ctx, ctx->in0, nullptr, ctx->tmp));
+            k_slab_dots<<<nt, 256, 0, ctx->stream>>>(Ns, ctx->tmp, phi, 0, d_H + ((size_t)i * nt + t) * nt);
+            ctx->launches++;
+        }
+        k_slab_dots<<<nt, 256, 0, ctx->stream>>>(Ns, ctx->d, phi, 1, d_D + (size_t)i * nt);
+        ctx->launches++;
+    }
+    k_transient_eigs<<<rs, 256, 0, ctx->stream>>>(nt, d_H, d_D, d_A, d_V, d_nu, d_Q);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    std::vector<double> nu_all((size_t)rs * nt);
+    CU(cudaMemcpyAsync(nu_all.data(), d_nu, nu_all.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    // ---- "selects the requested total rank from these spatial-temporal candidates": order (nu, i, j)
+    struct Pair { double nu; int i, j; };
+    std::vector<Pair> pr;
+    pr.reserve(nu_all.size());
+    for (int i = 0; i < rs; ++i)
+        for (int j = 0; j < nt; ++j) {
+            const double v = nu_all[(size_t)i * nt + j];
+            if (!(v == v)) return fail(ctx, RD_ENOTSPD, "spatial vector %d: temporal problem is not definite (zero vector?)", i);
+            pr.push_back(Pair{v, i, j});
+        }
+    std::sort(pr.begin(), pr.end(), [](const Pair& x, const Pair& y) {
+        if (x.nu != y.nu) return x.nu < y.nu;
+        if (x.i != y.i) return x.i < y.i;
+        return x.j < y.j;
+    });
+    std::vector<int32_t> sel((size_t)2 * k);
+    for (int c = 0; c < k; ++c) {
+        sel[2 * c] = pr[c].i;
+        sel[2 * c + 1] = pr[c].j;
+        if (nu_out) nu_out[c] = pr[c].nu;
+        if (pairs_out) { pairs_out[2 * c] = pr[c].i; pairs_out[2 * c + 1] = pr[c].j; }
+    }
+    CU(cudaMemcpyAsync(d_sel, sel.data(), sel.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemsetAsync(ctx->W, 0, (size_t)ctx->ldw * ctx->kp * sizeof(double), ctx->stream));  // pad rows stay zero
+    k_kron_vectors<<<g, kThreads, 0, ctx->stream>>>(Ns, nt, ctx->ldw, k, ctx->kp, d_sel, d_Phi, d_Q, ctx->W);
+    k_col_sumsq_parts<<<dim3(nparts, k), kThreads, 0, ctx->stream>>>(N, ctx->ldw, ctx->W, d_parts);
+    k_col_normalise<<<dim3(std::max(1, g / 8), k), kThreads, 0, ctx->stream>>>(N, ctx->ldw, nparts, d_parts, ctx->W, d_norms);
+    ctx->launches += 3;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->ref_degree = 0;
