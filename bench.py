@@ -144,9 +144,9 @@ def make_workload(args):
     return make_config(args.config)
 
 
-def workload_name(args, w):
+def workload_name(args, w, cap=None):
     return f"{w.name}: {w.kind} CHT {'x'.join(map(str, w.dims))}" + (f" x{w.nt} slabs" if w.nt > 1 else "") + \
-           f", N={w.N}, k={w.k}, {w.n_queries} queries/sequence, PDAS cap {w.pdas_cap}"
+           f", N={w.N}, k={w.k}, {w.n_queries} queries/sequence, PDAS cap {cap or w.pdas_cap}"
 
 
 def build_analytical_reference(g, w):
@@ -265,6 +265,63 @@ class Sequence:
         return self.g.solve_query(self.method, yd, psi, want_sets=False, **kw)
 
 
+def pdas_cap_for(args, w):
+    """PDAS step cap: --pdas-cap, else the paper's raised cap of 400 ("raised to 400 for Bore 4") on the
+    two full-size 2-D-in-space configs whose sequences need more than 100 steps (configs 2 and 4), else the workload's."""
+    if args.pdas_cap > 0:
+        return args.pdas_cap
+    if not args.twin and w.config in (2, 4):
+        return 400
+    return w.pdas_cap
+
+
+def query_ok(res):
+    """A query is a time-to-solution only if PDAS converged, every inner solve returned RD_OK and every KKT measure of
+    eq. (25) is <= 1e-8 (PAPER.md:343-348: "The reported times contain only sequences that satisfy these criteria")."""
+    return res["status"] == 0 and res["worst_inner_status"] == 0 and max(res["kkt"]) <= 1e-8
+
+
+def inactive_histogram(results, N):
+    """Share of the Algorithm-1 time spent at each |I|/N decile (S6: what compaction can save)."""
+    edges = [0.0, 0.1, 0.25, 0.5, 0.75, 0.9, 1.0000001]
+    t = [0.0] * (len(edges) - 1)
+    for res in results:
+        for s_ in res["steps"]:
+            if s_["n_inactive"] > 0:
+                f = s_["n_inactive"] / N
+                for b in range(len(t)):
+                    if edges[b] <= f < edges[b + 1]:
+                        t[b] += s_["t_iter"]
+    tot = sum(t) or 1.0
+    return {f"[{edges[b]:.2f},{min(edges[b + 1], 1.0):.2f})": round(t[b] / tot, 4) for b in range(len(t))}
+
+
+def latency_block(args, dev):
+    """Secondary block: config 2 (N = 262,144, k = 32), whose working set sits in the L2: the latency-bound case, judged
+    on microseconds per deflated iteration, not on GB/s.  One capped Algorithm-1 solve of H y = l from zero with the
+    analytical reference (milliseconds to build)."""
+    import torch
+
+    import paper_2606_17971_b200 as pkg
+    from workloads import make_config
+
+    w2 = make_config(2)
+    g2 = pkg.RefDef.from_workload(w2, pkg.Options(cg_cap=4000), stream=torch.cuda.current_stream().cuda_stream)
+    try:
+        g2.build_reference_sine(w2.k, w2.dims)
+        b = torch.from_numpy(w2.m * w2._target(2000)).to(dev)
+        act = torch.zeros(w2.N, dtype=torch.uint8, device=dev)
+        x0 = torch.zeros(w2.N, dtype=torch.float64, device=dev)
+        reps = [g2.solve_inactive(1, act, b, x0)[1] for _ in range(3)]
+        r = reps[-1]
+        return {"workload": "config2: 2d CHT 512x512, N=262144, k=32 (L2-resident: latency-bound)", "cg_iters": r["iters"],
+                "us_per_iter": round(1e3 * r["t_iter_ms"] / max(r["iters"], 1), 3),
+                "t_stage_us_per_iter": [round(x / max(r["iters"], 1), 3) for x in r["t_stage_us"]],
+                "stages": "A (K product), barrier, B (K^T product), barrier+reduce, k x k, C (updates + HW pass), barrier+reduce, outside loop"}
+    finally:
+        g2.close()
+
+
 def run_ours(args):
     import torch
 
@@ -283,7 +340,8 @@ def run_ours(args):
     w = make_workload(args)
     method = METHODS[args.method]
     stream = torch.cuda.current_stream()
-    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, alg1_variant=args.alg1_variant), stream=stream.cuda_stream)
+    cap = pdas_cap_for(args, w)
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=cap, alg1_variant=args.alg1_variant), stream=stream.cuda_stream)
     tall = 2 if args.alg1_variant == 1 else 1
     seq = Sequence(g, w, method, args.ref_tol, shard_queries(rank, world, w.n_queries), args.reference)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
@@ -309,21 +367,23 @@ def run_ours(args):
         res = seq.run(yd_in, psi_in)
         e1.record(stream)
         e1.synchronize()
-        return e0.elapsed_time(e1), res
+        return e0.elapsed_time(e1), res, q
 
-    warm_ms = [one_step(False)[0] for _ in range(args.warmup)]
+    warm = [one_step(False) for _ in range(args.warmup)]
+    warm_ms = [x[0] for x in warm]
     sampler = ClockSampler(local_rank)
     barrier()
     sampler.start()
     torch.cuda.profiler.start()  # ncu --profile-from-start off: only the timed region is listed
     launches0 = g.kernel_launches()
     builds0, refms0 = seq.ref_builds, seq.ref_ms
-    step_ms, results = [], []
+    step_ms, results, qpos = [], [], []
     t_wall0 = time.perf_counter()
     for _ in range(args.steps):
-        ms, res = one_step(False)
+        ms, res, q = one_step(False)
         step_ms.append(ms)
         results.append(res)
+        qpos.append(q)
     barrier()
     torch.cuda.profiler.stop()
     wall_ms = (time.perf_counter() - t_wall0) * 1e3
@@ -333,13 +393,14 @@ def run_ours(args):
     total_ms = sum(step_ms)
 
     # ---- roofline of the dominant kernel (persistent Algorithm-1 kernel, one launch per PDAS step with I != {})
-    alg_bytes = alg_ms = 0.0
+    alg_bytes = alg_bytes_N = alg_ms = 0.0
     alg_launches = iters = 0
     coarse_ms = upd_ms = 0.0
     n_steps = 0
-    statuses = {}
+    statuses, inner = {}, {}
     for res in results:
         statuses[res["status"]] = statuses.get(res["status"], 0) + 1
+        inner[res["worst_inner_status"]] = inner.get(res["worst_inner_status"], 0) + 1
         n_steps += res["n_steps"]
         for s in res["steps"]:
             coarse_ms += s["t_coarse"] + s["t_restrict"]
@@ -348,29 +409,39 @@ def run_ours(args):
                 alg_launches += 1
                 iters += s["cg_iters"]
                 alg_ms += s["t_iter"]
-                # + 3 applies outside the loop body (lines 3, 12, Verify) counted as iterations' worth of operator traffic
+                # the model charges the loop iterations only; the 3-5 operator applies and n x r passes outside the loop
+                # body (lines 3, 12, 16, Verify) are inside alg_ms but not in the bytes: the fraction errs low
                 alg_bytes += algorithmic_bytes_per_iter(w.nnz, w.N, s["n_inactive"], s["rank_used"], tall) * s["cg_iters"]
+                alg_bytes_N += algorithmic_bytes_per_iter(w.nnz, w.N, w.N, s["rank_used"], tall) * s["cg_iters"]
     peak, peak_src = load_peaks()
     achieved = alg_bytes / (alg_ms * 1e-3) / 1e9 if alg_ms > 0 else 0.0
     prof = load_profile().get(w.name, {})
-    roofline = {"kernel": "k_alg1 (persistent Algorithm-1 kernel: S3+S4+S5)", "bound": "hbm", "achieved": round(achieved, 1),
+    roofline = {"kernel": "k_alg1_v3 (persistent Algorithm-1 kernel: S3+S4+S5)", "bound": "hbm", "achieved": round(achieved, 1),
                 "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
                 # ncu dram__bytes_read + dram__bytes_write of one captured launch, per iteration, scaled to this run's
                 # mean iterations per launch (profiles/bench_workload_profile.json names the capture)
                 "traffic": (prof["dram_bytes_per_iter"] * iters / max(alg_launches, 1)) if "dram_bytes_per_iter" in prof else None,
                 "bytes_per_launch": alg_bytes / max(alg_launches, 1), "ms_per_launch": alg_ms / max(alg_launches, 1),
                 "launches": alg_launches, "cg_iters": iters, "us_per_iter": 1e3 * alg_ms / max(iters, 1),
-                "share_of_step": round(alg_ms / total_ms, 4) if total_ms else None}
+                "share_of_step": round(alg_ms / total_ms, 4) if total_ms else None,
+                "bytes_model": "24 nnz + 17 N + 112 n + 8 n r per iteration with n = |I|, r = retained rank of each launch (DESIGN.md 5)",
+                "achieved_if_every_launch_streamed_all_N_rows": round(alg_bytes_N / (alg_ms * 1e-3) / 1e9, 1) if alg_ms > 0 else 0.0,
+                "alg1_time_share_by_inactive_fraction": inactive_histogram(results, w.N)}
 
-    # ---- e2e: the same step with host buffers (one timed query; the context is already warm)
-    e2e_steps = max(1, args.e2e_steps)
-    e2e_ms = [one_step(True)[0] for _ in range(e2e_steps)]
+    # ---- e2e: the same metric with HOST buffers through the C ABI, continuing the same sequence for one full pass
+    # (every query id once, one reference build, one all-active start: the same mix as the timed region when K is a
+    # multiple of the pass length)
+    e2e_steps = args.e2e_steps if args.e2e_steps > 0 else w.n_queries
+    e2e = [one_step(True) for _ in range(e2e_steps)]
+    e2e_ms = [x[0] for x in e2e]
     h2d = 2 * 8 * w.N
     d2h = 3 * 8 * w.N
     mx_total, mx_e2e = reduce_max([total_ms, sum(e2e_ms)], dev if world > 1 else None)
     tot_steps = reduce_sum([float(args.steps)], dev if world > 1 else None)[0]
     value = mx_total * 1e-3 / tot_steps  # whole job: max-over-ranks time / queries all ranks processed
     e2e_value = mx_e2e * 1e-3 / (e2e_steps * world)
+    ok = [query_ok(r) for r in results]
+    conv_ms = [ms for ms, o in zip(step_ms, ok) if o]
 
     out = None
     if rank == 0:
@@ -378,15 +449,27 @@ def run_ours(args):
             "metric": "complete PDAS query time (incl. reference build)", "value": round(value, 4), "unit": "s/query",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(mx_total / args.steps, 3),
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": f"replicas x{world}",
+            "config": {"workload": workload_name(args, w, cap), "method": args.method, "parallelism": f"replicas x{world}",
                        "alg1_variant": args.alg1_variant, "reference": args.reference, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
-                       "l2": "flushed between steps (256 MiB write); the loop's working set (HW, K, K^T, vectors: about 120 MB) is the size of the L2"},
+                       "l2": "flushed between steps (256 MiB write)" + ("; the loop's working set is far larger than the 126 MB L2" if w.N > 1000000 else
+                                                                          "; the loop's working set (HW, K, K^T, vectors: about 120 MB) is the size of the L2")},
+            # time-to-solution bookkeeping: a query counts as converged only if PDAS stopped on a repeated
+            # active set, every inner solve verified, and all five KKT measures of eq. (25) are <= 1e-8
+            "converged_queries": int(sum(ok)), "non_converged_queries": int(len(ok) - sum(ok)),
+            "value_converged_only": round(sum(conv_ms) * 1e-3 / len(conv_ms), 4) if conv_ms else None,
+            "valid_time_to_solution": bool(all(ok)),
             "e2e": {"value": round(e2e_value, 4), "unit": "s/query", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps},
+                    "steps": e2e_steps, "query_positions": [x[2] for x in e2e], "converged_queries": int(sum(query_ok(x[1]) for x in e2e)),
+                    "query_s": [round(x * 1e-3, 3) for x in e2e_ms]},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": roofline,
             "breakdown": {"pdas_steps": n_steps, "query_status_counts": {str(k): v for k, v in statuses.items()},
+                          "worst_inner_status_counts": {str(k): v for k, v in inner.items()},
+                          "max_kkt": max(max(r["kkt"]) for r in results),
+                          "pdas_steps_per_query": [r["n_steps"] for r in results],
+                          "cg_iters_per_query": [int(r["total_cg_iters"]) for r in results],
+                          "query_positions": qpos,
                           "reference_builds_in_timed_region": ref_builds, "reference_ms": round(ref_ms, 1),
                           "alg1_ms": round(alg_ms, 1), "coarse_setup_ms": round(coarse_ms, 1), "update_ms": round(upd_ms, 1),
                           "wall_ms_incl_host": round(wall_ms, 1),
@@ -395,6 +478,10 @@ def run_ours(args):
                           "warmup_query_s": [round(x * 1e-3, 3) for x in warm_ms], "timed_query_s": [round(x * 1e-3, 3) for x in step_ms],
                           "reference_build_s_before_timed_region": round(refms0 * 1e-3, 3)},
         }
+        if method != 0:
+            out["reference_build"] = g.reference_info()
+        if world == 1 and not args.no_latency_block and not args.twin and w.config != 2:
+            out["latency_case"] = latency_block(args, dev)
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(args, w, g, method, iters / max(args.steps, 1), n_steps / max(args.steps, 1))
     g.close()
@@ -548,49 +635,77 @@ def run_replay(args):
 
 
 # ----------------------------------------------------------------------------------------------- oracle legs
-def oracle_sample(w, method, W, iters_per_query, steps_per_query, budget_s, seed_qid=0):
-    """Times the oracle, as it stands (single thread), on a bounded sample of one query of the workload: Algorithm 1
-    on the full inactive system of the first query (b = l), `cap` iterations, coarse setup included; the time per
-    iteration is scaled to a complete query with the CG iterations per query the CUDA arm observed."""
-    import oracle
+class OracleTimer:
+    """Times the oracle (test infrastructure; built here with -fopenmp so that its row loops use the host cores, the
+    arithmetic as it stands) on a bounded sample of the workload: Algorithm 1 on the full-domain inactive system of a
+    query (b = l, zero start).  Line 2 (the coarse setup: QR + SVD, B Z, E, Cholesky) is built and timed ONCE; every
+    sample is a capped run of the loop on it.  A complete query is extrapolated as
+    seconds per CG iteration x CG iterations per query + setup seconds x PDAS steps per query, labelled as such."""
 
-    o = oracle.Oracle.from_workload(w)
-    yd = w._target(1000 * w.config + seed_qid)
-    b = w.m * yd
-    idx = np.arange(w.N, dtype=np.int64)
-    Zt = W if (method != 0 and W is not None) else None
-    # calibrate: 2 and 34 iterations, then as many as fit the budget.  The coarse setup dominates both calibration
-    # runs on the deflated method, so their difference is noisy: the per-iteration estimate is floored at a quarter
-    # of t34/34 (an upper bound of the true value), which bounds the timed run at 4 x budget whatever the noise.
-    t0 = time.perf_counter()
-    o.alg1(idx, b, np.zeros(w.N), Zt, cap=2)
-    t2 = time.perf_counter() - t0
-    t0 = time.perf_counter()
-    o.alg1(idx, b, np.zeros(w.N), Zt, cap=34)
-    t34 = time.perf_counter() - t0
-    per_it = max((t34 - t2) / 32.0, 0.25 * t34 / 34.0, 1e-9)
-    setup = max(t2 - 2 * per_it, 0.0)
-    cap = int(max(16, min(20000, (budget_s - setup) / per_it)))
-    t0 = time.perf_counter()
-    _, rep = o.alg1(idx, b, np.zeros(w.N), Zt, cap=cap)
-    t = time.perf_counter() - t0
-    done = max(rep["iters"], 1)
-    per_it = max((t - setup) / done, 1e-9)
-    per_query = per_it * iters_per_query + setup * steps_per_query
-    return per_query, dict(s_per_cg_iter=per_it, s_coarse_setup=setup, iters_timed=done, seconds_timed=t,
-                           iters_per_query=iters_per_query, steps_per_query=steps_per_query)
+    def __init__(self, w, method, W):
+        import oracle
+
+        oracle.build_oracle(threaded=True)
+        self.w, self.method = w, method
+        self.o = oracle.Oracle.from_workload(w, threaded=True)
+        self.cores = self.o.threads
+        self.idx = np.arange(w.N, dtype=np.int64)
+        t0 = time.perf_counter()
+        self.cs = self.o.coarse(self.idx, W if (method != 0 and W is not None) else np.zeros((w.N, 0)))
+        self.setup_s = time.perf_counter() - t0 if method != 0 else 0.0
+        # one short run to size the samples
+        b = w.m * w._target(1000 * w.config)
+        t0 = time.perf_counter()
+        _, rep = self.o.alg1_on(self.cs, b, np.zeros(w.N), cap=4)
+        self.per_it_est = max((time.perf_counter() - t0) / (max(rep["iters"], 1) + 3.0), 1e-9)  # + the applies outside the loop
+
+    def sample(self, budget_s, seed_qid=0):
+        w = self.w
+        b = w.m * w._target(1000 * w.config + seed_qid)
+        cap = int(max(4, min(20000, budget_s / self.per_it_est)))
+        t0 = time.perf_counter()
+        _, rep = self.o.alg1_on(self.cs, b, np.zeros(w.N), cap=cap)
+        t = time.perf_counter() - t0
+        done = max(rep["iters"], 1)
+        return t / (done + 3.0), done, t
+
+    def per_query(self, per_it, iters_per_query, steps_per_query):
+        return per_it * iters_per_query + self.setup_s * steps_per_query
 
 
 def cpu_baseline(args, w, g, method, iters_per_query, steps_per_query):
     W = g.get_reference() if method != 0 else None
-    v, d = oracle_sample(w, method, W, iters_per_query, steps_per_query, args.cpu_budget)
+    tm = OracleTimer(w, method, W)
+    per_it, done, t = tm.sample(args.cpu_budget)
+    v = tm.per_query(per_it, iters_per_query, steps_per_query)
     return {"value": round(v, 2), "unit": "s/query (extrapolated: measured s per CG iteration x the CG iterations per query of this run)",
-            "cores": 1, "kind": "oracle",
-            "sample": f"oracle Algorithm 1 ({args.method}) on the full-domain inactive system of query 0, {d['iters_timed']} iterations "
-                      f"timed in {d['seconds_timed']:.1f} s ({d['s_per_cg_iter'] * 1e3:.3f} ms/iteration, coarse setup "
-                      f"{d['s_coarse_setup']:.2f} s/PDAS step); scaled by {d['iters_per_query']:.0f} iterations and "
-                      f"{d['steps_per_query']:.0f} PDAS steps per query",
-            "detail": d}
+            "cores": tm.cores, "kind": "oracle",
+            "sample": f"oracle Algorithm 1 ({args.method}, {tm.cores} OpenMP threads) on the full-domain inactive system of query 0: "
+                      f"{done} iterations timed in {t:.1f} s ({per_it * 1e3:.3f} ms/iteration), coarse setup {tm.setup_s:.2f} s per PDAS step "
+                      f"timed once; scaled by {iters_per_query:.0f} iterations and {steps_per_query:.0f} PDAS steps per query",
+            "detail": dict(s_per_cg_iter=per_it, s_coarse_setup=tm.setup_s, iters_timed=done, seconds_timed=t,
+                           iters_per_query=iters_per_query, steps_per_query=steps_per_query)}
+
+
+def oracle_reference(w, method):
+    """The reference W the oracle arm solves with.  Up to 1.5 M DOFs: the definition, a library eigensolver on the
+    assembled H (oracle.reference_eigs).  Above that the eigensolve does not fit a run of a few minutes and the oracle's
+    analytical reference stands in (the time per iteration does not depend on the values of W); said in `sample`."""
+    import oracle
+
+    if method == 0:
+        return None, 0.0, "none"
+    t0 = time.perf_counter()
+    if w.N <= 1500000:
+        _, W = oracle.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+        kind = "library eigensolver on the assembled H"
+    elif w.nt > 1:
+        W = oracle.spacetime_reference(w.dims, w.nt, 1.0 / w.nt, w.k)[-1]
+        kind = "analytical space-time reference (eigensolve of the assembled H skipped at this size)"
+    else:
+        W = oracle.sine_reference(w.dims, w.k)[-1]
+        kind = "analytical sine reference (eigensolve of the assembled H skipped at this size)"
+    return np.asfortranarray(W), time.perf_counter() - t0, kind
 
 
 def run_reference(args):
@@ -605,44 +720,46 @@ def run_reference(args):
     prof = load_profile().get(w.name, {}).get(args.method, {})
     iters_per_query = float(prof.get("cg_iters_per_query", 0.0))
     steps_per_query = float(prof.get("pdas_steps_per_query", w.pdas_cap))
-    W = None
-    t_ref = 0.0
-    if method != 0:
-        t0 = time.perf_counter()
-        _, W = oracle.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
-        t_ref = time.perf_counter() - t0
-    budget = max(2.0, min(args.cpu_budget, 240.0 / max(args.steps + args.warmup, 1)))
-    vals, detail = [], None
+    W, t_ref, ref_kind = oracle_reference(w, method)
+    tm = OracleTimer(w, method, W)
+    nsteps = max(args.steps + args.warmup, 1)
+    budget = max(0.5, min(args.cpu_budget, (180.0 - 2.0 * tm.setup_s) / nsteps))
+    vals, last = [], None
     for i in range(args.warmup + args.steps):
-        v, detail = oracle_sample(w, method, W, iters_per_query or 1.0, steps_per_query, budget, seed_qid=i % w.n_queries)
+        per_it, done, t = tm.sample(budget, seed_qid=i % w.n_queries)
+        last = (per_it, done, t)
         if i >= args.warmup:
-            vals.append(v)
+            vals.append(tm.per_query(per_it, iters_per_query or 1.0, steps_per_query))
     value = sum(vals) / len(vals) + t_ref / w.n_queries
     if not iters_per_query:
         unit_note = " (no recorded CG iterations per query for this workload: value is s per CG ITERATION-equivalent)"
     else:
         unit_note = ""
-    sample = (f"oracle Algorithm 1 ({args.method}) on the full-domain inactive system, {detail['iters_timed']} iterations per step "
-              f"({detail['s_per_cg_iter'] * 1e3:.3f} ms/iteration), scaled to a query by the recorded {iters_per_query:.0f} CG iterations "
-              f"and {steps_per_query:.0f} PDAS steps per query (profiles/bench_workload_profile.json); reference by a library "
-              f"eigensolver ({t_ref:.1f} s) charged over the {w.n_queries} queries of a pass{unit_note}")
+    sample = (f"oracle Algorithm 1 ({args.method}, {tm.cores} OpenMP threads) on the full-domain inactive system, {last[1]} iterations per step "
+              f"({last[0] * 1e3:.3f} ms/iteration; coarse setup {tm.setup_s:.1f} s timed once), scaled to a query by the recorded "
+              f"{iters_per_query:.0f} CG iterations and {steps_per_query:.0f} PDAS steps per query (profiles/bench_workload_profile.json); "
+              f"reference: {ref_kind} ({t_ref:.1f} s) charged over the {w.n_queries} queries of a pass{unit_note}")
     return {"impl": "reference", "metric": "complete PDAS query time (incl. reference build)", "value": round(value, 2),
             "unit": "s/query", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": round(1e3 * value, 1), "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args, w), "method": args.method, "parallelism": "host cores, rank 0 only"},
-            "cpu_baseline": {"value": round(value, 2), "unit": "s/query", "kind": "oracle", "cores": 1, "sample": sample},
+            "config": {"workload": workload_name(args, w, pdas_cap_for(args, w)), "method": args.method, "parallelism": "host cores, rank 0 only"},
+            "cpu_baseline": {"value": round(value, 2), "unit": "s/query", "kind": "oracle", "cores": tm.cores, "sample": sample},
             "e2e": {"value": round(value, 2), "unit": "s/query", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
 
 
-def main(argv=None):
+def build_parser():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json config; default 5 = the largest (160^3, N = 4,096,000, k = 64), the one the metric's "
+                         "bandwidth target is quoted on")
+    ap.add_argument("--pdas-cap", type=int, default=0, help="PDAS step cap; 0 = 400 on configs 2 and 4 (PAPER.md:341), else the workload's")
+    ap.add_argument("--no-latency-block", action="store_true", help="skip the config-2 microseconds-per-iteration block")
     ap.add_argument("--twin", default=None)
     ap.add_argument("--method", default="refdef", choices=list(METHODS))
     ap.add_argument("--ref-tol", type=float, default=1e-3)
@@ -650,7 +767,7 @@ def main(argv=None):
                     help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
                          "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4); "
                          "coarse: Jacobi-scaled modes of the half-resolution operator, P1-prolonged (PAPER.md:176)")
-    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--e2e-steps", type=int, default=0, help="host-buffer queries after the timed region; 0 = one full pass of the sequence")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default="query", choices=["query", "loop", "replay"],
@@ -658,7 +775,11 @@ def main(argv=None):
     ap.add_argument("--cg-cap", type=int, default=500000, help="--mode loop: iteration cap of each solve")
     ap.add_argument("--alg1-variant", type=int, default=0, help="rd_options.alg1_variant (0: default kernel; 1: literal recurrence)")
     ap.add_argument("--ref-sweeps", type=int, default=60, help="--mode loop: filter sweeps of the reference build")
-    args = ap.parse_args(argv)
+    return ap
+
+
+def main(argv=None):
+    args = build_parser().parse_args(argv)
     if args.impl == "reference":
         out = run_reference(args)
     elif args.mode == "loop":

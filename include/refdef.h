@@ -97,11 +97,19 @@ typedef struct {
 } rd_step_report;
 
 typedef struct {
-    int32_t n_steps, status;
+    int32_t n_steps, status; /* status: outcome of the PDAS loop (RD_OK: the active set repeated; RD_ESTEPS; RD_ECYCLE) */
     double kkt[5];    /* eq. (25): stationarity, primal, dual, complementarity, projected gradient */
     double t_total;   /* ms, whole call */
     double t_reference_charged; /* ms of rd_build_reference charged to this query (first query after a build) */
     int64_t total_cg_iters;
+    /* Inner solves are recorded separately from the outer loop ("Caps, cycles, ... and residual failures
+     * are recorded separately"): a query is a time-to-solution only if status == RD_OK, worst_inner_status == RD_OK
+     * and every kkt[i] <= 1e-8. */
+    int32_t worst_inner_status; /* the most severe steps[i].status of this query: RD_OK unless some Algorithm-1 solve ended
+                                   RD_ENOTSPD (-5, most severe), RD_ERESID (-9) or RD_ECAP (-6) */
+    int32_t n_inner_failed;     /* number of steps whose inner solve did not return RD_OK */
+    int32_t n_fallbacks;        /* number of steps that took the rank-zero fallback of PAPER.md:265 (cond(E) > 1e10) */
+    int32_t reserved;
 } rd_query_report;
 
 /* Report of one Algorithm-1 solve through rd_solve_inactive. */
@@ -220,7 +228,12 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
                       rd_solve_report* rep);
 /* S1+S2 for one active set: restricted basis, Gram G = W_I^T W_I and E_W = W_I^T H_II W_I (both k x k
  * column-major, may be NULL), and C = T E^{-1} T^T (k x k, the coarse solve in W_I coordinates, may be NULL);
- * rank / cond / fallback as in rd_step_report. */
+ * rank / cond / fallback as in rd_step_report.
+ * SEQUENCE STATE.  The single-step entry points (rd_coarse_setup, rd_solve_inactive, rd_energy_fraction) work on
+ * their own copy of the active flags: the active set and state a later rd_solve_query inherits under
+ * RD_INIT_PAPER are kept apart and are not touched by them.  The zero-extension history (eq. (13),
+ * DESIGN.md reading A9) is advanced by rd_solve_inactive (every restriction of the sequence counts, whichever
+ * method runs) and only read by rd_coarse_setup and rd_energy_fraction. */
 int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C,
                     int32_t* rank_used, double* cond_E, int32_t* fallback);
 

@@ -20,6 +20,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "refdef_oracle.c")
 _LIB = os.path.join(_HERE, "librefdef_oracle.so")
+_LIB_OMP = os.path.join(_HERE, "librefdef_oracle_omp.so")
 
 JACOBI_CG, REFDEF, ZEROEXT = 0, 1, 2
 INIT_PAPER, INIT_ALL_ACTIVE, INIT_ALL_INACTIVE, INIT_GIVEN = 0, 1, 2, 3
@@ -27,11 +28,15 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -5: "enotspd", -6: "ecap", 
                 -9: "eresid"}
 
 
-def build_oracle(force: bool = False) -> str:
-    """Compile the oracle with gcc (plain -O2, no fast-math, single thread)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-o", _LIB, _SRC, "-lm"])
-    return _LIB
+def build_oracle(force: bool = False, threaded: bool = False) -> str:
+    """Compile the oracle with gcc (plain -O2, no fast-math).  threaded = False: the single-thread build every parity
+    test uses.  threaded = True: the same file with -fopenmp (row loops split over the host cores), for the TIMING
+    legs of bench.py only."""
+    lib = _LIB_OMP if threaded else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c99"] + (["-fopenmp"] if threaded else []) +
+                              ["-fPIC", "-shared", "-o", lib, _SRC, "-lm"])
+    return lib
 
 
 class _StepReport(C.Structure):
@@ -77,8 +82,9 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def _load():
-    lib = C.CDLL(build_oracle())
+def _load(threaded: bool = False):
+    lib = C.CDLL(build_oracle(threaded=threaded))
+    lib.orc_threads.restype = C.c_int
     lib.orc_create.restype = C.c_void_p
     lib.orc_create.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]
     lib.orc_destroy.argtypes = [C.c_void_p]
@@ -99,6 +105,8 @@ def _load():
     lib.orc_coarse_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.orc_alg1.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                              C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(_SolveReport)]
+    lib.orc_alg1_cs.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(_SolveReport)]
     lib.orc_solve_query.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                     C.POINTER(_Options), C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.POINTER(_StepReport), C.c_void_p, C.POINTER(_QueryReport)]
@@ -107,21 +115,20 @@ def _load():
     return lib
 
 
-_lib = None
+_libs = {}
 
 
-def _get_lib():
-    global _lib
-    if _lib is None:
-        _lib = _load()
-    return _lib
+def _get_lib(threaded: bool = False):
+    if threaded not in _libs:
+        _libs[threaded] = _load(threaded)
+    return _libs[threaded]
 
 
 class CoarseSpace:
     """Handle on the oracle's coarse space of one inactive system (eq. (18))."""
 
     def __init__(self, orc: "Oracle", idx: np.ndarray, Zt: np.ndarray):
-        self._lib = _get_lib()
+        self._lib = orc._lib  # the build (plain or threaded) of the context it belongs to
         self._orc = orc
         self.idx = np.ascontiguousarray(idx, dtype=np.int64)
         self.n = len(self.idx)
@@ -162,8 +169,9 @@ class CoarseSpace:
 class Oracle:
     """One operator = one context (host arrays).  sigma = alpha (reading A1)."""
 
-    def __init__(self, rowptr, colidx, val, m, sigma):
-        self._lib = _get_lib()
+    def __init__(self, rowptr, colidx, val, m, sigma, threaded: bool = False):
+        self._lib = _get_lib(threaded)
+        self.threads = int(self._lib.orc_threads())
         self.N = len(m)
         self._rowptr = np.ascontiguousarray(rowptr, dtype=np.int64)
         self._colidx = np.ascontiguousarray(colidx, dtype=np.int32)
@@ -176,8 +184,8 @@ class Oracle:
             raise ValueError("orc_create failed (N <= 0 or m_i <= 0)")
 
     @classmethod
-    def from_workload(cls, w):
-        return cls(w.rowptr, w.colidx, w.val, w.m, w.alpha)
+    def from_workload(cls, w, threaded: bool = False):
+        return cls(w.rowptr, w.colidx, w.val, w.m, w.alpha, threaded=threaded)
 
     def __del__(self):
         try:
@@ -242,6 +250,16 @@ class Oracle:
         rep = _SolveReport()
         self._lib.orc_alg1(self._h, idx.ctypes.data, len(idx), b.ctypes.data, x.ctypes.data, zp, k, eps,
                            eps if eps_c is None else eps_c, cap, replace_period, jacobi, C.byref(rep))
+        return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+
+    def alg1_on(self, cs: "CoarseSpace", b, x0, eps=1e-8, eps_c=None, cap=500000, replace_period=0, jacobi=1):
+        """Algorithm 1 on a coarse space that line 2 has already built (self.coarse(idx, Zt)): the same solve as alg1
+        without repeating the setup.  Returns (x, report dict)."""
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        x = np.array(x0, dtype=np.float64, copy=True)
+        rep = _SolveReport()
+        self._lib.orc_alg1_cs(self._h, cs.idx.ctypes.data, cs.n, b.ctypes.data, x.ctypes.data, cs._h, eps,
+                              eps if eps_c is None else eps_c, cap, replace_period, jacobi, C.byref(rep))
         return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
 
     def solve_query(self, method, y_d, psi, W=None, opt: Optional[OracleOptions] = None, J0=None,

@@ -26,11 +26,27 @@
  * projector identities, restriction-residual identity eq. (20)-(21),
  * closed-form spectrum, rank-zero == Jacobi-CG, Fig. 2 transfer pattern, energy fraction
  * eq. (24).  Unpinned: CG iteration counts at full size ("parity unpinned").
+ *
+ * Threads.  The parity tests use the plain build (gcc -O2, single thread, the loops exactly as written).
+ * The TIMING legs of bench.py (cpu_baseline, --impl reference) may build the same file with -fopenmp: the
+ * ORC_PAR_FOR / ORC_PAR_SUM marks below then split the row loops over the host cores in static chunks
+ * (sums change their order, nothing else changes; K^T t becomes a row loop over a transposed copy whose
+ * entries are in the order of the scatter, so that product is bit-identical).  Without -fopenmp the marks
+ * are empty.  tests/test_oracle_pins.py checks the threaded build against the plain one.
  */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#define ORC_PRAGMA(x) _Pragma(#x)
+#define ORC_PAR_FOR ORC_PRAGMA(omp parallel for schedule(static))
+#define ORC_PAR_SUM(v) ORC_PRAGMA(omp parallel for schedule(static) reduction(+ : v))
+#else
+#define ORC_PAR_FOR
+#define ORC_PAR_SUM(v)
+#endif
 
 #define ORC_OK 0
 #define ORC_EINVAL (-1)
@@ -64,7 +80,20 @@ typedef struct {
     double *y_state;
     uint8_t *J_state;   /* 1 = active */
     uint8_t *A_hist;    /* 1 = DOF was active at an earlier restriction of this sequence */
+#ifdef _OPENMP
+    int64_t *t_rowptr; int32_t *t_row; double *t_val; /* K^T by rows, entries of a row in ascending row of K */
+#endif
 } orc_ctx;
+
+/* threads the timing build uses (1 for the plain build) */
+int orc_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
 
 typedef struct {
     int32_t n_inactive, cg_iters, rank_used, coarse_fallback, replacements, status;
@@ -114,6 +143,24 @@ orc_ctx *orc_create(int64_t N, const int64_t *rowptr, const int32_t *colidx, con
     for (int64_t r = 0; r < N; r++)
         for (int64_t e = rowptr[r]; e < rowptr[r + 1]; e++)
             c->d[colidx[e]] += sigma * val[e] * val[e] / m[r];
+#ifdef _OPENMP
+    /* transposed copy for the threaded K^T t (counting sort: ascending row of K inside each row of K^T) */
+    c->t_rowptr = (int64_t *)calloc((size_t)(N + 1), sizeof(int64_t));
+    c->t_row = (int32_t *)malloc((size_t)c->nnz * sizeof(int32_t));
+    c->t_val = (double *)malloc((size_t)c->nnz * sizeof(double));
+    for (int64_t e = 0; e < c->nnz; e++) c->t_rowptr[colidx[e] + 1]++;
+    for (int64_t i = 0; i < N; i++) c->t_rowptr[i + 1] += c->t_rowptr[i];
+    {
+        int64_t *cur = (int64_t *)malloc((size_t)N * sizeof(int64_t));
+        memcpy(cur, c->t_rowptr, (size_t)N * sizeof(int64_t));
+        for (int64_t r = 0; r < N; r++)
+            for (int64_t e = rowptr[r]; e < rowptr[r + 1]; e++) {
+                int64_t pos = cur[colidx[e]]++;
+                c->t_row[pos] = (int32_t)r; c->t_val[pos] = val[e];
+            }
+        free(cur);
+    }
+#endif
     return c;
 }
 
@@ -123,6 +170,9 @@ void orc_destroy(orc_ctx *c)
     free(c->rowptr); free(c->colidx); free(c->val); free(c->m); free(c->d);
     free(c->t); free(c->full_in); free(c->full_out);
     free(c->y_state); free(c->J_state); free(c->A_hist);
+#ifdef _OPENMP
+    free(c->t_rowptr); free(c->t_row); free(c->t_val);
+#endif
     free(c);
 }
 
@@ -137,6 +187,7 @@ void orc_reset_sequence(orc_ctx *c)
 /* out = K v */
 void orc_apply_K(const orc_ctx *c, const double *v, double *out)
 {
+    ORC_PAR_FOR
     for (int64_t r = 0; r < c->N; r++) {
         double s = 0.0;
         for (int64_t e = c->rowptr[r]; e < c->rowptr[r + 1]; e++) s += c->val[e] * v[c->colidx[e]];
@@ -147,17 +198,28 @@ void orc_apply_K(const orc_ctx *c, const double *v, double *out)
 /* out = K^T t */
 void orc_apply_KT(const orc_ctx *c, const double *t, double *out)
 {
+#ifdef _OPENMP
+    ORC_PAR_FOR
+    for (int64_t i = 0; i < c->N; i++) {
+        double s = 0.0;
+        for (int64_t e = c->t_rowptr[i]; e < c->t_rowptr[i + 1]; e++) s += c->t_val[e] * t[c->t_row[e]];
+        out[i] = s;
+    }
+#else
     for (int64_t i = 0; i < c->N; i++) out[i] = 0.0;
     for (int64_t r = 0; r < c->N; r++)
         for (int64_t e = c->rowptr[r]; e < c->rowptr[r + 1]; e++) out[c->colidx[e]] += c->val[e] * t[r];
+#endif
 }
 
 /* out = H v = m.*v + sigma K^T ((K v)./m)   (eq. (5); mass-weighted form :133) */
 void orc_apply_H(orc_ctx *c, const double *v, double *out)
 {
     orc_apply_K(c, v, c->t);
+    ORC_PAR_FOR
     for (int64_t r = 0; r < c->N; r++) c->t[r] /= c->m[r];
     orc_apply_KT(c, c->t, out);
+    ORC_PAR_FOR
     for (int64_t i = 0; i < c->N; i++) out[i] = c->m[i] * v[i] + c->sigma * out[i];
 }
 
@@ -167,8 +229,10 @@ void orc_diag_H(const orc_ctx *c, double *d_out) { memcpy(d_out, c->d, (size_t)c
 static void apply_B(orc_ctx *c, const int64_t *idx, int64_t n, const double *x, double *out)
 {
     memset(c->full_in, 0, (size_t)c->N * sizeof(double));
+    ORC_PAR_FOR
     for (int64_t q = 0; q < n; q++) c->full_in[idx[q]] = x[q];
     orc_apply_H(c, c->full_in, c->full_out);
+    ORC_PAR_FOR
     for (int64_t q = 0; q < n; q++) out[q] = c->full_out[idx[q]];
 }
 
@@ -179,6 +243,7 @@ void orc_apply_B(orc_ctx *c, const int64_t *idx, int64_t n, const double *x, dou
 static double dot(const double *a, const double *b, int64_t n)
 {
     double s = 0.0;
+    ORC_PAR_SUM(s)
     for (int64_t i = 0; i < n; i++) s += a[i] * b[i];
     return s;
 }
@@ -207,6 +272,7 @@ static void householder_qr(const double *A, int64_t n, int k, double *Q, double 
         for (int c2 = j; c2 < k; c2++) {
             double *cc = W + (size_t)c2 * n;
             double f = beta[j] * dot(v + j, cc + j, n - j);
+            ORC_PAR_FOR
             for (int64_t i = j; i < n; i++) cc[i] -= f * v[i];
         }
     }
@@ -220,6 +286,7 @@ static void householder_qr(const double *A, int64_t n, int k, double *Q, double 
             const double *v = V + (size_t)j * n;
             if (beta[j] == 0.0) continue;
             double f = beta[j] * dot(v + j, q + j, n - j);
+            ORC_PAR_FOR
             for (int64_t i = j; i < n; i++) q[i] -= f * v[i];
         }
     }
@@ -386,12 +453,14 @@ orc_coarse *orc_coarse_build(orc_ctx *c, const int64_t *idx, int64_t n, const do
         cs->E = (double *)malloc((size_t)r * r * sizeof(double));
         cs->L = (double *)malloc((size_t)r * r * sizeof(double));
         cs->small = (double *)malloc((size_t)r * sizeof(double));
-        for (int j = 0; j < r; j++)
+        for (int j = 0; j < r; j++) {
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) {
                 double acc = 0.0;
                 for (int q = 0; q < p; q++) acc += Q[(size_t)q * n + i] * V[(size_t)j * p + q];
                 cs->Z[(size_t)j * n + i] = acc;
             }
+        }
         for (int j = 0; j < r; j++) apply_B(c, idx, n, cs->Z + (size_t)j * n, cs->BZ + (size_t)j * n);
         for (int a = 0; a < r; a++)
             for (int b2 = 0; b2 < r; b2++)
@@ -427,8 +496,10 @@ void orc_coarse_Q(orc_coarse *cs, const double *v, double *out)
     if (r == 0) return;
     for (int j = 0; j < r; j++) cs->small[j] = dot(cs->Z + (size_t)j * n, v, n);
     chol_solve(cs->L, r, cs->small);
-    for (int j = 0; j < r; j++)
+    for (int j = 0; j < r; j++) {
+        ORC_PAR_FOR
         for (int64_t i = 0; i < n; i++) out[i] += cs->Z[(size_t)j * n + i] * cs->small[j];
+    }
 }
 
 /* out = P v = v - Z E^{-1} (BZ)^T v  (eq. (18); cached BZ) */
@@ -439,8 +510,10 @@ void orc_coarse_P(orc_coarse *cs, const double *v, double *out)
     if (r == 0) return;
     for (int j = 0; j < r; j++) cs->small[j] = dot(cs->BZ + (size_t)j * n, v, n);
     chol_solve(cs->L, r, cs->small);
-    for (int j = 0; j < r; j++)
+    for (int j = 0; j < r; j++) {
+        ORC_PAR_FOR
         for (int64_t i = 0; i < n; i++) out[i] -= cs->Z[(size_t)j * n + i] * cs->small[j];
+    }
 }
 
 int orc_coarse_rank(const orc_coarse *cs) { return cs->r; }
@@ -472,11 +545,11 @@ static double verify(orc_ctx *c, const int64_t *idx, int64_t n, const double *b,
     return (nb > 0.0) ? sqrt(s) / nb : sqrt(s);
 }
 
-/* Algorithm 1, line numbers as reconstructed in SURVEY.md §8(c) O3.
- * idx: the n inactive DOFs (ascending); b, x: length n (x holds x0 on entry);
- * Zt: restricted candidate basis Z~ (n x k column-major) or NULL / k = 0 for Jacobi-CG. */
-int orc_alg1(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double *x, const double *Zt, int k,
-             double eps, double eps_c, int cap, int replace_period, int jacobi, orc_solve_report *rep)
+/* Algorithm 1, line numbers as reconstructed in SURVEY.md §8(c) O3, on a coarse space that
+ * line 2 has already built (orc_coarse_build; rank zero = Jacobi-CG).
+ * idx: the n inactive DOFs (ascending); b, x: length n (x holds x0 on entry). */
+int orc_alg1_cs(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double *x, orc_coarse *cs,
+                double eps, double eps_c, int cap, int replace_period, int jacobi, orc_solve_report *rep)
 {
     memset(rep, 0, sizeof(*rep));
     double *r = (double *)malloc((size_t)n * sizeof(double));
@@ -488,8 +561,7 @@ int orc_alg1(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double 
     /* 1 */
     double nb = nrm2(b, n);
     double tau = (nb > 0.0) ? eps_c * nb : eps_c;
-    /* 2 */
-    orc_coarse *cs = orc_coarse_build(c, idx, n, Zt, k);
+    /* 2 (done by the caller) */
     rep->rank_used = cs->r; rep->coarse_fallback = cs->fallback; rep->cond_E = cs->cond_E;
     for (int64_t i = 0; i < n; i++) jac[i] = jacobi ? 1.0 / c->d[idx[i]] : 1.0;
     int status = ORC_ECAP, done = 0;
@@ -519,35 +591,43 @@ int orc_alg1(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double 
         if (!(pw > 0.0) || !(rho > 0.0)) { status = ORC_ENOTSPD; break; }
         /* 10 */
         double a = rho / pw;
+        ORC_PAR_FOR
         for (int64_t i = 0; i < n; i++) x[i] += a * p[i];
+        ORC_PAR_FOR
         for (int64_t i = 0; i < n; i++) r[i] -= a * w[i];
         /* 11 */
         if (nrm2(r, n) <= tau || (replace_period > 0 && it % replace_period == 0)) {
             rep->replacements++;
             /* 12 */
             apply_B(c, idx, n, x, w);
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) r[i] = b[i] - w[i];
             /* 13-15 */
             if (nrm2(r, n) <= tau) { status = ORC_OK; break; }
             /* 16 */
             orc_coarse_Q(cs, r, z);
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) x[i] += z[i];
             apply_B(c, idx, n, x, w);
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) r[i] = b[i] - w[i];
             /* 17-19 */
             if (nrm2(r, n) <= tau) { status = ORC_OK; break; }
             /* 20 */
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) Jr[i] = jac[i] * r[i];
             orc_coarse_P(cs, Jr, z);
             memcpy(p, z, (size_t)n * sizeof(double));
             rho = dot(r, z, n);
         } else {
             /* 22 */
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) Jr[i] = jac[i] * r[i];
             orc_coarse_P(cs, Jr, z);
             double rho_new = dot(r, z, n);
             /* 23 */
             double beta = rho_new / rho;
+            ORC_PAR_FOR
             for (int64_t i = 0; i < n; i++) p[i] = z[i] + beta * p[i];
             rho = rho_new;
         }
@@ -556,8 +636,17 @@ int orc_alg1(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double 
     rep->rel_resid_verified = verify(c, idx, n, b, x, w);
     if (status == ORC_OK && !(rep->rel_resid_verified <= eps)) status = ORC_ERESID;
     rep->status = status;
-    orc_coarse_free(cs);
     free(r); free(z); free(p); free(w); free(Jr); free(jac);
+    return status;
+}
+
+/* Algorithm 1 with its line 2: Zt = restricted candidate basis Z~ (n x k column-major) or NULL / k = 0 for Jacobi-CG. */
+int orc_alg1(orc_ctx *c, const int64_t *idx, int64_t n, const double *b, double *x, const double *Zt, int k,
+             double eps, double eps_c, int cap, int replace_period, int jacobi, orc_solve_report *rep)
+{
+    orc_coarse *cs = orc_coarse_build(c, idx, n, Zt, k);
+    int status = orc_alg1_cs(c, idx, n, b, x, cs, eps, eps_c, cap, replace_period, jacobi, rep);
+    orc_coarse_free(cs);
     return status;
 }
 

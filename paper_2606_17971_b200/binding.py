@@ -46,7 +46,8 @@ class _StepReport(C.Structure):
 
 class _QueryReport(C.Structure):
     _fields_ = [("n_steps", C.c_int32), ("status", C.c_int32), ("kkt", C.c_double * 5), ("t_total", C.c_double),
-                ("t_reference_charged", C.c_double), ("total_cg_iters", C.c_int64)]
+                ("t_reference_charged", C.c_double), ("total_cg_iters", C.c_int64), ("worst_inner_status", C.c_int32),
+                ("n_inner_failed", C.c_int32), ("n_fallbacks", C.c_int32), ("reserved", C.c_int32)]
 
 
 class _SolveReport(C.Structure):
@@ -380,4 +381,5 @@ class RefDef:
         step_list = [{f: getattr(steps[i], f) for f, _ in _StepReport._fields_} for i in range(ns)]
         return dict(status=st, n_steps=ns, kkt=[rep.kkt[i] for i in range(5)], y=y, u=u, lam=lam, steps=step_list,
                     J_bits=(Jb[:ns] if want_sets else None), hashes=[s["active_hash"] for s in step_list],
-                    t_total_ms=rep.t_total, t_reference_ms=rep.t_reference_charged, total_cg_iters=rep.total_cg_iters)
+                    t_total_ms=rep.t_total, t_reference_ms=rep.t_reference_charged, total_cg_iters=rep.total_cg_iters,
+                    worst_inner_status=rep.worst_inner_status, n_inner_failed=rep.n_inner_failed, n_fallbacks=rep.n_fallbacks)

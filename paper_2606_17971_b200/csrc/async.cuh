@@ -2,9 +2,12 @@
 // from global to shared memory.  No arithmetic of the method lives here.
 //
 // Use: a warp owns one stage buffer and one mbarrier (arrival count 1).  Lane 0 arms the barrier with the byte
-// count of the copies of that stage (arrive.expect_tx), lanes issue the copies, every lane waits on the phase
-// parity before reading the buffer.  The owner re-issues into the buffer only after all its lanes have read it
-// (__syncwarp), so no "empty" barrier is needed; the barrier's phases are waited on in order by one warp only.
+// count of the copies of that stage (arrive.expect_tx) and issues the copies, every lane waits on the phase
+// parity before reading the buffer (read-after-write: the mbarrier's complete_tx makes the async-proxy writes
+// visible to the waiting threads).  Write-after-read: the buffer is read through the generic proxy and refilled
+// through the async proxy; the owner warp orders the two with refill_fence() -- __syncwarp (every lane's
+// shared-memory loads of the old contents precede it) followed by fence.proxy.async.shared::cta in the issuing
+// lane, the documented cross-proxy fence -- before it re-arms the barrier and issues the next copy.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -41,6 +44,14 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
     while (!mbar_try_wait(bar, parity)) {}
+}
+
+// Orders this warp's generic-proxy accesses to shared memory (the loads of a staging buffer's old contents) before
+// the async-proxy writes of bulk copies issued after it.  All lanes of the warp call it (convergent).
+__device__ __forceinline__ void refill_fence()
+{
+    __syncwarp();
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
 // 1-D bulk copy global -> shared of `bytes` (multiple of 16; both addresses 16-byte aligned), completion

@@ -191,14 +191,10 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             cc[q] = ok ? scol[q * 32 + lane] : 0;
             aa[q] = ok ? sval[q * 32 + lane] : 0.0;
         }
-        // The refill below is an asynchronous write into the slot just read.  Shared-memory loads complete out of
-        // program order with respect to it (they can queue behind this SM's global gathers for longer than a bulk
-        // copy takes to land: measured as rare wrong rows on config 5), so the loaded registers are CONSUMED by a
-        // real instruction first: the warp cannot issue the vote before every load has written back.
-        int chk = 0;
-#pragma unroll
-        for (int q = 0; q < WDC; ++q) chk ^= cc[q] ^ __double2hiint(aa[q]) ^ __double2loint(aa[q]);
-        if (__ballot_sync(0xffffffffu, chk == 0x5a5a5a5b)) __nanosleep(1);  // harmless if it ever fires
+        // The refill below is an async-proxy write into the slot just read through the generic proxy (a bulk copy
+        // issued right after the loads can otherwise land before they have executed: seen on config 5 in round 1).
+        // refill_fence = __syncwarp + fence.proxy.async.shared::cta orders the two (async.cuh).
+        refill_fence();
         next();
 #pragma unroll
         for (int q = 0; q < WDC; ++q) xx[q] = (q < wd) ? v0[cc[q]] : 0.0;
@@ -232,6 +228,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         };
         int64_t s = s0 + warp;
         int wd = 0;
+        refill_fence();  // the ring was last read (generic proxy) by the previous stage, possibly by another warp, before a CTA barrier
         if (s < s1) {
             int64_t o;
             extent(s, o, wd);
@@ -393,6 +390,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             auto issue = [&](int64_t t) { issue_tile(t); };
             int64_t t = warp;
             double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi = 0.0;
+            refill_fence();  // as in spmv_staged: previous stage's generic reads of these bytes precede the CTA barrier above
             if (t < ntiles) {
                 issue(t);
                 const int64_t i = row0 + 32 * t + lane;
@@ -455,7 +453,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
                     acc[0] += a0 + a1;
                     acc[1] += b0 + b1;
                 }
-                __syncwarp();  // every lane has read the tile and zb
+                refill_fence();  // every lane has read the tile and zb; generic reads ordered before the async refill
                 if (tn < ntiles) issue(tn);
                 ri = rin; wi = win; di = din; pi = pin; xi = xin;
             }

@@ -61,6 +61,7 @@ struct rd_ctx {
     double *b = nullptr, *tmp = nullptr, *Hy = nullptr, *ell = nullptr, *y = nullptr, *ystate = nullptr;
     double *lam = nullptr, *u = nullptr, *in0 = nullptr, *in1 = nullptr;  // staging for host callers
     uint8_t *act = nullptr, *act_new = nullptr, *hist = nullptr, *bits = nullptr, *act_stage = nullptr;
+    uint8_t* act_seq = nullptr;  // the active set the next query of the sequence inherits; only rd_solve_query writes it
     uint8_t* h_bits = nullptr;  // pinned
     int* d_nactive = nullptr;
     int* h_nactive = nullptr;
@@ -565,6 +566,7 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     RDTRY(dalloc(ctx, &ctx->act_new, L));
     RDTRY(dalloc(ctx, &ctx->hist, L));
     RDTRY(dalloc(ctx, &ctx->act_stage, L));
+    RDTRY(dalloc(ctx, &ctx->act_seq, L));
     RDTRY(dalloc(ctx, &ctx->bits, (size_t)(N + 7) / 8));
     RDTRY(halloc(ctx, &ctx->h_bits, (size_t)(N + 7) / 8));
     RDTRY(dalloc(ctx, &ctx->d_nactive, 1));
@@ -618,6 +620,7 @@ int rd_reset_sequence(rd_ctx* ctx)
     ctx->have_state = false;
     CU(cudaMemsetAsync(ctx->ystate, 0, ctx->ldw * sizeof(double), ctx->stream));
     CU(cudaMemsetAsync(ctx->act, 0, ctx->ldw, ctx->stream));
+    CU(cudaMemsetAsync(ctx->act_seq, 0, ctx->ldw, ctx->stream));
     CU(cudaMemsetAsync(ctx->hist, 0, ctx->ldw, ctx->stream));
     return RD_OK;
 }
@@ -1329,6 +1332,8 @@ int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double*
     int init = ctx->opt.init;
     if (init == RD_INIT_PAPER) init = ctx->have_state ? -1 : RD_INIT_ALL_ACTIVE;
     if (!ctx->have_state) CU(cudaMemsetAsync(ctx->ystate, 0, ctx->ldw * sizeof(double), ctx->stream));
+    if (init == -1)  // inherit the set saved by the previous query (single-step entry points may have used ctx->act since)
+        CU(cudaMemcpyAsync(ctx->act, ctx->act_seq, N, cudaMemcpyDeviceToDevice, ctx->stream));
     k_init_active<<<g, kThreads, 0, ctx->stream>>>(N, init, dJ0, dpsi, ctx->act);
     ctx->launches += 2;
     CU(cudaGetLastError());
@@ -1404,9 +1409,19 @@ int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double*
         if (cyc) { status = RD_ECYCLE; break; }
     }
     ctx->have_state = true;
+    CU(cudaMemcpyAsync(ctx->act_seq, ctx->act, N, cudaMemcpyDeviceToDevice, ctx->stream));  // what the next query inherits
     rep->n_steps = nsteps;
     rep->status = status;
     rep->total_cg_iters = total_iters;
+    for (int i = 0; i < nsteps; ++i) {
+        const int st = steps[i].status;
+        if (st != RD_OK) {
+            rep->n_inner_failed++;
+            auto sev = [](int q) { return q == RD_ENOTSPD ? 3 : q == RD_ERESID ? 2 : q == RD_ECAP ? 1 : q == RD_OK ? 0 : 4; };
+            if (sev(st) > sev(rep->worst_inner_status)) rep->worst_inner_status = st;
+        }
+        rep->n_fallbacks += steps[i].coarse_fallback ? 1 : 0;
+    }
     // u = M^{-1} K y (eq. (9), f = 0), all state values incl. the active ones
     k_apply_K<<<grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->minv, ctx->y, ctx->u);
     ctx->launches++;

@@ -71,3 +71,29 @@ def test_reference_arm_runs_on_cpu(capsys):
     d = json.loads(line)
     assert d["impl"] == "reference" and d["unit"] == "s/query" and d["higher_is_better"] is False
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["cpu_baseline"]["kind"] == "oracle"
+    assert d["cpu_baseline"]["cores"] >= 1 and "OpenMP threads" in d["cpu_baseline"]["sample"]
+
+
+def test_default_workload_is_the_largest_config():
+    # the driver runs plain `python bench.py --gpus 1 --steps K --warmup W`: that line must be on config 5
+    import argparse
+
+    ns = argparse.Namespace(pdas_cap=0, twin=None)
+    assert bench.build_parser().parse_args([]).config == 5
+
+    class W:  # noqa: N801 - stand-in with the two fields pdas_cap_for reads
+        config, pdas_cap = 2, 100
+
+    assert bench.pdas_cap_for(ns, W) == 400  # the paper's raised cap
+    W.config = 5
+    assert bench.pdas_cap_for(ns, W) == 100
+    ns.pdas_cap = 37
+    assert bench.pdas_cap_for(ns, W) == 37
+
+
+def test_query_ok_needs_outer_inner_and_kkt():
+    ok = dict(status=0, worst_inner_status=0, kkt=[1e-12] * 5)
+    assert bench.query_ok(ok)
+    assert not bench.query_ok(dict(ok, status=-7))
+    assert not bench.query_ok(dict(ok, worst_inner_status=-6))
+    assert not bench.query_ok(dict(ok, kkt=[0, 0, 0, 2e-8, 0]))

@@ -792,3 +792,30 @@ def test_transient_reference_deflates_the_twin_of_config4(oracle_mod):
     assert rj["status"] == rs["status"] == 0 and rs["rank_used"] == w.k
     assert rs["iters"] < 0.9 * rj["iters"]
     assert np.linalg.norm(xs - xj) <= 1e-5 * np.linalg.norm(xj)
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# the threaded TIMING build of the oracle (gcc -fopenmp, bench.py's cpu_baseline / --impl reference) against the plain one
+def test_threaded_timing_build_matches_the_plain_oracle():
+    import oracle
+
+    w = make_config(twin="c2_48")
+    o1 = oracle.Oracle.from_workload(w)
+    o2 = oracle.Oracle.from_workload(w, threaded=True)
+    assert o1.threads == 1 and o2.threads >= 1
+    rng = np.random.default_rng(7)
+    v = rng.standard_normal(w.N)
+    assert np.array_equal(o1.apply_K(v), o2.apply_K(v))
+    assert np.array_equal(o1.apply_KT(v), o2.apply_KT(v))  # transposed row loop: same order of the sums as the scatter
+    assert np.array_equal(o1.apply_H(v), o2.apply_H(v))
+    _, W = oracle.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, 8)
+    idx = np.flatnonzero(rng.random(w.N) > 0.3).astype(np.int64)
+    b = rng.standard_normal(len(idx))
+    x1, r1 = o1.alg1(idx, b, np.zeros(len(idx)), W[idx])
+    x2, r2 = o2.alg1(idx, b, np.zeros(len(idx)), W[idx])
+    assert r1["status"] == r2["status"] == 0 and r1["rank_used"] == r2["rank_used"]
+    assert abs(r1["iters"] - r2["iters"]) <= 2  # sums are taken in another order, nothing else differs
+    assert np.linalg.norm(x1 - x2) <= 1e-7 * np.linalg.norm(x1)
+    # alg1_on (line 2 built once by the caller) is the same solve as alg1
+    x3, r3 = o1.alg1_on(o1.coarse(idx, W[idx]), b, np.zeros(len(idx)))
+    assert np.array_equal(x1, x3) and r1["iters"] == r3["iters"]
