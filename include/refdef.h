@@ -237,6 +237,13 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
 int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* G, double* EW, double* C,
                     int32_t* rank_used, double* cond_E, int32_t* fallback);
 
+/* S7, the acceptance measures of eq. (25) for ANY pair (y, lambda), as rd_solve_query computes them for
+ * its result: with g = H y - l, l = M y_d, s = max(1, ||l||_inf),
+ *   kkt[0] = ||g + lambda||_inf / s,  kkt[1] = ||[y - psi]_+||_inf (absolute),  kkt[2] = ||[-lambda]_+||_inf / s,
+ *   kkt[3] = ||lambda .* (psi - y)||_inf / s,  kkt[4] = ||y - min(psi, y - g)||_inf / s.
+ * y_d, psi, y, lambda: N doubles, host or device (psi_i = +inf allowed).  kkt: 5 host doubles. */
+int rd_kkt(rd_ctx* ctx, const double* y_d, const double* psi, const double* y, const double* lambda, double* kkt);
+
 /* Transient variant of the coarse-mesh reference, eq. (14) (section 2.2.2; reading A21).
  * The context holds the all-at-once operator of N = N_s * nt DOFs in the layout id = space + N_s * t.  Phi: N_s x rs
  * spatial vectors, column-major, host or device (e.g. prolonged coarse vectors, or the reference of a steady

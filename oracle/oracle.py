@@ -110,6 +110,7 @@ def _load(threaded: bool = False):
     lib.orc_solve_query.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                     C.POINTER(_Options), C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.POINTER(_StepReport), C.c_void_p, C.POINTER(_QueryReport)]
+    lib.orc_kkt.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.orc_restrict.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.c_void_p]
     lib.orc_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     return lib
@@ -251,6 +252,16 @@ class Oracle:
         self._lib.orc_alg1(self._h, idx.ctypes.data, len(idx), b.ctypes.data, x.ctypes.data, zp, k, eps,
                            eps if eps_c is None else eps_c, cap, replace_period, jacobi, C.byref(rep))
         return x, {f: getattr(rep, f) for f, _ in _SolveReport._fields_}
+
+    def kkt(self, y_d, psi, y, lam):
+        """The five measures of eq. (25) for any (y, lambda); l = M y_d."""
+        ell = np.ascontiguousarray(self._m * np.asarray(y_d, dtype=np.float64))
+        psi = np.ascontiguousarray(psi, dtype=np.float64)
+        y = np.ascontiguousarray(y, dtype=np.float64)
+        lam = np.ascontiguousarray(lam, dtype=np.float64)
+        out = np.zeros(5)
+        self._lib.orc_kkt(self._h, ell.ctypes.data, psi.ctypes.data, y.ctypes.data, lam.ctypes.data, out.ctypes.data)
+        return out
 
     def alg1_on(self, cs: "CoarseSpace", b, x0, eps=1e-8, eps_c=None, cap=500000, replace_period=0, jacobi=1):
         """Algorithm 1 on a coarse space that line 2 has already built (self.coarse(idx, Zt)): the same solve as alg1

@@ -695,6 +695,44 @@ static uint64_t fnv1a_bits(const uint8_t *flags, int64_t N, uint8_t *packed /* c
     return hsh;
 }
 
+/* O4: the five acceptance measures of eq. (25) for any pair (y, lambda):
+ *   g = H y - l,  s = max(1, ||l||_inf)
+ *   kkt[0] = ||g + lambda||_inf / s              stationarity
+ *   kkt[1] = ||[y - psi]_+||_inf                 primal feasibility ("The primal-feasibility quantity is absolute")
+ *   kkt[2] = ||[-lambda]_+||_inf / s             dual feasibility
+ *   kkt[3] = ||lambda .* (psi - y)||_inf / s     complementarity
+ *   kkt[4] = ||y - min(psi, y - g)||_inf / s     projected gradient
+ * psi_i = +inf contributes 0 to [1], [3] and y_i - min(inf, y_i - g_i) = g_i to [4].  ell = M y_d, length N. */
+void orc_kkt(orc_ctx *c, const double *ell, const double *psi, const double *y, const double *lambda, double *kkt)
+{
+    int64_t N = c->N;
+    double *Hy = (double *)malloc((size_t)N * sizeof(double));
+    orc_apply_H(c, y, Hy);
+    double s = 1.0, k0 = 0, k1 = 0, k2 = 0, k3 = 0, k4 = 0;
+    for (int64_t i = 0; i < N; i++) if (fabs(ell[i]) > s) s = fabs(ell[i]);
+    for (int64_t i = 0; i < N; i++) {
+        double g = Hy[i] - ell[i];
+        double v0 = fabs(g + lambda[i]);
+        double v2 = (lambda[i] < 0.0) ? -lambda[i] : 0.0;
+        double v1 = 0.0, v3 = 0.0, v4;
+        if (isinf(psi[i])) {
+            v4 = fabs(g); /* y - min(inf, y - g) = g */
+        } else {
+            v1 = (y[i] > psi[i]) ? y[i] - psi[i] : 0.0;
+            v3 = fabs(lambda[i] * (psi[i] - y[i]));
+            double mn = (psi[i] < y[i] - g) ? psi[i] : (y[i] - g);
+            v4 = fabs(y[i] - mn);
+        }
+        if (v0 > k0) k0 = v0;
+        if (v1 > k1) k1 = v1;
+        if (v2 > k2) k2 = v2;
+        if (v3 > k3) k3 = v3;
+        if (v4 > k4) k4 = v4;
+    }
+    kkt[0] = k0 / s; kkt[1] = k1; kkt[2] = k2 / s; kkt[3] = k3 / s; kkt[4] = k4 / s;
+    free(Hy);
+}
+
 /* One optimisation query: PDAS (eq. (7)-(8); Alg. 2 steps 9-15, :392-398),
  * control recovery (eq. (9), :121) and the KKT measures (eq. (25), :343-346).
  * W: full-domain reference, N x k column-major (may be NULL for Jacobi-CG).
@@ -803,30 +841,7 @@ int orc_solve_query(orc_ctx *c, int method, const double *y_d, const double *psi
     orc_apply_K(c, y, tmp);
     for (int64_t i = 0; i < N; i++) u[i] = tmp[i] / c->m[i];
 
-    /* KKT measures, eq. (25): g = H y - l, s = max(1, ||l||_inf) */
-    orc_apply_H(c, y, Hy);
-    double s = 1.0, k0 = 0, k1 = 0, k2 = 0, k3 = 0, k4 = 0;
-    for (int64_t i = 0; i < N; i++) if (fabs(ell[i]) > s) s = fabs(ell[i]);
-    for (int64_t i = 0; i < N; i++) {
-        double g = Hy[i] - ell[i];
-        double v0 = fabs(g + lambda[i]);
-        double v2 = (lambda[i] < 0.0) ? -lambda[i] : 0.0;
-        double v1 = 0.0, v3 = 0.0, v4;
-        if (isinf(psi[i])) {
-            v4 = fabs(g); /* y - min(inf, y - g) = g */
-        } else {
-            v1 = (y[i] > psi[i]) ? y[i] - psi[i] : 0.0;
-            v3 = fabs(lambda[i] * (psi[i] - y[i]));
-            double mn = (psi[i] < y[i] - g) ? psi[i] : (y[i] - g);
-            v4 = fabs(y[i] - mn);
-        }
-        if (v0 > k0) k0 = v0;
-        if (v1 > k1) k1 = v1;
-        if (v2 > k2) k2 = v2;
-        if (v3 > k3) k3 = v3;
-        if (v4 > k4) k4 = v4;
-    }
-    rep->kkt[0] = k0 / s; rep->kkt[1] = k1; rep->kkt[2] = k2 / s; rep->kkt[3] = k3 / s; rep->kkt[4] = k4 / s;
+    orc_kkt(c, ell, psi, y, lambda, rep->kkt);
 
     free(J); free(Jn); free(ell); free(tmp); free(Hy); free(idx); free(b); free(x); free(seen);
     return status;

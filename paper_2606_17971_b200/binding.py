@@ -23,7 +23,7 @@ SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
            "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
-           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction"]
+           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt"]
 
 
 class RefDefError(RuntimeError):
@@ -117,6 +117,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_solve_inactive.argtypes = [vp, i32, vp, vp, vp, C.POINTER(_SolveReport)]
     lib.rd_coarse_setup.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl), C.POINTER(i32)]
     lib.rd_energy_fraction.argtypes = [vp, i32, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
+    lib.rd_kkt.argtypes = [vp, vp, vp, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -357,6 +358,12 @@ class RefDef:
         self._check(self._lib.rd_energy_fraction(self._h, method, _ptr(active), _ptr(b), _ptr(x_star), C.byref(chi),
                                                  C.byref(qb), C.byref(xs)), "rd_energy_fraction")
         return chi.value, qb.value, xs.value
+
+    def kkt(self, y_d, psi, y, lam):
+        """The five measures of eq. (25) for any (y, lambda)."""
+        out = (C.c_double * 5)()
+        self._check(self._lib.rd_kkt(self._h, _ptr(y_d), _ptr(psi), _ptr(y), _ptr(lam), out), "rd_kkt")
+        return np.array(list(out))
 
     # ---- the query
     def solve_query(self, method, y_d, psi, J0=None, y=None, u=None, lam=None, want_sets=True):

@@ -1311,6 +1311,31 @@ int rd_energy_fraction(rd_ctx* ctx, int32_t method, const uint8_t* active, const
     return RD_OK;
 }
 
+int rd_kkt(rd_ctx* ctx, const double* y_d, const double* psi, const double* y, const double* lambda, double* kkt)
+{
+    if (!ctx || !y_d || !psi || !y || !lambda || !kkt) return RD_EINVAL;
+    const int64_t N = ctx->N;
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    const double *dyd, *dpsi, *dy, *dl;
+    RDTRY(in_dev(ctx, y_d, N, ctx->in0, &dyd));
+    k_ell<<<g, kThreads, 0, ctx->stream>>>(N, ctx->m, dyd, ctx->ell);
+    RDTRY(in_dev(ctx, psi, N, ctx->in1, &dpsi));
+    RDTRY(in_dev(ctx, y, N, ctx->in0, &dy));       // in0 is free again: l has been formed (same stream)
+    RDTRY(in_dev(ctx, lambda, N, ctx->tmp, &dl));
+    RDTRY(launch_apply_H(ctx, dy, nullptr, ctx->Hy));
+    CU(cudaMemsetAsync(ctx->d_cnt, 0, sizeof(PdasCounters), ctx->stream));
+    k_kkt<<<g, kThreads, 0, ctx->stream>>>(N, ctx->ell, ctx->Hy, dy, dpsi, dl, ctx->d_cnt);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(PdasCounters), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    double kk[6];
+    memcpy(kk, ctx->h_cnt->kkt_bits, sizeof kk);
+    const double s = std::max(1.0, kk[5]);
+    kkt[0] = kk[0] / s; kkt[1] = kk[1]; kkt[2] = kk[2] / s; kkt[3] = kk[3] / s; kkt[4] = kk[4] / s;
+    return RD_OK;
+}
+
 int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double* psi, const uint8_t* J0, double* y, double* u,
                    double* lambda, rd_step_report* steps, uint8_t* J_bits, rd_query_report* rep)
 {
