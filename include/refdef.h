@@ -76,9 +76,10 @@ typedef struct {
     int32_t c_is_diag;     /* eq. (8): c_i = H_ii (1) or c = 1 (0, BASELINE.json configs) */
     int32_t init;          /* rd_init */
     int32_t alg1_variant;  /* 0: projection carried in coefficient form, one pass over H_II W_I per iteration, operands
-                              staged through shared memory by TMA bulk copies (default);
-                              1: the literal recurrence of Alg. 1 (passes over H_II W_I and W_I), register-staged;
-                              2: coefficient form, register-staged.  Same method, same results up to rounding */
+                              staged through shared memory by TMA bulk copies, work restricted to the 32-row slices that
+                              hold inactive rows (default);
+                              1: the literal recurrence of Alg. 1 (passes over H_II W_I and W_I), register-staged, all
+                              rows visited and masked.  Same method, same results up to rounding */
 } rd_options;
 
 /* One PDAS step (one inactive system).  Times are milliseconds measured with CUDA events on the stream. */
@@ -121,6 +122,8 @@ typedef struct {
                               [2] stage B (K^T product)  [3] grid barrier + reduction  [4] k x k coefficient updates
                               [5] stage C (updates + H_II W_I pass)  [6] grid barrier + reduction  [7] outside the loop;
                               zeros for the other variants */
+    int32_t live_slices_A, live_slices_B; /* S6 compaction: 32-row slices the K product / the K^T product, vector updates
+                              and tall-skinny pass of this solve touch (of ceil(N/32)); all others are skipped */
 } rd_solve_report;
 
 void rd_default_options(rd_options* opt);

@@ -54,7 +54,7 @@ class _SolveReport(C.Structure):
     _fields_ = [("iters", C.c_int32), ("rank_used", C.c_int32), ("coarse_fallback", C.c_int32),
                 ("replacements", C.c_int32), ("status", C.c_int32), ("rel_resid_verified", C.c_double),
                 ("cond_E", C.c_double), ("t_iter_ms", C.c_double), ("bytes_per_iter", C.c_double),
-                ("t_stage_us", C.c_double * 8)]
+                ("t_stage_us", C.c_double * 8), ("live_slices_A", C.c_int32), ("live_slices_B", C.c_int32)]
 
 
 @dataclass

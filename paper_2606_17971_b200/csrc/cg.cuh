@@ -40,8 +40,11 @@ struct CgParams {
     double *x, *r, *p0, *p1, *z, *w, *t;
     const double *Wm, *HWm;  // chi_I W and chi_I H chi_I W, N x kp column-major (ld = ldw)
     const double* HWt;       // HWm tile-major: (i, j) at (i / 32) * 32 kp + 32 j + i % 32 (k_alg1_v3)
+    const double* Wt;        // Wm tile-major, same layout (k_alg1_v3: coarse corrections outside the loop)
+    const int32_t *listA, *listB;  // S6 compaction: live 32-row slices of the current active set (pdas.cuh k_slice_lists)
+    const int32_t* live_counts;    // [0] = |listA|, [1] = |listB|
     const double* C;         // kp x kp column-major
-    const double* EW;        // W_I^T H_II W_I, kp x kp column-major (k_alg1_v2)
+    const double* EW;        // W_I^T H_II W_I, kp x kp column-major (k_alg1_v3: curvature in coefficient form)
     double eps, eps_c;
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]

@@ -1,21 +1,42 @@
-// cg3.cuh -- k_alg1_v3: Algorithm 1 in the coefficient form of cg2.cuh, with every streamed
-// operand staged through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier, async.cuh) instead of
-// register loads.  Default kernel of the library (rd_options.alg1_variant = 0).
+// cg3.cuh -- k_alg1_v3: Algorithm 1 with the projection carried in coefficient form, every
+// streamed operand staged through shared memory by 1-D TMA bulk copies (cp.async.bulk + mbarrier, async.cuh), and all
+// work restricted to the live 32-row slices of the current active set (S6 compaction, pdas.cuh).  Default kernel of the
+// library (rd_options.alg1_variant = 0); cg.cuh keeps the literal two-pass recurrence as variant 1.
 //
-// Why: the loop is HBM-bound (DESIGN.md bytes model) and a register-staged kernel at 64 registers per thread
-// cannot keep enough bytes in flight: every 32-row tile of the HW_I pass waited on its own loads.  Here
-//   stage C  the n x kp block HW_I streams through a ring of NST = min(32, 512/kp) tiles of 32 rows x kp columns
-//            (256 kp bytes each, 128 KB in total); consumer warp cw owns ring slot cw and its mbarrier, processes
-//            tiles cw, cw + NST, ... and refills its slot as soon as its lanes have read it.  A tile is consumed
-//            by ONE warp in two passes over shared memory: lane = row for q_i = sum_j HW_ij (a nu_j) and the
-//            row updates, then lane = column for c_j += sum_i HW_ij z~_i, rows visited in a skewed order
-//            (i + lane) mod 32 so that the transposed reads are bank-conflict free.  No cross-warp exchange.
-//   stage A/B the sliced-ELL streams of K and K^T: every warp prefetches the values and column indices of its
-//            next 32-row slice into its own 4 KB slot while it gathers for the current one.
-// The arithmetic per row and all reduction orders are fixed, so results are bit-reproducible run to run.
+// ---- coefficient form.  Write the search direction and the iterate of Alg. 1 as  p = p~ - W_I nu,  x = x~ - W_I xi  with
+// k-vectors nu, xi kept (replicated, bit-identical) in the shared memory of every CTA.  With z~ = J r (never projected):
+//   line 22  z = P J r = z~ - W_I mu,  mu = C c,  c = (HW_I)^T z~                       (eq. (18))
+//   line 23  p = z + beta p      <=>  p~ = z~ + beta p~,   nu = mu + beta nu
+//   line  9  w = B p = w~ - HW_I nu  with w~ = B p~  (the two SpMVs act on p~ only)
+//            p^T w = p~^T w~ - 2 nu^T g + nu^T E_W nu,   g = (HW_I)^T p~ = c + beta g,   E_W = W_I^T HW_I
+//   line 10  x~ += a p~, xi += a nu;   r = r - a w~ + HW_I (a nu)
+//   line 22  rho = r^T z = r^T z~ - s^T mu,   s = W_I^T r = s - a (g - E_W nu)   (zero in exact arithmetic,
+//            Z^T(b - B x_c) = 0 and Z^T B P = 0; the recurrence carries its rounding-level drift)
+// One pass over a 32-row tile of HW_I does both  q_i = sum_j HW_ij (a nu_j)  (needed for r_i) and
+// c_j += HW_ij z~_i.  x is made explicit (x = x~ - W_I xi, one pass over W_I) only where Alg. 1 recomputes the
+// residual (lines 12, 16, Verify).  ONE pass over the cached product HW_I per iteration instead of a pass over HW_I
+// and a pass over W_I.
+//
+// ---- stages of one iteration (grid barrier after each):
+//   A  p~ = z~ + beta p~ (fused into the gather),  t = M^{-1} K p~           over listA, this CTA's share    S3
+//   B  w~ = chi_I (m.p~ + sigma K^T t),  p~^T w~                             over listB, this CTA's share    S3
+//   C  x~, r, z~ updates, ||r||^2, r^T z~, c = (HW_I)^T z~   (one pass over HW_I, tile-major, through the ring)  S4 + S5
+// Each stage splits ITS list evenly over the CTAs (listA and listB differ only near the boundary of the inactive
+// set), so a PDAS step with |I| << N streams |I|-proportional bytes and stays balanced.  The k x k recurrences
+// between C and A are spread over all 32 warps (two block barriers).
+//
+// ---- staging.  Stage C: the n x kp block streams through a ring of NST = min(32, 512/kp) tiles of 32 rows x kp
+// columns (256 kp bytes each, 128 KB in total); consumer warp cw owns ring slot cw and its mbarrier, processes the
+// tiles cw, cw + NST, ... of this CTA's share and refills its slot as soon as its lanes have read it.  A tile is
+// consumed by ONE warp in two passes over shared memory: lane = row for q_i and the row updates, then lane = column
+// for c_j, rows visited in the skewed order (i + lane) mod 32 so that the transposed reads are bank-conflict free.
+// Stages A/B: every warp prefetches the values and column indices of its next slice into its own 4 KB slot while it
+// gathers for the current one.  Write-after-read on a slot (generic-proxy loads, then an async-proxy refill) is
+// ordered by refill_fence() (async.cuh).  The arithmetic per row and all reduction orders are fixed by the lists and
+// the grid size, so results are bit-reproducible run to run.
 #pragma once
 #include "async.cuh"
-#include "cg2.cuh"
+#include "cg.cuh"
 
 namespace rd {
 
@@ -24,14 +45,12 @@ namespace rd {
 #define RD_SPMV_SLOT_BYTES 4096  // per warp: values 8 x 256 B, then indices 8 x 128 B
 
 struct __align__(128) Cg3Shared {
-    double C[RD_MAX_K * RD_MAX_K];
-    double EW[RD_MAX_K * RD_MAX_K];
-    double s[RD_CG_THREADS];  // transposition buffer of stage_recompute (outside the loop)
-    double zb[32][32];        // stage C: z~ of the warp's tile, for the transposed pass
-    double cpart[512];        // stage C: c partials of the consumer warps, NST x kp <= 512
-    double c[RD_MAX_K], mu[RD_MAX_K], nu[RD_MAX_K], g[RD_MAX_K], sv[RD_MAX_K], xi[RD_MAX_K], anu[RD_MAX_K], e[RD_MAX_K];
+    double C[RD_MAX_K * RD_MAX_K];   // T E^{-1} T^T, symmetric
+    double EW[RD_MAX_K * RD_MAX_K];  // W_I^T H_II W_I, symmetrised on load
+    double zb[32][32];               // tile streams: the per-row multiplier of the warp's tile, for the transposed pass
+    double cpart[512];               // tile streams: c partials of the consumer warps, NST x kp <= 512
+    double c[RD_MAX_K], mu[RD_MAX_K], nu[2][RD_MAX_K], g[2][RD_MAX_K], sv[RD_MAX_K], xi[RD_MAX_K], anu[RD_MAX_K], e[RD_MAX_K];
     double scal[SL_NSCAL];
-    double small[4];
     double red[32];
     uint64_t full[32];  // one mbarrier per warp
     uint64_t tacc[8];
@@ -39,13 +58,26 @@ struct __align__(128) Cg3Shared {
     __align__(128) unsigned char ring[RD_RING_BYTES];  // written by the async proxy only
 };
 
+enum { TS_UPDATE = 0, TS_RECOMP_Z = 1, TS_RECOMP_R = 2, TS_ADDW = 3 };
 
-struct Cg3Cta : Cg2CtaT<Cg3Shared> {
-    using Base = Cg2CtaT<Cg3Shared>;
-    uint32_t ph;  // phase parity of this warp's mbarrier (uniform in the warp)
+struct Cg3Cta {
+    const CgParams& P;
+    Cg3Shared& sh;
+    int64_t a0, a1, b0, b1;  // this CTA's shares of listA / listB (index ranges)
+    unsigned int nbar;
+    int G;
+    uint32_t ph;    // phase parity of this warp's mbarrier (uniform in the warp)
+    int par;        // which copy of nu / g is current
+    double ng, ne;  // nu^T g, nu^T E_W nu of the current direction (every thread holds them)
 
-    __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : Base(p, s), ph(0)
+    __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : P(p), sh(s), nbar(0), ph(0), par(0), ng(0.0), ne(0.0)
     {
+        G = gridDim.x;
+        const int64_t nA = P.live_counts[0], nB = P.live_counts[1];
+        a0 = (int64_t)blockIdx.x * nA / G;
+        a1 = (int64_t)(blockIdx.x + 1) * nA / G;
+        b0 = (int64_t)blockIdx.x * nB / G;
+        b1 = (int64_t)(blockIdx.x + 1) * nB / G;
         if (threadIdx.x == 0) {
             for (int w = 0; w < 32; ++w) mbar_init(&sh.full[w], 1);
             mbar_fence_init();
@@ -55,11 +87,16 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         __syncthreads();
     }
 
-    __device__ void tick(int slot)
+    __device__ double* slot(int sl) const { return P.partial + ((size_t)(nbar & 1u) * SL_NSLOT + sl) * G; }
+    __device__ void put(int sl, double v) const
+    {
+        if (threadIdx.x == 0) slot(sl)[blockIdx.x] = v;
+    }
+    __device__ void tick(int slot_)
     {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             const uint64_t t = global_timer_ns();
-            sh.tacc[slot] += t - sh.tlast;
+            sh.tacc[slot_] += t - sh.tlast;
             sh.tlast = t;
         }
     }
@@ -82,16 +119,16 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         const int nsl = want_c ? SL_NSCAL + P.kp : SL_NSCAL;
         const int sl = threadIdx.x >> 3, sub = threadIdx.x & 7;
         if ((sl & ~3) < nsl) {  // warp-uniform: some slot of this warp is live
-            double a0 = 0.0, a1 = 0.0;
+            double a0_ = 0.0, a1_ = 0.0;
             if (sl < nsl) {
                 const double* q = base + (size_t)sl * G;
 #pragma unroll 4
                 for (int i = sub; i < G; i += 16) {
-                    a0 += __ldcg(q + i);
-                    if (i + 8 < G) a1 += __ldcg(q + i + 8);
+                    a0_ += __ldcg(q + i);
+                    if (i + 8 < G) a1_ += __ldcg(q + i + 8);
                 }
             }
-            double a = a0 + a1;
+            double a = a0_ + a1_;
             a += __shfl_xor_sync(0xffffffffu, a, 4);
             a += __shfl_xor_sync(0xffffffffu, a, 2);
             a += __shfl_xor_sync(0xffffffffu, a, 1);
@@ -102,66 +139,79 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         __syncthreads();
     }
 
-    // ---- k x k coefficient recurrences (cg2.cuh header), done by warp 0 alone: lane owns rows lane and lane + 32
-    // of the kp x kp matrices (column-major: conflict-free), vectors are broadcast reads.  One __syncthreads.
-    __device__ __forceinline__ void matvec_w0(const double* M, const double* v, int kp, int lane, double& o0, double& o1)
+    // ---- k x k part, all 32 warps.  Matrices are symmetric and column-major: row i is read as column i (contiguous,
+    // conflict-free); warp w owns rows w and w + 32, lane j owns entries j and j + 32 of the vectors.
+    __device__ __forceinline__ double row_dot(const double* M, int i, int kp, int lane, double v0, double v1)
     {
-        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-        const bool r0 = lane < kp, r1 = lane + 32 < kp;
-        const double* m0 = M + (r0 ? lane : 0);
-        const double* m1 = M + (r1 ? lane + 32 : 0);
-        for (int j = 0; j < kp; j += 2) {
-            const double v0 = v[j], v1 = v[j + 1];
-            a0 = fma(m0[(size_t)j * kp], v0, a0);
-            b0 = fma(m0[(size_t)(j + 1) * kp], v1, b0);
-            a1 = fma(m1[(size_t)j * kp], v0, a1);
-            b1 = fma(m1[(size_t)(j + 1) * kp], v1, b1);
-        }
-        o0 = r0 ? a0 + b0 : 0.0;
-        o1 = r1 ? a1 + b1 : 0.0;
+        double a = (lane < kp) ? M[lane + (size_t)i * kp] * v0 : 0.0;
+        if (lane + 32 < kp) a = fma(M[lane + 32 + (size_t)i * kp], v1, a);
+        return warp_sum(a);
     }
-    // lines 7 / 20 / 22-23 and the curvature terms of line 9 that do not need p~^T w~:
+    // mu = C c  (the coarse solve of eq. (18) in W_I coordinates; lines 3 and 16)
+    __device__ void coarse_solve()
+    {
+        const int kp = P.kp, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const double c0 = (lane < kp) ? sh.c[lane] : 0.0, c1 = (lane + 32 < kp) ? sh.c[lane + 32] : 0.0;
+        for (int i = warp; i < kp; i += 32) {
+            const double a = row_dot(sh.C, i, kp, lane, c0, c1);
+            if (lane == 0) sh.mu[i] = a;
+        }
+        __syncthreads();
+    }
+    // lines 7 / 20 / 22-23 in coefficients and the curvature terms of line 9 that do not need p~^T w~:
     //   mu = C c, rho = r^T z~ - s^T mu, beta, nu = mu + beta nu, g = c + beta g, e = E_W nu, nu^T g, nu^T e
     __device__ void coef_direction(bool restart, double rho_prime, double& rho, double& beta)
     {
-        const int kp = P.kp;
-        if (threadIdx.x < 32) {
-            const int lane = threadIdx.x;
-            const bool r0 = lane < kp, r1 = lane + 32 < kp;
-            double mu0, mu1;
-            matvec_w0(sh.C, sh.c, kp, lane, mu0, mu1);
-            const double s0_ = (restart || !r0) ? 0.0 : sh.sv[lane], s1_ = (restart || !r1) ? 0.0 : sh.sv[lane + 32];
-            const double smu = warp_sum(fma(s0_, mu0, s1_ * mu1));
-            const double rho_new = rho_prime - smu;
-            const double bt = restart ? 0.0 : rho_new / rho;
-            double nu0 = 0.0, nu1 = 0.0, g0 = 0.0, g1 = 0.0;
-            if (r0) { nu0 = fma(bt, sh.nu[lane], mu0); g0 = fma(bt, sh.g[lane], sh.c[lane]); sh.nu[lane] = nu0; sh.g[lane] = g0; sh.mu[lane] = mu0; if (restart) sh.sv[lane] = 0.0; }
-            if (r1) { nu1 = fma(bt, sh.nu[lane + 32], mu1); g1 = fma(bt, sh.g[lane + 32], sh.c[lane + 32]); sh.nu[lane + 32] = nu1; sh.g[lane + 32] = g1; sh.mu[lane + 32] = mu1; if (restart) sh.sv[lane + 32] = 0.0; }
-            __syncwarp();
-            double e0, e1;
-            matvec_w0(sh.EW, sh.nu, kp, lane, e0, e1);
-            if (r0) sh.e[lane] = e0;
-            if (r1) sh.e[lane + 32] = e1;
-            const double ng = warp_sum(fma(nu0, g0, nu1 * g1));
-            const double ne = warp_sum(fma(nu0, e0, nu1 * e1));
-            if (lane == 0) { sh.small[0] = rho_new; sh.small[1] = bt; sh.small[2] = ng; sh.small[3] = ne; }
+        const int kp = P.kp, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const bool r0 = lane < kp, r1 = lane + 32 < kp;
+        const double c0 = r0 ? sh.c[lane] : 0.0, c1 = r1 ? sh.c[lane + 32] : 0.0;
+        for (int i = warp; i < kp; i += 32) {
+            const double a = row_dot(sh.C, i, kp, lane, c0, c1);
+            if (lane == 0) sh.mu[i] = a;
         }
         __syncthreads();
-        rho = sh.small[0];
-        beta = sh.small[1];
+        // every warp forms the new nu, g in registers (same order everywhere: bit-identical)
+        const double* nu_o = sh.nu[par];
+        const double* g_o = sh.g[par];
+        const double mu0 = r0 ? sh.mu[lane] : 0.0, mu1 = r1 ? sh.mu[lane + 32] : 0.0;
+        const double s0_ = (restart || !r0) ? 0.0 : sh.sv[lane], s1_ = (restart || !r1) ? 0.0 : sh.sv[lane + 32];
+        const double smu = warp_sum(fma(s0_, mu0, s1_ * mu1));
+        const double rho_new = rho_prime - smu;
+        const double bt = restart ? 0.0 : rho_new / rho;
+        const double nu0 = r0 ? fma(bt, nu_o[lane], mu0) : 0.0, nu1 = r1 ? fma(bt, nu_o[lane + 32], mu1) : 0.0;
+        const double g0 = r0 ? fma(bt, g_o[lane], c0) : 0.0, g1 = r1 ? fma(bt, g_o[lane + 32], c1) : 0.0;
+        for (int i = warp; i < kp; i += 32) {
+            const double a = row_dot(sh.EW, i, kp, lane, nu0, nu1);
+            if (lane == 0) sh.e[i] = a;
+        }
+        if (warp == 0) {  // the other copy of nu / g: nobody reads it before the barrier below
+            double* nu_n = sh.nu[par ^ 1];
+            double* g_n = sh.g[par ^ 1];
+            if (r0) { nu_n[lane] = nu0; g_n[lane] = g0; if (restart) sh.sv[lane] = 0.0; }
+            if (r1) { nu_n[lane + 32] = nu1; g_n[lane + 32] = g1; if (restart) sh.sv[lane + 32] = 0.0; }
+        }
+        __syncthreads();
+        par ^= 1;
+        const double e0 = r0 ? sh.e[lane] : 0.0, e1 = r1 ? sh.e[lane + 32] : 0.0;
+        ng = warp_sum(fma(nu0, g0, nu1 * g1));
+        ne = warp_sum(fma(nu0, e0, nu1 * e1));
+        rho = rho_new;
+        beta = bt;
     }
-    __device__ double coef_curvature(double pw) { return pw - 2.0 * sh.small[2] + sh.small[3]; }
-    // line 10 in coefficients; the __syncthreads that opens stage_update_coarse publishes anu
+    __device__ double coef_curvature(double pw) const { return pw - 2.0 * ng + ne; }  // p^T B p
+    // line 10 in coefficients; the __syncthreads that opens the tile stream publishes anu
     __device__ void coef_step(double a)
     {
         if ((int)threadIdx.x < P.kp) {
             const int j = threadIdx.x;
-            sh.sv[j] = fma(-a, sh.g[j] - sh.e[j], sh.sv[j]);
-            sh.anu[j] = a * sh.nu[j];
-            sh.xi[j] = fma(a, sh.nu[j], sh.xi[j]);
+            const double nuj = sh.nu[par][j];
+            sh.sv[j] = fma(-a, sh.g[par][j] - sh.e[j], sh.sv[j]);
+            sh.anu[j] = a * nuj;
+            sh.xi[j] = fma(a, nuj, sh.xi[j]);
         }
     }
 
+    // ================================================================== stages A / B: staged sliced-ELL products
     // values and column indices of one 32-row slice (wd entries per row) into this warp's slot
     __device__ __forceinline__ void issue_slice(const Ell& A, int64_t o, int wd)
     {
@@ -170,15 +220,13 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             uint64_t* bar = &sh.full[threadIdx.x >> 5];
             mbar_arrive_expect_tx(bar, (uint32_t)wd * 384u);
             if (wd > 0) {
-                {
-                    bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
-                    bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
-                }
+                bulk_g2s(slot_, A.val + o, (uint32_t)wd * 256u, bar);
+                bulk_g2s(slot_ + RD_SPMV_WD * 256, A.col + o, (uint32_t)wd * 128u, bar);
             }
         }
     }
     // sum_e A[row,e] vin[col_e] for this lane's row of the slice staged in (sval, scol); WDC = register budget
-    // (entries per row).  All gathers are issued before the first use; `next` refills the slot in between.
+    // (entries per row).  The slot is read into registers, then refilled (`next`), then the gathers go out.
     template <bool COMBINE, int WDC, class Next>
     __device__ __forceinline__ double staged_row_dot(const double* sval, const int32_t* scol, int wd, int lane,
                                                      const double* v0, const double* v1, double beta, Next next)
@@ -191,9 +239,8 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             cc[q] = ok ? scol[q * 32 + lane] : 0;
             aa[q] = ok ? sval[q * 32 + lane] : 0.0;
         }
-        // The refill below is an async-proxy write into the slot just read through the generic proxy (a bulk copy
-        // issued right after the loads can otherwise land before they have executed: seen on config 5 in round 1).
-        // refill_fence = __syncwarp + fence.proxy.async.shared::cta orders the two (async.cuh).
+        // The refill is an async-proxy write into the slot just read through the generic proxy (a bulk copy issued
+        // right after the loads can otherwise land before they have executed: seen on config 5 in round 1).
         refill_fence();
         next();
 #pragma unroll
@@ -210,11 +257,12 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         return acc;
     }
 
-    // ---- staged sliced-ELL product over this CTA's slices.  pre(row) loads what the epilogue needs of the row
-    // (issued before the wait on the slice, so it never adds a round trip); epi(row, acc, pre(row)) consumes
-    // sum_e A[row,e] vin[col_e].  A matrix of uniform slice width needs no extent lookups (Ell::uwd).
-    template <bool COMBINE, class Pre, class Epi>
-    __device__ __forceinline__ void spmv_staged(const Ell& A, const double* v0, const double* v1, double beta, Pre pre, Epi epi)
+    // Staged product over the list entries [i0, i1) of `list` (SHIFT = 1: entries carry a flag in bit 0).
+    // pre(row, flag) loads what the epilogue needs of the row (issued before the wait on the slice, so it never adds a
+    // round trip); epi(row, flag, acc, pre(row)) consumes sum_e A[row,e] vin[col_e].
+    template <bool COMBINE, int SHIFT, class Pre, class Epi>
+    __device__ __forceinline__ void spmv_staged(const Ell& A, const int32_t* list, int64_t i0, int64_t i1, const double* v0,
+                                                const double* v1, double beta, Pre pre, Epi epi)
     {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         unsigned char* slot_ = sh.ring + warp * RD_SPMV_SLOT_BYTES;
@@ -226,22 +274,27 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             if (uwd >= 0) { o = s * 32 * uwd; wd = uwd; }
             else { o = A.off[s]; wd = (int)((A.off[s + 1] - o) >> 5); }
         };
-        int64_t s = s0 + warp;
+        int64_t i = i0 + warp;
+        int32_t ecur = (i < i1) ? __ldg(list + i) : 0;
+        int32_t enxt = (i + 32 < i1) ? __ldg(list + i + 32) : 0;
         int wd = 0;
-        refill_fence();  // the ring was last read (generic proxy) by the previous stage, possibly by another warp, before a CTA barrier
-        if (s < s1) {
+        refill_fence();  // the ring was last read (generic proxy) by the previous stage, before a CTA barrier
+        if (i < i1) {
             int64_t o;
-            extent(s, o, wd);
+            extent((int64_t)(ecur >> SHIFT), o, wd);
             if (wd <= RD_SPMV_WD) issue_slice(A, o, wd);
         }
-        for (; s < s1; s += 32) {
-            const int64_t sn = s + 32;
+        for (; i < i1; i += 32) {
+            const int64_t in = i + 32;
+            const int32_t enn = (in + 32 < i1) ? __ldg(list + in + 32) : 0;  // two ahead: its latency hides behind this slice
+            const int64_t s = (int64_t)(ecur >> SHIFT), sn = (int64_t)(enxt >> SHIFT);
+            const int flag = SHIFT ? (ecur & 1) : 1;
             int64_t on = 0;
             int wdn = 0;
-            if (sn < s1) extent(sn, on, wdn);
+            if (in < i1) extent(sn, on, wdn);
             const int64_t row = s * RD_SLICE + lane;
-            auto rowdata = pre(row);
-            auto next = [&]() { if (sn < s1 && wdn <= RD_SPMV_WD) issue_slice(A, on, wdn); };
+            auto rowdata = pre(row, flag);
+            auto next = [&]() { if (in < i1 && wdn <= RD_SPMV_WD) issue_slice(A, on, wdn); };
             double acc;
             if (wd <= RD_SPMV_WD) {
                 mbar_wait(bar, ph);
@@ -253,42 +306,45 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
                 next();
                 acc = ell_row_dot<COMBINE>(A, s, lane, v0, v1, beta);
             }
-            epi(row, acc, rowdata);
+            epi(row, flag, acc, rowdata);
             wd = wdn;
+            ecur = enxt;
+            enxt = enn;
         }
     }
 
     struct RowK { double minv, x; };
     struct RowKT { double v, m; bool act; };
 
-    // stage A: t = M^{-1} K (v0 + beta v1), pnew = v0 + beta v1 on this CTA's rows  (Alg. 1 lines 23 + 9)
+    // stage A: t = M^{-1} K (v0 + beta v1) on the rows of listA; pnew = v0 + beta v1 on those that hold inactive rows
+    // (elsewhere p~ is identically zero and stays so)                                       (Alg. 1 lines 23 + 9)
     template <bool COMBINE>
     __device__ void opK(const double* v0, const double* v1, double beta, double* pnew)
     {
         const int64_t N = P.N;
         const double* minv = P.minv;
         double* t = P.t;
-        spmv_staged<COMBINE>(
-            P.K, v0, v1, beta,
-            [&](int64_t row) {
+        spmv_staged<COMBINE, 1>(
+            P.K, P.listA, a0, a1, v0, v1, beta,
+            [&](int64_t row, int flag) {
                 RowK r{0.0, 0.0};
                 if (row < N) {
                     r.minv = ldg_f64(minv + row);
-                    if (pnew) {
+                    if (pnew && flag) {
                         r.x = v0[row];
                         if (COMBINE) r.x = fma(beta, v1[row], r.x);
                     }
                 }
                 return r;
             },
-            [&](int64_t row, double acc, const RowK& r) {
+            [&](int64_t row, int flag, double acc, const RowK& r) {
                 if (row < N) {
                     t[row] = acc * r.minv;
-                    if (pnew) pnew[row] = r.x;
+                    if (pnew && flag) pnew[row] = r.x;
                 }
             });
     }
-    // stage B: w = chi_I (m.v + sigma K^T t); returns this thread's partial of v^T w  (Alg. 1 line 9)
+    // stage B: w = chi_I (m.v + sigma K^T t) on the rows of listB; returns this thread's partial of v^T w  (line 9)
     __device__ double opKT(const double* v)
     {
         const int64_t N = P.N;
@@ -297,9 +353,9 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         const double sigma = P.sigma;
         double* w = P.w;
         double dot = 0.0;
-        spmv_staged<false>(
-            P.KT, P.t, nullptr, 0.0,
-            [&](int64_t row) {
+        spmv_staged<false, 0>(
+            P.KT, P.listB, b0, b1, P.t, nullptr, 0.0,
+            [&](int64_t row, int) {
                 RowKT r{0.0, 0.0, false};
                 if (row < N) {
                     r.v = v[row];
@@ -308,7 +364,7 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
                 }
                 return r;
             },
-            [&](int64_t row, double acc, const RowKT& r) {
+            [&](int64_t row, int, double acc, const RowKT& r) {
                 if (row < N) {
                     double wi = fma(sigma, acc, r.m * r.v);
                     if (r.act) wi = 0.0;
@@ -319,31 +375,49 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         return dot;
     }
 
-    // Stage C without a coarse space (rank-zero execution = Jacobi-CG): two rows per thread in flight
-    __device__ void stage_update_plain(double a, const double* p)
+    // ================================================================== row stages without a tall-skinny block
+    // ||b||^2 over this CTA's share (b is zero outside listB's rows)
+    __device__ double bnorm2_part()
     {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        double bb = 0.0;
+        for (int64_t t = b0 + warp; t < b1; t += 32) {
+            const int64_t i = (int64_t)__ldg(P.listB + t) * 32 + lane;
+            if (i < P.N) { const double v = P.b[i]; bb = fma(v, v, bb); }
+        }
+        return block_sum(bb, sh.red);
+    }
+    // UPDATE = true: x += a p, r -= a w (line 10, rank zero = Jacobi-CG).  false: r = b - w (lines 3, 12,
+    // 16, Verify).  Then z~ = J r, ||r||^2, r^T z~.  Two slices per warp in flight.
+    template <bool UPDATE>
+    __device__ void stage_rows_plain(double a, const double* p)
+    {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         double rr = 0.0, rho = 0.0;
-        __syncthreads();
-        const int64_t step = 2 * (int64_t)blockDim.x;
-        for (int64_t i0 = row0 + threadIdx.x; i0 < row1; i0 += step) {
-            const int64_t i1 = i0 + blockDim.x;
-            const bool in1 = i1 < row1;
-            const double w0 = P.w[i0], r0 = P.r[i0], d0 = ldg_f64(P.dinv + i0), p0 = p[i0], x0 = P.x[i0];
-            double w1 = 0.0, r1 = 0.0, d1 = 0.0, p1 = 0.0, x1 = 0.0;
-            if (in1) { w1 = P.w[i1]; r1 = P.r[i1]; d1 = ldg_f64(P.dinv + i1); p1 = p[i1]; x1 = P.x[i1]; }
-            const double rn0 = fma(-a, w0, r0), zn0 = rn0 * d0;
-            P.x[i0] = fma(a, p0, x0);
-            P.r[i0] = rn0;
-            P.z[i0] = zn0;
-            rr = fma(rn0, rn0, rr);
-            rho = fma(rn0, zn0, rho);
+        __syncthreads();  // w of this CTA's rows was written by other threads of the CTA
+        for (int64_t t = b0 + warp; t < b1; t += 64) {
+            const int64_t i0 = (int64_t)__ldg(P.listB + t) * 32 + lane;
+            const bool two = t + 32 < b1;
+            const int64_t i1 = two ? (int64_t)__ldg(P.listB + t + 32) * 32 + lane : 0;
+            const bool in0 = i0 < P.N, in1 = two && i1 < P.N;
+            double w0 = 0.0, r0 = 0.0, d0 = 0.0, p0 = 0.0, x0 = 0.0, w1 = 0.0, r1 = 0.0, d1 = 0.0, p1 = 0.0, x1 = 0.0;
+            if (in0) { w0 = P.w[i0]; d0 = ldg_f64(P.dinv + i0); if (UPDATE) { r0 = P.r[i0]; p0 = p[i0]; x0 = P.x[i0]; } else r0 = P.b[i0]; }
+            if (in1) { w1 = P.w[i1]; d1 = ldg_f64(P.dinv + i1); if (UPDATE) { r1 = P.r[i1]; p1 = p[i1]; x1 = P.x[i1]; } else r1 = P.b[i1]; }
+            if (in0) {
+                const double rn = UPDATE ? fma(-a, w0, r0) : r0 - w0, zn = rn * d0;
+                if (UPDATE) P.x[i0] = fma(a, p0, x0);
+                P.r[i0] = rn;
+                P.z[i0] = zn;
+                rr = fma(rn, rn, rr);
+                rho = fma(rn, zn, rho);
+            }
             if (in1) {
-                const double rn1 = fma(-a, w1, r1), zn1 = rn1 * d1;
-                P.x[i1] = fma(a, p1, x1);
-                P.r[i1] = rn1;
-                P.z[i1] = zn1;
-                rr = fma(rn1, rn1, rr);
-                rho = fma(rn1, zn1, rho);
+                const double rn = UPDATE ? fma(-a, w1, r1) : r1 - w1, zn = rn * d1;
+                if (UPDATE) P.x[i1] = fma(a, p1, x1);
+                P.r[i1] = rn;
+                P.z[i1] = zn;
+                rr = fma(rn, rn, rr);
+                rho = fma(rn, zn, rho);
             }
         }
         rr = block_sum(rr, sh.red);
@@ -352,8 +426,9 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
         put(SL_RHO, rho);
     }
 
-    // one 32-row x kp tile of the tile-major copy of HW_I (contiguous 256 kp bytes) into this consumer warp's slot
-    __device__ __forceinline__ void issue_tile(int64_t t)
+    // ================================================================== tile streams over a tile-major n x kp block
+    // one 32-row x kp tile (contiguous 256 kp bytes) of slice s into this consumer warp's slot
+    __device__ __forceinline__ void issue_tile(const double* Mt, int64_t s, bool keep)
     {
         if ((threadIdx.x & 31) == 0) {
             const int warp = threadIdx.x >> 5;
@@ -361,113 +436,139 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
             void* tile = sh.ring + (size_t)warp * tile_bytes;
             uint64_t* bar = &sh.full[warp];
             mbar_arrive_expect_tx(bar, tile_bytes);
-            const double* src = P.HWt + ((size_t)(row0 >> 5) + t) * 32 * P.kp;
             // no reuse before the next iteration: evict_first keeps the gathered vectors and K in L2; when the working
             // set nearly fits the L2 the first hw_res_tiles tiles of every CTA are kept instead (evict_last)
-            bulk_g2s_hint(tile, src, tile_bytes, bar, t < P.hw_res_tiles ? l2_policy_evict_last() : l2_policy_evict_first());
+            bulk_g2s_hint(tile, Mt + (size_t)s * 32 * P.kp, tile_bytes, bar, keep ? l2_policy_evict_last() : l2_policy_evict_first());
         }
     }
-    // Stage C with a coarse space: one pass over HW_I through the shared-memory ring (header comment).
-    //   r_i  <- r_i - a w~_i + sum_j HW_ij (a nu_j)      x~_i <- x~_i + a p~_i      z~_i <- r_i / d_i
-    //   ||r||^2, r^T z~,  c_j = sum_i HW_ij z~_i                                      (eq. (18))
-    __device__ void stage_update_coarse(double a, const double* p)
+    // MODE (Mt = the tile-major copy of HW_I or of W_I):
+    //   TS_UPDATE    r_i <- r_i - a w~_i + sum_j HW_ij (a nu_j), x~_i <- x~_i + a p~_i, z~_i <- r_i / d_i,
+    //                ||r||^2, r^T z~, c_j = sum_i HW_ij z~_i                                  (line 10 + line 22; eq. (18))
+    //   TS_RECOMP_Z  r = b - w, z~ = J r, ||r||^2, r^T z~, c = HW_I^T z~                      (after lines 3, 16)
+    //   TS_RECOMP_R  r = b - w, z~ = J r, ||r||^2, r^T z~, c = W_I^T r                        (lines 3, 12: Q r needs Z^T r)
+    //   TS_ADDW      x_i <- x_i + sign sum_j W_ij v_j     (x + Q r of lines 3 / 16 with v = mu; x = x~ - W_I xi with v = xi)
+    template <int MODE>
+    __device__ void stage_tiles(const double* Mt, double a, const double* p, const double* v, double sign)
     {
+        constexpr bool PASS1 = (MODE == TS_UPDATE || MODE == TS_ADDW);
+        constexpr bool PASS2 = (MODE != TS_ADDW);
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         const int kp = P.kp;
         const uint32_t tile_bytes = 256u * (uint32_t)kp;
         const int nst = min(32, (int)(RD_RING_BYTES / tile_bytes));
-        const int64_t ntiles = (row1 - row0 + 31) >> 5;
+        const int64_t ntiles = b1 - b0;
+        const int64_t N = P.N;
         double rr = 0.0, rho = 0.0;
         double acc[(RD_MAX_K + 31) / 32];
 #pragma unroll
         for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) acc[q] = 0.0;
-        __syncthreads();  // w~ of this CTA's rows was written by other threads of the CTA; anu is in place
+        __syncthreads();  // w~ of this CTA's rows was written by other threads of the CTA; v / anu are in place
         if (warp < nst) {
             double* tile = reinterpret_cast<double*>(sh.ring + (size_t)warp * tile_bytes);
             uint64_t* bar = &sh.full[warp];
             double* zbw = sh.zb[warp];
-            const double* anu = sh.anu;
-            auto issue = [&](int64_t t) { issue_tile(t); };
             int64_t t = warp;
-            double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi = 0.0;
-            refill_fence();  // as in spmv_staged: previous stage's generic reads of these bytes precede the CTA barrier above
+            int32_t s = (t < ntiles) ? __ldg(P.listB + b0 + t) : 0;
+            int32_t sn = (t + nst < ntiles) ? __ldg(P.listB + b0 + t + nst) : 0;
+            double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi_ = 0.0;
+            auto load_rows = [&](int64_t i, double& r_, double& w_, double& d_, double& p_, double& x_) {
+                r_ = w_ = d_ = p_ = x_ = 0.0;
+                if (i < N) {
+                    if (MODE == TS_UPDATE) { r_ = P.r[i]; w_ = P.w[i]; d_ = ldg_f64(P.dinv + i); p_ = p[i]; x_ = P.x[i]; }
+                    else if (MODE == TS_ADDW) { x_ = P.x[i]; }
+                    else { r_ = P.b[i]; w_ = P.w[i]; d_ = ldg_f64(P.dinv + i); }
+                }
+            };
+            refill_fence();  // previous stage's generic reads of these bytes precede the CTA barrier above
             if (t < ntiles) {
-                issue(t);
-                const int64_t i = row0 + 32 * t + lane;
-                if (i < row1) { ri = P.r[i]; wi = P.w[i]; di = ldg_f64(P.dinv + i); pi = p[i]; xi = P.x[i]; }
+                issue_tile(Mt, s, MODE == TS_UPDATE && t < P.hw_res_tiles);
+                load_rows((int64_t)s * 32 + lane, ri, wi, di, pi, xi_);
             }
             for (; t < ntiles; t += nst) {
-                const int64_t i = row0 + 32 * t + lane;
-                const bool in = i < row1;
-                // next tile's row data: in flight while this tile is processed
+                const int64_t i = (int64_t)s * 32 + lane;
+                const bool in = i < N;
                 const int64_t tn = t + nst;
-                const int64_t inx = row0 + 32 * tn + lane;
+                const int32_t snn = (tn + nst < ntiles) ? __ldg(P.listB + b0 + tn + nst) : 0;
+                // next tile's row data: in flight while this tile is processed
                 double rin = 0.0, win = 0.0, din = 0.0, pin = 0.0, xin = 0.0;
-                if (tn < ntiles && inx < row1) { rin = P.r[inx]; win = P.w[inx]; din = ldg_f64(P.dinv + inx); pin = p[inx]; xin = P.x[inx]; }
+                if (tn < ntiles) load_rows((int64_t)sn * 32 + lane, rin, win, din, pin, xin);
                 mbar_wait(bar, ph);
                 ph ^= 1u;
-                // pass 1: lane = row
-                double q0 = 0.0, q1 = 0.0, q2 = 0.0, q3 = 0.0;
-                const double* trow = tile + lane;
+                double q = 0.0;
+                if (PASS1) {  // lane = row
+                    double q0 = 0.0, q1 = 0.0, q2 = 0.0, q3 = 0.0;
+                    const double* trow = tile + lane;
 #pragma unroll 2
-                for (int j = 0; j < kp; j += 4) {
-                    q0 = fma(trow[(j + 0) * 32], anu[j + 0], q0);
-                    q1 = fma(trow[(j + 1) * 32], anu[j + 1], q1);
-                    q2 = fma(trow[(j + 2) * 32], anu[j + 2], q2);
-                    q3 = fma(trow[(j + 3) * 32], anu[j + 3], q3);
-                }
-                const double rn = fma(-a, wi, ri) + ((q0 + q1) + (q2 + q3));
-                const double zn = in ? rn * di : 0.0;
-                if (in) {
-                    P.r[i] = rn;
-                    P.x[i] = fma(a, pi, xi);
-                    P.z[i] = zn;
-                    rr = fma(rn, rn, rr);
-                    rho = fma(rn, zn, rho);
-                }
-                zbw[lane] = zn;
-                __syncwarp();
-                // pass 2: lane = column(s) lane and lane + 32, rows in the skewed order (ii + lane) mod 32
-                if (lane < kp) {
-                    const double* t0 = tile + lane * 32;
-                    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-                    if (lane + 32 < kp) {
-                        const double* t1 = t0 + 32 * 32;
-#pragma unroll 8
-                        for (int ii = 0; ii < 32; ii += 2) {
-                            const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
-                            const double z0 = zbw[r0], z1 = zbw[r1];
-                            a0 = fma(t0[r0], z0, a0);
-                            a1 = fma(t0[r1], z1, a1);
-                            b0 = fma(t1[r0], z0, b0);
-                            b1 = fma(t1[r1], z1, b1);
-                        }
-                    } else {
-#pragma unroll 8
-                        for (int ii = 0; ii < 32; ii += 2) {
-                            const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
-                            a0 = fma(t0[r0], zbw[r0], a0);
-                            a1 = fma(t0[r1], zbw[r1], a1);
-                        }
+                    for (int j = 0; j < kp; j += 4) {
+                        q0 = fma(trow[(j + 0) * 32], v[j + 0], q0);
+                        q1 = fma(trow[(j + 1) * 32], v[j + 1], q1);
+                        q2 = fma(trow[(j + 2) * 32], v[j + 2], q2);
+                        q3 = fma(trow[(j + 3) * 32], v[j + 3], q3);
                     }
-                    acc[0] += a0 + a1;
-                    acc[1] += b0 + b1;
+                    q = (q0 + q1) + (q2 + q3);
                 }
-                refill_fence();  // every lane has read the tile and zb; generic reads ordered before the async refill
-                if (tn < ntiles) issue(tn);
-                ri = rin; wi = win; di = din; pi = pin; xi = xin;
+                if (MODE == TS_ADDW) {
+                    if (in) P.x[i] = fma(sign, q, xi_);
+                } else {
+                    const double rn = (MODE == TS_UPDATE) ? fma(-a, wi, ri) + q : ri - wi;
+                    const double zn = in ? rn * di : 0.0;
+                    if (in) {
+                        P.r[i] = rn;
+                        if (MODE == TS_UPDATE) P.x[i] = fma(a, pi, xi_);
+                        P.z[i] = zn;
+                        rr = fma(rn, rn, rr);
+                        rho = fma(rn, zn, rho);
+                    }
+                    zbw[lane] = (MODE == TS_RECOMP_R) ? (in ? rn : 0.0) : zn;
+                    __syncwarp();
+                }
+                if (PASS2) {  // lane = column(s) lane and lane + 32, rows in the skewed order (ii + lane) mod 32
+                    if (lane < kp) {
+                        const double* t0 = tile + lane * 32;
+                        double a0_ = 0.0, a1_ = 0.0, b0_ = 0.0, b1_ = 0.0;
+                        if (lane + 32 < kp) {
+                            const double* t1 = t0 + 32 * 32;
+#pragma unroll 8
+                            for (int ii = 0; ii < 32; ii += 2) {
+                                const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
+                                const double z0 = zbw[r0], z1 = zbw[r1];
+                                a0_ = fma(t0[r0], z0, a0_);
+                                a1_ = fma(t0[r1], z1, a1_);
+                                b0_ = fma(t1[r0], z0, b0_);
+                                b1_ = fma(t1[r1], z1, b1_);
+                            }
+                        } else {
+#pragma unroll 8
+                            for (int ii = 0; ii < 32; ii += 2) {
+                                const int r0 = (ii + lane) & 31, r1 = (ii + 1 + lane) & 31;
+                                a0_ = fma(t0[r0], zbw[r0], a0_);
+                                a1_ = fma(t0[r1], zbw[r1], a1_);
+                            }
+                        }
+                        acc[0] += a0_ + a1_;
+                        acc[1] += b0_ + b1_;
+                    }
+                }
+                refill_fence();  // every lane has read the tile and zb: generic reads ordered before the async refill
+                if (tn < ntiles) issue_tile(Mt, sn, MODE == TS_UPDATE && tn < P.hw_res_tiles);
+                ri = rin; wi = win; di = din; pi = pin; xi_ = xin;
+                s = sn;
+                sn = snn;
             }
+            if (PASS2) {
 #pragma unroll
-            for (int q = 0; q < (RD_MAX_K + 31) / 32; ++q) {
-                const int j = lane + 32 * q;
-                if (j < kp) sh.cpart[warp * kp + j] = acc[q];
+                for (int q_ = 0; q_ < (RD_MAX_K + 31) / 32; ++q_) {
+                    const int j = lane + 32 * q_;
+                    if (j < kp) sh.cpart[warp * kp + j] = acc[q_];
+                }
             }
         }
+        if (!PASS2) return;
         __syncthreads();
         if ((int)threadIdx.x < kp) {
-            double v = 0.0;
-            for (int cw = 0; cw < nst; ++cw) v += sh.cpart[cw * kp + threadIdx.x];
-            slot(SL_NSCAL + threadIdx.x)[blockIdx.x] = v;
+            double vsum = 0.0;
+            for (int cw = 0; cw < nst; ++cw) vsum += sh.cpart[cw * kp + threadIdx.x];
+            slot(SL_NSCAL + threadIdx.x)[blockIdx.x] = vsum;
         }
         rr = block_sum(rr, sh.red);
         rho = block_sum(rho, sh.red);
@@ -476,12 +577,172 @@ struct Cg3Cta : Cg2CtaT<Cg3Shared> {
     }
 };
 
+// w = B v (both SpMVs with the barrier between them); v^T w goes to SL_DOT.
+__device__ __forceinline__ void apply_B_plain(Cg3Cta& cta, const double* v)
+{
+    cta.opK<false>(v, nullptr, 0.0, nullptr);
+    cta.sync_fetch(false, false);
+    double d = cta.opKT(v);
+    d = block_sum(d, cta.sh.red);
+    cta.put(SL_DOT, d);
+}
+
+// Algorithm 1, the whole solve (line numbers of SURVEY.md 8(c) O3).
 __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Cg3Shared& sh = *reinterpret_cast<Cg3Shared*>(smem_raw);
     Cg3Cta cta(P, sh);
-    alg1_coeff_body(P, sh, cta);
+    const bool coarse = P.use_coarse != 0;
+    const int kp = P.kp;
+    if (coarse)
+        for (int q = threadIdx.x; q < kp * kp; q += blockDim.x) {
+            const int i = q % kp, j = q / kp;
+            sh.C[q] = P.C[q];
+            sh.EW[q] = 0.5 * (P.EW[q] + P.EW[j + (size_t)i * kp]);
+        }
+    if (threadIdx.x < RD_MAX_K) {
+        const int j = threadIdx.x;
+        sh.xi[j] = 0.0; sh.nu[0][j] = 0.0; sh.nu[1][j] = 0.0; sh.g[0][j] = 0.0; sh.g[1][j] = 0.0; sh.sv[j] = 0.0; sh.anu[j] = 0.0;
+        sh.e[j] = 0.0; sh.mu[j] = 0.0; sh.c[j] = 0.0;
+    }
+    // line 1: tau = eps_c ||b||_2
+    {
+        const double bb = cta.bnorm2_part();
+        cta.put(SL_BB, bb);
+    }
+    // line 3: x <- x0 + Q (b - B x0);  r <- b - B x
+    cta.opK<false>(P.x, nullptr, 0.0, nullptr);
+    cta.sync_fetch(true, false);
+    const double bnorm = sqrt(sh.scal[SL_BB]);
+    const double tau = (bnorm > 0.0) ? P.eps_c * bnorm : P.eps_c;
+    __syncthreads();
+    (void)cta.opKT(P.x);
+    int status = RD_ECAP_DEV;
+    int iters = 0, replacements = 0;
+    bool done = false;
+    bool x_split = false;  // x = x~ - W_I xi with xi != 0
+    double rho = 0.0, beta = 0.0;
+    int cur = 0;
+
+    if (coarse) {
+        cta.stage_tiles<TS_RECOMP_R>(P.Wt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x0, c = W_I^T r
+        cta.sync_fetch(true, true);
+        cta.coarse_solve();
+        cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.mu, 1.0);  // x += W_I C W_I^T r
+        cta.sync_fetch(false, false);
+        apply_B_plain(cta, P.x);
+        cta.stage_tiles<TS_RECOMP_Z>(P.HWt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x, z~ = J r, c = (HW_I)^T z~
+    } else {
+        cta.stage_rows_plain<false>(0.0, nullptr);
+    }
+    cta.sync_fetch(true, coarse);
+    // lines 4-6
+    if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; done = true; }
+    bool restart = true;  // line 7 / line 20: p <- z, i.e. p~ = z~, nu = mu, g = c, s = 0
+    double rho_prime = sh.scal[SL_RHO];
+    // line 8
+    cta.tick(7);
+    while (!done && iters < P.cap) {
+        // ---- coefficient part of lines 7 / 20 / 22-23
+        if (coarse) {
+            cta.coef_direction(restart, rho_prime, rho, beta);
+        } else {
+            beta = restart ? 0.0 : rho_prime / rho;
+            rho = rho_prime;
+        }
+        restart = false;
+        cta.tick(4);
+        // ---- stage A: line 23 fused into line 9's first product
+        double* pold = cur ? P.p1 : P.p0;
+        double* pnew = cur ? P.p0 : P.p1;
+        cta.opK<true>(P.z, pold, beta, pnew);
+        cur ^= 1;
+        cta.tick(0);
+        cta.sync_fetch(false, false);
+        cta.tick(1);
+        // ---- stage B
+        {
+            double d = cta.opKT(pnew);
+            d = block_sum(d, sh.red);
+            cta.put(SL_DOT, d);
+        }
+        cta.tick(2);
+        cta.sync_fetch(true, false);
+        cta.tick(3);
+        iters++;
+        double pw = sh.scal[SL_DOT];
+        if (coarse) pw = cta.coef_curvature(pw);  // p^T B p
+        if (!(pw > 0.0) || !(rho > 0.0)) { status = RD_ENOTSPD_DEV; break; }
+        // line 10
+        const double a = rho / pw;
+        if (coarse) {
+            cta.coef_step(a);
+            x_split = true;
+            cta.tick(4);
+            cta.stage_tiles<TS_UPDATE>(P.HWt, a, pnew, sh.anu, 0.0);
+        } else {
+            cta.tick(4);
+            cta.stage_rows_plain<true>(a, pnew);
+        }
+        cta.tick(5);
+        cta.sync_fetch(true, coarse);
+        cta.tick(6);
+        rho_prime = sh.scal[SL_RHO];
+        // line 11
+        const bool scheduled = P.replace_period > 0 && (iters % P.replace_period) == 0;
+        if (sqrt(sh.scal[SL_RR]) <= tau || scheduled) {
+            replacements++;
+            if (x_split) {  // x = x~ - W_I xi
+                cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
+                __syncthreads();
+                if (threadIdx.x < RD_MAX_K) sh.xi[threadIdx.x] = 0.0;
+                x_split = false;
+                cta.sync_fetch(false, false);
+            }
+            // line 12: recompute r = b - B x
+            apply_B_plain(cta, P.x);
+            if (coarse) cta.stage_tiles<TS_RECOMP_R>(P.Wt, 0.0, nullptr, nullptr, 0.0);
+            else cta.stage_rows_plain<false>(0.0, nullptr);
+            cta.sync_fetch(true, coarse);
+            if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 13-15
+            if (coarse) {
+                // line 16: x <- x + Q r; r <- b - B x
+                cta.coarse_solve();
+                cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.mu, 1.0);
+                cta.sync_fetch(false, false);
+                apply_B_plain(cta, P.x);
+                cta.stage_tiles<TS_RECOMP_Z>(P.HWt, 0.0, nullptr, nullptr, 0.0);
+                cta.sync_fetch(true, true);
+                if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 17-19
+            }
+            rho_prime = sh.scal[SL_RHO];
+            restart = true;  // line 20
+        }
+    }
+    // line 26: Verify(x, eps) from a fresh apply on the explicit x
+    const double rr_last = sh.scal[SL_RR];
+    __syncthreads();
+    if (x_split) {
+        cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
+        cta.sync_fetch(false, false);
+    }
+    apply_B_plain(cta, P.x);
+    cta.stage_rows_plain<false>(0.0, nullptr);
+    cta.sync_fetch(true, false);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const double rn = sqrt(sh.scal[SL_RR]);
+        const double rel = (bnorm > 0.0) ? rn / bnorm : rn;
+        if (status == 0 && !(rel <= P.eps)) status = RD_ERESID_DEV;
+        P.rep->iters = iters;
+        P.rep->replacements = replacements;
+        P.rep->status = status;
+        P.rep->rel_resid_verified = rel;
+        P.rep->bnorm = bnorm;
+        P.rep->rr_last = rr_last;
+        cta.tick(7);
+        cta.finish(P.rep);
+    }
 }
 
 }  // namespace rd

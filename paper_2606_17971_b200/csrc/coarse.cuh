@@ -13,13 +13,19 @@
 namespace rd {
 
 // ---------------------------------------------------------------- S1
+// Wt (may be NULL): the same block written tile-major for k_alg1_v3's ring, element (i, j) at
+// (i / 32) * 32 kp + 32 j + i % 32 (one 32-row x kp tile = one contiguous 256 kp bytes), like HWt below.
 __global__ void k_restrict(int64_t N, int64_t ldw, int k, int kp, const double* W, const uint8_t* act,
-                           const uint8_t* hist, int zeroext, double* Wm)
+                           const uint8_t* hist, int zeroext, double* Wm, double* Wt)
 {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
         const bool keep = !act[i] && !(zeroext && hist[i]);
-        for (int j = 0; j < kp; ++j)
-            Wm[i + (size_t)j * ldw] = (keep && j < k) ? ldg_f64(W + i + (size_t)j * ldw) : 0.0;
+        double* wt = Wt ? Wt + (size_t)(i >> 5) * 32 * kp + (i & 31) : nullptr;
+        for (int j = 0; j < kp; ++j) {
+            const double v = (keep && j < k) ? ldg_f64(W + i + (size_t)j * ldw) : 0.0;
+            Wm[i + (size_t)j * ldw] = v;
+            if (wt) wt[(size_t)j * 32] = v;
+        }
     }
 }
 // zero-extension history: A <- A u J after every restriction (reading A9 in DESIGN.md)

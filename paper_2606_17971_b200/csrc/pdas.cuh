@@ -3,7 +3,7 @@
 // (1 = active); a packed LSB-first bitset is produced per step for the report / hash.
 #pragma once
 #include <math_constants.h>
-#include "common.cuh"
+#include "operator.cuh"
 
 namespace rd {
 
@@ -122,6 +122,72 @@ __global__ void k_pack_bits(int64_t N, const uint8_t* act, uint8_t* bits, int* n
     }
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
     if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(n_active, cnt);
+}
+
+// ---- S6 compaction, at the granularity of the 32-row slices / tiles every stage of Algorithm 1 works on -----------
+// ("restrict the reference on the GPU", Alg. 2 step 12; "rebuild bitset / index list
+// by a prefix scan").  Vectors stay full-domain and zero on J, so a slice whose 32 rows are all active holds no row of
+// the inactive system: nothing of it has to be read or written by an iteration.  Two compact, ascending lists:
+//   listB  slices with at least one inactive row                      -> K^T product, vector updates, HW_I / W_I tiles
+//   listA  slices where t = M^{-1} K p~ can be nonzero (p~ = 0 on J): some stored K entry of a row of the slice sits
+//          in an inactive column, or the slice is in listB; entry = 2 s + [s in listB]
+// flags[s]: bit 0 = in listA, bit 1 = in listB.
+__global__ void k_slice_flags(Ell K, int64_t N, const uint8_t* act, uint8_t* flags)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t s = gw; s < K.nslices; s += nwt) {
+        const int64_t row = s * RD_SLICE + lane;
+        const bool inactive = row < N && !act[row];
+        const int64_t o = K.off[s];
+        const int wd = (int)((K.off[s + 1] - o) >> 5);
+        bool hit = false;
+        for (int e = 0; e < wd; ++e) {
+            const int c = ldg_i32(K.col + o + e * 32 + lane);
+            const double a = ldg_f64(K.val + o + e * 32 + lane);
+            hit = hit || (a != 0.0 && !act[c]);
+        }
+        const unsigned anyB = __ballot_sync(0xffffffffu, inactive);
+        const unsigned anyA = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) flags[s] = (uint8_t)(((anyA | anyB) ? 1 : 0) | (anyB ? 2 : 0));
+    }
+}
+
+// One CTA: exclusive scan of the two flag bits over all slices, compact lists, counts[0] = |listA|, counts[1] = |listB|.
+__global__ void __launch_bounds__(1024) k_slice_lists(int64_t nslices, const uint8_t* flags, int32_t* listA, int32_t* listB,
+                                                      int32_t* counts)
+{
+    __shared__ int sa[1024], sb[1024];
+    const int tid = threadIdx.x;
+    const int64_t per = (nslices + blockDim.x - 1) / blockDim.x;
+    const int64_t s0 = min((int64_t)tid * per, nslices), s1 = min(s0 + per, nslices);
+    int ca = 0, cb = 0;
+    for (int64_t s = s0; s < s1; ++s) { const int f = flags[s]; ca += f & 1; cb += (f >> 1) & 1; }
+    sa[tid] = ca;
+    sb[tid] = cb;
+    __syncthreads();
+    for (int o = 1; o < (int)blockDim.x; o <<= 1) {  // Hillis-Steele inclusive scan
+        const int va = (tid >= o) ? sa[tid - o] : 0, vb = (tid >= o) ? sb[tid - o] : 0;
+        __syncthreads();
+        sa[tid] += va;
+        sb[tid] += vb;
+        __syncthreads();
+    }
+    int pa = sa[tid] - ca, pb = sb[tid] - cb;
+    for (int64_t s = s0; s < s1; ++s) {
+        const int f = flags[s];
+        if (f & 1) listA[pa++] = (int32_t)(2 * s + ((f >> 1) & 1));
+        if (f & 2) listB[pb++] = (int32_t)s;
+    }
+    if (tid == (int)blockDim.x - 1) { counts[0] = sa[tid]; counts[1] = sb[tid]; }
+}
+
+// one launch instead of seven memsets: the work vectors of a solve start at zero (rows of slices outside the lists
+// are never written by the kernel and must read as zero)
+__global__ void k_zero_vectors(int64_t n, double* a, double* b, double* c, double* d, double* e, double* f)
+{
+    RD_GRID_STRIDE(i, n) { a[i] = 0.0; b[i] = 0.0; c[i] = 0.0; d[i] = 0.0; e[i] = 0.0; f[i] = 0.0; }
 }
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* p, double v)

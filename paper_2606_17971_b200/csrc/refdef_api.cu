@@ -15,7 +15,6 @@
 
 #include "../../include/refdef.h"
 #include "cg.cuh"
-#include "cg2.cuh"
 #include "cg3.cuh"
 #include "sine.cuh"
 #include "prolong.cuh"
@@ -67,7 +66,11 @@ struct rd_ctx {
     int* h_nactive = nullptr;
     // reference
     int k = 0, kp = 0;
-    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *HWt = nullptr, *Tchunk = nullptr;
+    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *HWt = nullptr, *Wt = nullptr, *Tchunk = nullptr;
+    // S6 compaction: per-slice flags and the two compact lists of live slices of the current active set
+    uint8_t* sflags = nullptr;
+    int32_t *listA = nullptr, *listB = nullptr, *d_live = nullptr;
+    int32_t* h_live = nullptr;
     double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;
     int gram_nparts = 0;
     CoarseInfo* d_cinfo = nullptr;
@@ -268,6 +271,7 @@ int alloc_reference(rd_ctx* ctx, int k)
     RDTRY(dalloc(ctx, &ctx->Wm, nk));
     RDTRY(dalloc(ctx, &ctx->HWm, nk));
     RDTRY(dalloc(ctx, &ctx->HWt, nk));  // tile-major copy of HWm (k_alg1_v3); pad rows stay zero
+    RDTRY(dalloc(ctx, &ctx->Wt, nk));   // tile-major copy of Wm
     RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
     ctx->gram_nparts = ctx->num_sms * 2;
     RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
@@ -287,7 +291,8 @@ int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse)
     const int kp = ctx->kp;
     CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     k_restrict<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
-        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
+        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm,
+        ctx->opt.alg1_variant == 0 ? ctx->Wt : nullptr);
     ctx->launches++;
     CU(cudaEventRecord(ctx->ev[1], ctx->stream));
     const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
@@ -351,21 +356,26 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
         const double hw_bytes = 8.0 * (double)ctx->ldw * ctx->kp;
         const double other = 12.0 * (double)(ctx->K.entries + ctx->KT.entries) + 80.0 * (double)N;
         double frac = hw_bytes > 0 ? std::min(0.5, std::max(0.0, (60e6 - other) / hw_bytes)) : 0.0;
-        const int64_t tiles_per_cta = ((ctx->K.nslices + ctx->cg_grid - 1) / ctx->cg_grid);
+        const int64_t tiles_per_cta = ((n_inactive + 31) / 32 + ctx->cg_grid - 1) / ctx->cg_grid;
         P.hw_res_tiles = (int32_t)((double)tiles_per_cta * frac);
     } P.rep = ctx->d_cgrep;
-    CU(cudaMemsetAsync(ctx->p0, 0, ctx->ldw * sizeof(double), ctx->stream));
-    CU(cudaMemsetAsync(ctx->p1, 0, ctx->ldw * sizeof(double), ctx->stream));
-    CU(cudaMemsetAsync(ctx->z, 0, ctx->ldw * sizeof(double), ctx->stream));
+    const int variant = ctx->opt.alg1_variant == 1 ? 1 : 0;
+    {   // S6 compaction: live 32-row slices of this active set, as two compact lists (pdas.cuh), and zeroed work vectors
+        // (rows outside the lists are never written by k_alg1_v3 and must read as zero)
+        const int gsl = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+        k_slice_flags<<<gsl, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->act, ctx->sflags);
+        k_slice_lists<<<1, 1024, 0, ctx->stream>>>(ctx->K.nslices, ctx->sflags, ctx->listA, ctx->listB, ctx->d_live);
+        k_zero_vectors<<<grid_for(ctx->ldw, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->ldw, ctx->p0, ctx->p1, ctx->z, ctx->w,
+                                                                                               ctx->t, ctx->r);
+        ctx->launches += 3;
+        CU(cudaMemcpyAsync(ctx->h_live, ctx->d_live, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+        P.listA = ctx->listA; P.listB = ctx->listB; P.live_counts = ctx->d_live; P.Wt = ctx->Wt;
+    }
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
-    const int variant = ctx->opt.alg1_variant;
-    const bool v2 = variant != 1;  // coefficient form: one n x r pass per iteration
     if (variant == 0)
         CU(cudaLaunchCooperativeKernel((const void*)k_alg1_v3, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, sizeof(Cg3Shared), ctx->stream));
-    else if (variant == 2)
-        CU(cudaLaunchCooperativeKernel((const void*)k_alg1_v2, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, sizeof(Cg2Shared), ctx->stream));
     else
         CU(cudaLaunchCooperativeKernel((const void*)k_alg1, dim3(ctx->cg_grid), dim3(RD_CG_THREADS), args, 0, ctx->stream));
     ctx->launches++;
@@ -384,9 +394,11 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     // both ELL matrices once (8 B value + 4 B index per stored nonzero), t written and read on all N rows,
     // 14 vector passes over the n inactive rows, the two n x r passes over HW_I and W_I, the mask.
     const double rnk = use_coarse ? (double)rep->rank_used : 0.0;
-    // k_alg1_v2 (default) passes over HW_I only: 8 n r instead of 16 n r.
+    // k_alg1_v3 (default) passes over HW_I only: 8 n r instead of 16 n r.
     rep->bytes_per_iter = 24.0 * (double)ctx->nnz + 16.0 * (double)N + 112.0 * (double)n_inactive +
-                          (v2 ? 8.0 : 16.0) * (double)n_inactive * rnk + (double)N;
+                          (variant == 0 ? 8.0 : 16.0) * (double)n_inactive * rnk + (double)N;
+    rep->live_slices_A = ctx->h_live[0];
+    rep->live_slices_B = ctx->h_live[1];
     return RD_OK;
 }
 
@@ -578,13 +590,15 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     RDTRY(dalloc(ctx, &ctx->d_cnt, 1));
     RDTRY(halloc(ctx, &ctx->h_cnt, 1));
     RDTRY(dalloc(ctx, &ctx->bar, 1));
+    RDTRY(dalloc(ctx, &ctx->sflags, (size_t)ctx->K.nslices));
+    RDTRY(dalloc(ctx, &ctx->listA, (size_t)ctx->K.nslices));
+    RDTRY(dalloc(ctx, &ctx->listB, (size_t)ctx->K.nslices));
+    RDTRY(dalloc(ctx, &ctx->d_live, 2));
+    RDTRY(halloc(ctx, &ctx->h_live, 2));
     // persistent Algorithm-1 kernel: one CTA per SM, all co-resident
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1, RD_CG_THREADS, 0));
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1 does not fit an SM (occupancy 0)");
-    CU(cudaFuncSetAttribute(k_alg1_v2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Cg2Shared)));
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1_v2, RD_CG_THREADS, sizeof(Cg2Shared)));
-    if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v2 does not fit an SM (occupancy 0)");
     CU(cudaFuncSetAttribute(k_alg1_v3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Cg3Shared)));
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_alg1_v3, RD_CG_THREADS, sizeof(Cg3Shared)));
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v3 does not fit an SM (occupancy 0)");

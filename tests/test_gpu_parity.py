@@ -272,9 +272,9 @@ def test_query_device_buffers_match_host_buffers(setup):
 
 @pytest.mark.parametrize("method", [0, 1])
 def test_alg1_kernel_variants_agree(setup, rd, method):
-    """The three persistent kernels (TMA-staged coefficient form, literal recurrence, register-staged coefficient
-    form) run the same Algorithm 1: same status and rank, iteration counts within a few, solutions equal at the
-    level of the 1e-8 stop."""
+    """The two persistent kernels (TMA-staged coefficient form over the live slices, literal recurrence over all rows)
+    run the same Algorithm 1: same status and rank, iteration counts within a few, solutions equal at the level of the
+    1e-8 stop."""
     w, o, g, W = setup
     rng = np.random.default_rng(16)
     act = (rng.random(w.N) < 0.2).astype(np.uint8)
@@ -282,13 +282,13 @@ def test_alg1_kernel_variants_agree(setup, rd, method):
     x0 = np.zeros(w.N)
     out = {}
     try:
-        for variant in (0, 1, 2):
+        for variant in (0, 1):
             g.set_options(rd.Options(pdas_cap=w.pdas_cap, alg1_variant=variant))
             out[variant] = g.solve_inactive(method, act, b, x0)
     finally:
         g.set_options(rd.Options(pdas_cap=w.pdas_cap))
     x_ref, r_ref = out[1]
-    for variant in (0, 2):
+    for variant in (0,):
         x, r = out[variant]
         assert r["status"] == r_ref["status"] == 0 and r["rank_used"] == r_ref["rank_used"]
         assert r["rel_resid_verified"] <= 1e-8
