@@ -559,7 +559,10 @@ def run_loop(args):
                         "unit": "GB/s", "frac": round(achieved / peak, 4), "frac_of_nominal_8TBs": round(achieved / 8000.0, 4),
                         "traffic": prof.get("dram_bytes_per_iter"), "bytes_per_iter": nbytes / max(iters, 1),
                         "us_per_iter": 1e3 * ms / max(iters, 1), "cg_iters": iters, "rank": reps[-1]["rank_used"],
-                        "status": reps[-1]["status"]},
+                        "status": reps[-1]["status"],
+                        "t_stage_us_per_iter": [round(x / max(reps[-1]["iters"], 1), 3) for x in reps[-1]["t_stage_us"]],
+                        "stages": "A (K product), barrier, B (K^T product), barrier+reduce, k x k, C (updates + HW pass), barrier+reduce, outside loop",
+                        "live_slices": [reps[-1]["live_slices_A"], reps[-1]["live_slices_B"]]},
            "reference": ref}
     g.close()
     return out

@@ -23,7 +23,7 @@
 //   C  x~, r, z~ updates, ||r||^2, r^T z~, c = (HW_I)^T z~   (one pass over HW_I, tile-major, through the ring)  S4 + S5
 // Each stage splits ITS list evenly over the CTAs (listA and listB differ only near the boundary of the inactive
 // set), so a PDAS step with |I| << N streams |I|-proportional bytes and stays balanced.  The k x k recurrences
-// between C and A are spread over all 32 warps (two block barriers).
+// between C and A run on two warps (one thread per matrix row, no shuffles in the products).
 //
 // ---- staging.  Stage C: the n x kp block streams through a ring of NST = min(32, 512/kp) tiles of 32 rows x kp
 // columns (256 kp bytes each, 128 KB in total); consumer warp cw owns ring slot cw and its mbarrier, processes the
@@ -51,19 +51,35 @@ struct __align__(128) Cg3Shared {
     double cpart[512];               // tile streams: c partials of the consumer warps, NST x kp <= 512
     double c[RD_MAX_K], mu[RD_MAX_K], nu[2][RD_MAX_K], g[2][RD_MAX_K], sv[RD_MAX_K], xi[RD_MAX_K], anu[RD_MAX_K], e[RD_MAX_K];
     double scal[SL_NSCAL];
+    double small[4];                 // rho, beta, nu^T g, nu^T E_W nu of the current direction
     double red[32];
     uint64_t full[32];  // one mbarrier per warp
-    uint64_t tacc[8];
-    uint64_t tlast;
+    uint64_t tacc[8];   // SM clock cycles per phase (CTA 0 only)
+    uint64_t tlast;     // clock64 at the last tick
+    uint64_t t0_ns;     // %globaltimer at kernel start: cycles are scaled to microseconds with it at the end
+    uint64_t c0;        // clock64 at kernel start
     __align__(128) unsigned char ring[RD_RING_BYTES];  // written by the async proxy only
 };
 
 enum { TS_UPDATE = 0, TS_RECOMP_Z = 1, TS_RECOMP_R = 2, TS_ADDW = 3 };
 
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// entry i of a live-slice list; DENSE: the list is the identity (entry 2 i + 1 with SHIFT = 1: flag set)
+template <bool DENSE, int SHIFT>
+__device__ __forceinline__ int32_t list_entry(const int32_t* list, int64_t i)
+{
+    return DENSE ? (int32_t)((i << SHIFT) | SHIFT) : __ldg(list + i);
+}
+
 struct Cg3Cta {
     const CgParams& P;
     Cg3Shared& sh;
     int64_t a0, a1, b0, b1;  // this CTA's shares of listA / listB (index ranges)
+    bool dense;              // every slice is live (the lists are the identity): the loop stages index directly
     unsigned int nbar;
     int G;
     uint32_t ph;    // phase parity of this warp's mbarrier (uniform in the warp)
@@ -78,11 +94,13 @@ struct Cg3Cta {
         a1 = (int64_t)(blockIdx.x + 1) * nA / G;
         b0 = (int64_t)blockIdx.x * nB / G;
         b1 = (int64_t)(blockIdx.x + 1) * nB / G;
+        dense = (nB == P.K.nslices);  // listA contains listB
         if (threadIdx.x == 0) {
             for (int w = 0; w < 32; ++w) mbar_init(&sh.full[w], 1);
             mbar_fence_init();
             for (int q = 0; q < 8; ++q) sh.tacc[q] = 0;
-            sh.tlast = global_timer_ns();
+            sh.t0_ns = global_timer_ns();
+            sh.c0 = sh.tlast = (uint64_t)clock64();
         }
         __syncthreads();
     }
@@ -94,15 +112,18 @@ struct Cg3Cta {
     }
     __device__ void tick(int slot_)
     {
+        // the SM's own cycle counter (a %globaltimer read per phase would slow CTA 0, and every barrier waits for it)
         if (blockIdx.x == 0 && threadIdx.x == 0) {
-            const uint64_t t = global_timer_ns();
+            const uint64_t t = (uint64_t)clock64();
             sh.tacc[slot_] += t - sh.tlast;
             sh.tlast = t;
         }
     }
     __device__ void finish(CgDevReport* rep)
     {
-        for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = 1e-3 * (double)sh.tacc[q];
+        const double ns = (double)(global_timer_ns() - sh.t0_ns), cyc = (double)((uint64_t)clock64() - sh.c0);
+        const double us_per_cycle = cyc > 0.0 ? 1e-3 * ns / cyc : 0.0;
+        for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = us_per_cycle * (double)sh.tacc[q];
     }
 
     // ---- grid barrier + all-reduce.  Every CTA has written one partial per reduced quantity; the barrier is the
@@ -139,64 +160,77 @@ struct Cg3Cta {
         __syncthreads();
     }
 
-    // ---- k x k part, all 32 warps.  Matrices are symmetric and column-major: row i is read as column i (contiguous,
-    // conflict-free); warp w owns rows w and w + 32, lane j owns entries j and j + 32 of the vectors.
-    __device__ __forceinline__ double row_dot(const double* M, int i, int kp, int lane, double v0, double v1)
+    // ---- k x k part.  Matrices are symmetric and column-major.  Two warps (64 threads, one per row: M[i + j kp] is
+    // conflict-free across a warp and the vector entry is a broadcast) form the matrix-vector products with serial FMA
+    // chains and no shuffles; warp 0 alone takes the k-long dots; named barrier 1 (64 threads) separates the steps and
+    // one block barrier publishes the scalars.  The chain c -> mu -> beta -> nu -> e -> nu^T e is sequential by nature.
+    __device__ __forceinline__ double row_matvec(const double* M, const double* v, int i, int kp)
     {
-        double a = (lane < kp) ? M[lane + (size_t)i * kp] * v0 : 0.0;
-        if (lane + 32 < kp) a = fma(M[lane + 32 + (size_t)i * kp], v1, a);
-        return warp_sum(a);
+        const double* m = M + i;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+#pragma unroll 2
+        for (int j = 0; j < kp; j += 4) {  // kp is a multiple of 8
+            a0 = fma(m[(size_t)(j + 0) * kp], v[j + 0], a0);
+            a1 = fma(m[(size_t)(j + 1) * kp], v[j + 1], a1);
+            a2 = fma(m[(size_t)(j + 2) * kp], v[j + 2], a2);
+            a3 = fma(m[(size_t)(j + 3) * kp], v[j + 3], a3);
+        }
+        return (a0 + a1) + (a2 + a3);
     }
     // mu = C c  (the coarse solve of eq. (18) in W_I coordinates; lines 3 and 16)
     __device__ void coarse_solve()
     {
-        const int kp = P.kp, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        const double c0 = (lane < kp) ? sh.c[lane] : 0.0, c1 = (lane + 32 < kp) ? sh.c[lane + 32] : 0.0;
-        for (int i = warp; i < kp; i += 32) {
-            const double a = row_dot(sh.C, i, kp, lane, c0, c1);
-            if (lane == 0) sh.mu[i] = a;
-        }
+        const int kp = P.kp;
+        if ((int)threadIdx.x < kp) sh.mu[threadIdx.x] = row_matvec(sh.C, sh.c, threadIdx.x, kp);
         __syncthreads();
     }
     // lines 7 / 20 / 22-23 in coefficients and the curvature terms of line 9 that do not need p~^T w~:
     //   mu = C c, rho = r^T z~ - s^T mu, beta, nu = mu + beta nu, g = c + beta g, e = E_W nu, nu^T g, nu^T e
     __device__ void coef_direction(bool restart, double rho_prime, double& rho, double& beta)
     {
-        const int kp = P.kp, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-        const bool r0 = lane < kp, r1 = lane + 32 < kp;
-        const double c0 = r0 ? sh.c[lane] : 0.0, c1 = r1 ? sh.c[lane + 32] : 0.0;
-        for (int i = warp; i < kp; i += 32) {
-            const double a = row_dot(sh.C, i, kp, lane, c0, c1);
-            if (lane == 0) sh.mu[i] = a;
-        }
-        __syncthreads();
-        // every warp forms the new nu, g in registers (same order everywhere: bit-identical)
-        const double* nu_o = sh.nu[par];
-        const double* g_o = sh.g[par];
-        const double mu0 = r0 ? sh.mu[lane] : 0.0, mu1 = r1 ? sh.mu[lane + 32] : 0.0;
-        const double s0_ = (restart || !r0) ? 0.0 : sh.sv[lane], s1_ = (restart || !r1) ? 0.0 : sh.sv[lane + 32];
-        const double smu = warp_sum(fma(s0_, mu0, s1_ * mu1));
-        const double rho_new = rho_prime - smu;
-        const double bt = restart ? 0.0 : rho_new / rho;
-        const double nu0 = r0 ? fma(bt, nu_o[lane], mu0) : 0.0, nu1 = r1 ? fma(bt, nu_o[lane + 32], mu1) : 0.0;
-        const double g0 = r0 ? fma(bt, g_o[lane], c0) : 0.0, g1 = r1 ? fma(bt, g_o[lane + 32], c1) : 0.0;
-        for (int i = warp; i < kp; i += 32) {
-            const double a = row_dot(sh.EW, i, kp, lane, nu0, nu1);
-            if (lane == 0) sh.e[i] = a;
-        }
-        if (warp == 0) {  // the other copy of nu / g: nobody reads it before the barrier below
+        const int kp = P.kp, tid = threadIdx.x;
+        if (tid < 64) {
+            const int lane = tid & 31;
+            const bool row = tid < kp;
+            const bool r0 = lane < kp, r1 = lane + 32 < kp;
+            const double* nu_o = sh.nu[par];
+            const double* g_o = sh.g[par];
             double* nu_n = sh.nu[par ^ 1];
             double* g_n = sh.g[par ^ 1];
-            if (r0) { nu_n[lane] = nu0; g_n[lane] = g0; if (restart) sh.sv[lane] = 0.0; }
-            if (r1) { nu_n[lane + 32] = nu1; g_n[lane + 32] = g1; if (restart) sh.sv[lane + 32] = 0.0; }
+            if (row) sh.mu[tid] = row_matvec(sh.C, sh.c, tid, kp);
+            named_bar_sync(1, 64);
+            if (tid < 32) {  // lane j owns entries j and j + 32
+                const double mu0 = r0 ? sh.mu[lane] : 0.0, mu1 = r1 ? sh.mu[lane + 32] : 0.0;
+                const double s0_ = (restart || !r0) ? 0.0 : sh.sv[lane], s1_ = (restart || !r1) ? 0.0 : sh.sv[lane + 32];
+                const double smu = warp_sum(fma(s0_, mu0, s1_ * mu1));
+                const double rho_new = rho_prime - smu;
+                const double bt = restart ? 0.0 : rho_new / rho;
+                if (r0) { nu_n[lane] = fma(bt, nu_o[lane], mu0); g_n[lane] = fma(bt, g_o[lane], sh.c[lane]); if (restart) sh.sv[lane] = 0.0; }
+                if (r1) { nu_n[lane + 32] = fma(bt, nu_o[lane + 32], mu1); g_n[lane + 32] = fma(bt, g_o[lane + 32], sh.c[lane + 32]); if (restart) sh.sv[lane + 32] = 0.0; }
+                if (lane == 0) { sh.small[0] = rho_new; sh.small[1] = bt; }
+            }
+            named_bar_sync(1, 64);
+            if (row) sh.e[tid] = row_matvec(sh.EW, nu_n, tid, kp);
+            named_bar_sync(1, 64);
+            if (tid < 32) {
+                const double nu0 = r0 ? nu_n[lane] : 0.0, nu1 = r1 ? nu_n[lane + 32] : 0.0;
+                const double g0 = r0 ? g_n[lane] : 0.0, g1 = r1 ? g_n[lane + 32] : 0.0;
+                const double e0 = r0 ? sh.e[lane] : 0.0, e1 = r1 ? sh.e[lane + 32] : 0.0;
+                double x = fma(nu0, g0, nu1 * g1), y = fma(nu0, e0, nu1 * e1);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {  // the two sums interleaved
+                    x += __shfl_xor_sync(0xffffffffu, x, o);
+                    y += __shfl_xor_sync(0xffffffffu, y, o);
+                }
+                if (lane == 0) { sh.small[2] = x; sh.small[3] = y; }
+            }
         }
         __syncthreads();
         par ^= 1;
-        const double e0 = r0 ? sh.e[lane] : 0.0, e1 = r1 ? sh.e[lane + 32] : 0.0;
-        ng = warp_sum(fma(nu0, g0, nu1 * g1));
-        ne = warp_sum(fma(nu0, e0, nu1 * e1));
-        rho = rho_new;
-        beta = bt;
+        rho = sh.small[0];
+        beta = sh.small[1];
+        ng = sh.small[2];
+        ne = sh.small[3];
     }
     __device__ double coef_curvature(double pw) const { return pw - 2.0 * ng + ne; }  // p^T B p
     // line 10 in coefficients; the __syncthreads that opens the tile stream publishes anu
@@ -260,7 +294,7 @@ struct Cg3Cta {
     // Staged product over the list entries [i0, i1) of `list` (SHIFT = 1: entries carry a flag in bit 0).
     // pre(row, flag) loads what the epilogue needs of the row (issued before the wait on the slice, so it never adds a
     // round trip); epi(row, flag, acc, pre(row)) consumes sum_e A[row,e] vin[col_e].
-    template <bool COMBINE, int SHIFT, class Pre, class Epi>
+    template <bool COMBINE, int SHIFT, bool DENSE, class Pre, class Epi>
     __device__ __forceinline__ void spmv_staged(const Ell& A, const int32_t* list, int64_t i0, int64_t i1, const double* v0,
                                                 const double* v1, double beta, Pre pre, Epi epi)
     {
@@ -275,8 +309,8 @@ struct Cg3Cta {
             else { o = A.off[s]; wd = (int)((A.off[s + 1] - o) >> 5); }
         };
         int64_t i = i0 + warp;
-        int32_t ecur = (i < i1) ? __ldg(list + i) : 0;
-        int32_t enxt = (i + 32 < i1) ? __ldg(list + i + 32) : 0;
+        int32_t ecur = (i < i1) ? list_entry<DENSE, SHIFT>(list, i) : 0;
+        int32_t enxt = (i + 32 < i1) ? list_entry<DENSE, SHIFT>(list, i + 32) : 0;
         int wd = 0;
         refill_fence();  // the ring was last read (generic proxy) by the previous stage, before a CTA barrier
         if (i < i1) {
@@ -286,7 +320,7 @@ struct Cg3Cta {
         }
         for (; i < i1; i += 32) {
             const int64_t in = i + 32;
-            const int32_t enn = (in + 32 < i1) ? __ldg(list + in + 32) : 0;  // two ahead: its latency hides behind this slice
+            const int32_t enn = (in + 32 < i1) ? list_entry<DENSE, SHIFT>(list, in + 32) : 0;  // two ahead: its latency hides behind this slice
             const int64_t s = (int64_t)(ecur >> SHIFT), sn = (int64_t)(enxt >> SHIFT);
             const int flag = SHIFT ? (ecur & 1) : 1;
             int64_t on = 0;
@@ -318,13 +352,13 @@ struct Cg3Cta {
 
     // stage A: t = M^{-1} K (v0 + beta v1) on the rows of listA; pnew = v0 + beta v1 on those that hold inactive rows
     // (elsewhere p~ is identically zero and stays so)                                       (Alg. 1 lines 23 + 9)
-    template <bool COMBINE>
+    template <bool COMBINE, bool DENSE>
     __device__ void opK(const double* v0, const double* v1, double beta, double* pnew)
     {
         const int64_t N = P.N;
         const double* minv = P.minv;
         double* t = P.t;
-        spmv_staged<COMBINE, 1>(
+        spmv_staged<COMBINE, 1, DENSE>(
             P.K, P.listA, a0, a1, v0, v1, beta,
             [&](int64_t row, int flag) {
                 RowK r{0.0, 0.0};
@@ -345,6 +379,7 @@ struct Cg3Cta {
             });
     }
     // stage B: w = chi_I (m.v + sigma K^T t) on the rows of listB; returns this thread's partial of v^T w  (line 9)
+    template <bool DENSE>
     __device__ double opKT(const double* v)
     {
         const int64_t N = P.N;
@@ -353,7 +388,7 @@ struct Cg3Cta {
         const double sigma = P.sigma;
         double* w = P.w;
         double dot = 0.0;
-        spmv_staged<false, 0>(
+        spmv_staged<false, 0, DENSE>(
             P.KT, P.listB, b0, b1, P.t, nullptr, 0.0,
             [&](int64_t row, int) {
                 RowKT r{0.0, 0.0, false};
@@ -389,16 +424,16 @@ struct Cg3Cta {
     }
     // UPDATE = true: x += a p, r -= a w (line 10, rank zero = Jacobi-CG).  false: r = b - w (lines 3, 12,
     // 16, Verify).  Then z~ = J r, ||r||^2, r^T z~.  Two slices per warp in flight.
-    template <bool UPDATE>
+    template <bool UPDATE, bool DENSE>
     __device__ void stage_rows_plain(double a, const double* p)
     {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         double rr = 0.0, rho = 0.0;
         __syncthreads();  // w of this CTA's rows was written by other threads of the CTA
         for (int64_t t = b0 + warp; t < b1; t += 64) {
-            const int64_t i0 = (int64_t)__ldg(P.listB + t) * 32 + lane;
+            const int64_t i0 = (int64_t)list_entry<DENSE, 0>(P.listB, t) * 32 + lane;
             const bool two = t + 32 < b1;
-            const int64_t i1 = two ? (int64_t)__ldg(P.listB + t + 32) * 32 + lane : 0;
+            const int64_t i1 = two ? (int64_t)list_entry<DENSE, 0>(P.listB, t + 32) * 32 + lane : 0;
             const bool in0 = i0 < P.N, in1 = two && i1 < P.N;
             double w0 = 0.0, r0 = 0.0, d0 = 0.0, p0 = 0.0, x0 = 0.0, w1 = 0.0, r1 = 0.0, d1 = 0.0, p1 = 0.0, x1 = 0.0;
             if (in0) { w0 = P.w[i0]; d0 = ldg_f64(P.dinv + i0); if (UPDATE) { r0 = P.r[i0]; p0 = p[i0]; x0 = P.x[i0]; } else r0 = P.b[i0]; }
@@ -447,7 +482,7 @@ struct Cg3Cta {
     //   TS_RECOMP_Z  r = b - w, z~ = J r, ||r||^2, r^T z~, c = HW_I^T z~                      (after lines 3, 16)
     //   TS_RECOMP_R  r = b - w, z~ = J r, ||r||^2, r^T z~, c = W_I^T r                        (lines 3, 12: Q r needs Z^T r)
     //   TS_ADDW      x_i <- x_i + sign sum_j W_ij v_j     (x + Q r of lines 3 / 16 with v = mu; x = x~ - W_I xi with v = xi)
-    template <int MODE>
+    template <int MODE, bool DENSE>
     __device__ void stage_tiles(const double* Mt, double a, const double* p, const double* v, double sign)
     {
         constexpr bool PASS1 = (MODE == TS_UPDATE || MODE == TS_ADDW);
@@ -468,8 +503,8 @@ struct Cg3Cta {
             uint64_t* bar = &sh.full[warp];
             double* zbw = sh.zb[warp];
             int64_t t = warp;
-            int32_t s = (t < ntiles) ? __ldg(P.listB + b0 + t) : 0;
-            int32_t sn = (t + nst < ntiles) ? __ldg(P.listB + b0 + t + nst) : 0;
+            int32_t s = (t < ntiles) ? list_entry<DENSE, 0>(P.listB, b0 + t) : 0;
+            int32_t sn = (t + nst < ntiles) ? list_entry<DENSE, 0>(P.listB, b0 + t + nst) : 0;
             double ri = 0.0, wi = 0.0, di = 0.0, pi = 0.0, xi_ = 0.0;
             auto load_rows = [&](int64_t i, double& r_, double& w_, double& d_, double& p_, double& x_) {
                 r_ = w_ = d_ = p_ = x_ = 0.0;
@@ -488,7 +523,7 @@ struct Cg3Cta {
                 const int64_t i = (int64_t)s * 32 + lane;
                 const bool in = i < N;
                 const int64_t tn = t + nst;
-                const int32_t snn = (tn + nst < ntiles) ? __ldg(P.listB + b0 + tn + nst) : 0;
+                const int32_t snn = (tn + nst < ntiles) ? list_entry<DENSE, 0>(P.listB, b0 + tn + nst) : 0;
                 // next tile's row data: in flight while this tile is processed
                 double rin = 0.0, win = 0.0, din = 0.0, pin = 0.0, xin = 0.0;
                 if (tn < ntiles) load_rows((int64_t)sn * 32 + lane, rin, win, din, pin, xin);
@@ -580,9 +615,9 @@ struct Cg3Cta {
 // w = B v (both SpMVs with the barrier between them); v^T w goes to SL_DOT.
 __device__ __forceinline__ void apply_B_plain(Cg3Cta& cta, const double* v)
 {
-    cta.opK<false>(v, nullptr, 0.0, nullptr);
+    cta.opK<false, false>(v, nullptr, 0.0, nullptr);
     cta.sync_fetch(false, false);
-    double d = cta.opKT(v);
+    double d = cta.opKT<false>(v);
     d = block_sum(d, cta.sh.red);
     cta.put(SL_DOT, d);
 }
@@ -612,12 +647,15 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
         cta.put(SL_BB, bb);
     }
     // line 3: x <- x0 + Q (b - B x0);  r <- b - B x
-    cta.opK<false>(P.x, nullptr, 0.0, nullptr);
+    cta.opK<false, false>(P.x, nullptr, 0.0, nullptr);
     cta.sync_fetch(true, false);
     const double bnorm = sqrt(sh.scal[SL_BB]);
     const double tau = (bnorm > 0.0) ? P.eps_c * bnorm : P.eps_c;
+    // ||r||_2 <= tau is tested as ||r||^2 <= tau^2 (no square root on the loop's critical path) unless tau^2 underflows
+    const double tau2 = tau * tau;
+    auto below_tau = [&](double rr) { return tau2 > 0.0 ? rr <= tau2 : sqrt(rr) <= tau; };
     __syncthreads();
-    (void)cta.opKT(P.x);
+    (void)cta.opKT<false>(P.x);
     int status = RD_ECAP_DEV;
     int iters = 0, replacements = 0;
     bool done = false;
@@ -626,19 +664,19 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
     int cur = 0;
 
     if (coarse) {
-        cta.stage_tiles<TS_RECOMP_R>(P.Wt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x0, c = W_I^T r
+        cta.stage_tiles<TS_RECOMP_R, false>(P.Wt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x0, c = W_I^T r
         cta.sync_fetch(true, true);
         cta.coarse_solve();
-        cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.mu, 1.0);  // x += W_I C W_I^T r
+        cta.stage_tiles<TS_ADDW, false>(P.Wt, 0.0, nullptr, sh.mu, 1.0);  // x += W_I C W_I^T r
         cta.sync_fetch(false, false);
         apply_B_plain(cta, P.x);
-        cta.stage_tiles<TS_RECOMP_Z>(P.HWt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x, z~ = J r, c = (HW_I)^T z~
+        cta.stage_tiles<TS_RECOMP_Z, false>(P.HWt, 0.0, nullptr, nullptr, 0.0);  // r = b - B x, z~ = J r, c = (HW_I)^T z~
     } else {
-        cta.stage_rows_plain<false>(0.0, nullptr);
+        cta.stage_rows_plain<false, false>(0.0, nullptr);
     }
     cta.sync_fetch(true, coarse);
     // lines 4-6
-    if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; done = true; }
+    if (below_tau(sh.scal[SL_RR])) { status = 0; done = true; }
     bool restart = true;  // line 7 / line 20: p <- z, i.e. p~ = z~, nu = mu, g = c, s = 0
     double rho_prime = sh.scal[SL_RHO];
     // line 8
@@ -656,14 +694,15 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
         // ---- stage A: line 23 fused into line 9's first product
         double* pold = cur ? P.p1 : P.p0;
         double* pnew = cur ? P.p0 : P.p1;
-        cta.opK<true>(P.z, pold, beta, pnew);
+        if (cta.dense) cta.opK<true, true>(P.z, pold, beta, pnew);
+        else cta.opK<true, false>(P.z, pold, beta, pnew);
         cur ^= 1;
         cta.tick(0);
         cta.sync_fetch(false, false);
         cta.tick(1);
         // ---- stage B
         {
-            double d = cta.opKT(pnew);
+            double d = cta.dense ? cta.opKT<true>(pnew) : cta.opKT<false>(pnew);
             d = block_sum(d, sh.red);
             cta.put(SL_DOT, d);
         }
@@ -680,10 +719,12 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
             cta.coef_step(a);
             x_split = true;
             cta.tick(4);
-            cta.stage_tiles<TS_UPDATE>(P.HWt, a, pnew, sh.anu, 0.0);
+            if (cta.dense) cta.stage_tiles<TS_UPDATE, true>(P.HWt, a, pnew, sh.anu, 0.0);
+            else cta.stage_tiles<TS_UPDATE, false>(P.HWt, a, pnew, sh.anu, 0.0);
         } else {
             cta.tick(4);
-            cta.stage_rows_plain<true>(a, pnew);
+            if (cta.dense) cta.stage_rows_plain<true, true>(a, pnew);
+            else cta.stage_rows_plain<true, false>(a, pnew);
         }
         cta.tick(5);
         cta.sync_fetch(true, coarse);
@@ -691,10 +732,10 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
         rho_prime = sh.scal[SL_RHO];
         // line 11
         const bool scheduled = P.replace_period > 0 && (iters % P.replace_period) == 0;
-        if (sqrt(sh.scal[SL_RR]) <= tau || scheduled) {
+        if (below_tau(sh.scal[SL_RR]) || scheduled) {
             replacements++;
             if (x_split) {  // x = x~ - W_I xi
-                cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
+                cta.stage_tiles<TS_ADDW, false>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
                 __syncthreads();
                 if (threadIdx.x < RD_MAX_K) sh.xi[threadIdx.x] = 0.0;
                 x_split = false;
@@ -702,19 +743,19 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
             }
             // line 12: recompute r = b - B x
             apply_B_plain(cta, P.x);
-            if (coarse) cta.stage_tiles<TS_RECOMP_R>(P.Wt, 0.0, nullptr, nullptr, 0.0);
-            else cta.stage_rows_plain<false>(0.0, nullptr);
+            if (coarse) cta.stage_tiles<TS_RECOMP_R, false>(P.Wt, 0.0, nullptr, nullptr, 0.0);
+            else cta.stage_rows_plain<false, false>(0.0, nullptr);
             cta.sync_fetch(true, coarse);
-            if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 13-15
+            if (below_tau(sh.scal[SL_RR])) { status = 0; break; }  // lines 13-15
             if (coarse) {
                 // line 16: x <- x + Q r; r <- b - B x
                 cta.coarse_solve();
-                cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.mu, 1.0);
+                cta.stage_tiles<TS_ADDW, false>(P.Wt, 0.0, nullptr, sh.mu, 1.0);
                 cta.sync_fetch(false, false);
                 apply_B_plain(cta, P.x);
-                cta.stage_tiles<TS_RECOMP_Z>(P.HWt, 0.0, nullptr, nullptr, 0.0);
+                cta.stage_tiles<TS_RECOMP_Z, false>(P.HWt, 0.0, nullptr, nullptr, 0.0);
                 cta.sync_fetch(true, true);
-                if (sqrt(sh.scal[SL_RR]) <= tau) { status = 0; break; }  // lines 17-19
+                if (below_tau(sh.scal[SL_RR])) { status = 0; break; }  // lines 17-19
             }
             rho_prime = sh.scal[SL_RHO];
             restart = true;  // line 20
@@ -724,11 +765,11 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
     const double rr_last = sh.scal[SL_RR];
     __syncthreads();
     if (x_split) {
-        cta.stage_tiles<TS_ADDW>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
+        cta.stage_tiles<TS_ADDW, false>(P.Wt, 0.0, nullptr, sh.xi, -1.0);
         cta.sync_fetch(false, false);
     }
     apply_B_plain(cta, P.x);
-    cta.stage_rows_plain<false>(0.0, nullptr);
+    cta.stage_rows_plain<false, false>(0.0, nullptr);
     cta.sync_fetch(true, false);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         const double rn = sqrt(sh.scal[SL_RR]);

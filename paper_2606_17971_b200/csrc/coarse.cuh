@@ -3,9 +3,15 @@
 //   S1  Wm = chi_I W               direct restriction, eq. (12); for the zero-extension
 //                                  comparator rows whose DOF was active at an earlier restriction of the
 //                                  sequence are zero as well, eq. (13) PAPER.md:158-162.
-//   S2  HWm = chi_I H Wm           k masked operator applies as a blocked SpMM (cached "BZ")
-//       G = Wm^T Wm, EW = Wm^T HWm two N x k by k contractions on the FP64 tensor cores (mma.sync DMMA)
-//       rank-revealing T from G, E = T^T EW T, cond(E) guard, Cholesky, C = T E^{-1} T^T
+//   S2  G = Wm^T Wm                Gram matrix of the restricted candidate basis on the FP64 tensor cores (mma.sync DMMA)
+//       T from G = V S V^T        rank-revealing transform T = V_r S_r^{-1/2} (keep S_j > 1e-14 S_max)
+//       Zm = Wm T                 the basis Z of eq. (18), formed EXPLICITLY (orthonormal up to the rounding of G),
+//                                 column-major and tile-major (k_alg1_v3's ring)
+//       HZm = chi_I H Zm          r masked operator applies as a blocked SpMM (the cached "BZ")
+//       E = Zm^T HZm              second DMMA contraction; cond(E) guard, Cholesky, C = E^{-1}
+// E is formed from the Z that the iteration really uses, so Q = Z E^{-1} Z^T is the Galerkin projector of span(Z) to
+// working accuracy however ill-conditioned W_I is (forming E = T^T (W_I^T H W_I) T instead amplifies the rounding of
+// the k x k products by 1/S_min and breaks down on small or clustered inactive sets).
 #pragma once
 #include "dense.cuh"
 #include "operator.cuh"
@@ -13,18 +19,41 @@
 namespace rd {
 
 // ---------------------------------------------------------------- S1
-// Wt (may be NULL): the same block written tile-major for k_alg1_v3's ring, element (i, j) at
-// (i / 32) * 32 kp + 32 j + i % 32 (one 32-row x kp tile = one contiguous 256 kp bytes), like HWt below.
 __global__ void k_restrict(int64_t N, int64_t ldw, int k, int kp, const double* W, const uint8_t* act,
-                           const uint8_t* hist, int zeroext, double* Wm, double* Wt)
+                           const uint8_t* hist, int zeroext, double* Wm)
 {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
         const bool keep = !act[i] && !(zeroext && hist[i]);
-        double* wt = Wt ? Wt + (size_t)(i >> 5) * 32 * kp + (i & 31) : nullptr;
-        for (int j = 0; j < kp; ++j) {
-            const double v = (keep && j < k) ? ldg_f64(W + i + (size_t)j * ldw) : 0.0;
-            Wm[i + (size_t)j * ldw] = v;
-            if (wt) wt[(size_t)j * 32] = v;
+        for (int j = 0; j < kp; ++j)
+            Wm[i + (size_t)j * ldw] = (keep && j < k) ? ldg_f64(W + i + (size_t)j * ldw) : 0.0;
+    }
+}
+
+// Zm = Wm T (N x kp by kp x kp; columns of T beyond the retained rank are zero), written column-major and, if Zt != NULL,
+// tile-major for k_alg1_v3's ring: element (i, j) at (i / 32) * 32 kp + 32 j + i % 32 (one 32-row x kp tile = one
+// contiguous 256 kp bytes).  One thread per row and 8 output columns (blockIdx.y = column chunk); T sits in shared
+// memory and is read as broadcasts.
+__global__ void __launch_bounds__(256) k_basis_transform(int64_t N, int64_t ldw, int kp, const double* Wm, const double* T,
+                                                         double* Zm, double* Zt)
+{
+    extern __shared__ double sT[];  // kp x 8: the 8 columns of T of this chunk
+    const int j0 = blockIdx.y * 8;
+    for (int e = threadIdx.x; e < kp * 8; e += blockDim.x) sT[e] = T[(e % kp) + (size_t)(j0 + e / kp) * kp];
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        double acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+        for (int l = 0; l < kp; ++l) {
+            const double w = ldg_f64(Wm + i + (size_t)l * ldw);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) acc[q] = fma(w, sT[l + q * kp], acc[q]);
+        }
+        double* zt = Zt ? Zt + (size_t)(i >> 5) * 32 * kp + (size_t)j0 * 32 + (i & 31) : nullptr;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            Zm[i + (size_t)(j0 + q) * ldw] = acc[q];
+            if (zt) zt[q * 32] = acc[q];
         }
     }
 }
@@ -182,29 +211,22 @@ struct CoarseInfo {
     double cond_E;
 };
 
-// In:  G, EW (kp x kp, column-major, ld kp).  Work: 6 kp x kp scratch matrices.  Out: C = T E^{-1} T^T
-// (kp x kp), info.  Reading A6 of DESIGN.md: G = V S V^T (Jacobi), keep S_j > 1e-14 S_max (singular
-// values of W_I above 1e-7 relative; the paper's QR + SVD threshold is 1e-12),
-// T = V_r S_r^{-1/2}, so Z = W_I T has orthonormal columns; E = T^T EW T = Z^T B Z (eq. (18));
-// cond_2(E) from a Jacobi eigensolve, rank-zero fallback above 1e10.
-__global__ void __launch_bounds__(1024) k_coarse_small(int kp, const double* G, const double* EW, double* work,
-                                                       double* C, CoarseInfo* info)
+// Step 1 of the k x k part.  In: G = Wm^T Wm (kp x kp).  Work: 2 kp x kp scratch.  Out: T (kp x kp, column-major):
+// G = V S V^T (Jacobi), keep S_j > 1e-14 S_max (singular values of W_I above 1e-7 relative; reading A6 of DESIGN.md:
+// the paper's QR + SVD threshold is 1e-12), T[:, q] = V[:, sel_q] S_sel_q^{-1/2} for q < rank, zero
+// columns beyond; info->rank.
+__global__ void __launch_bounds__(1024) k_coarse_T(int kp, const double* G, double* work, double* T, CoarseInfo* info)
 {
     __shared__ DenseShared ds;
     __shared__ int sel[RD_MAX_K];
     __shared__ int s_rank;
-    __shared__ double s_lmin, s_lmax;
     const int n = kp;
     const size_t nn = (size_t)n * n;
-    double* A1 = work;            // G -> eigenvalues on the diagonal; later copy of E for cond; later L^{-1}
-    double* V = work + nn;        // eigenvectors -> T (in place)
-    double* A3 = work + 2 * nn;   // EW symmetrised; later E^{-1}
-    double* A4 = work + 3 * nn;   // EW T ; later L (Cholesky of E); later T E^{-1}
-    double* E = work + 4 * nn;    // E
-    for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) { A1[e] = G[e]; A3[e] = EW[e]; }
+    double* A1 = work;       // G -> eigenvalues on the diagonal
+    double* V = work + nn;   // eigenvectors
+    for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) A1[e] = G[e];
     __syncthreads();
     cta_symmetrize(A1, n, n);
-    cta_symmetrize(A3, n, n);
     cta_jacobi_eig(A1, n, n, V, n, true, ds);
     if (threadIdx.x == 0) {
         double smax = 0.0;
@@ -213,47 +235,69 @@ __global__ void __launch_bounds__(1024) k_coarse_small(int kp, const double* G, 
         for (int j = 0; j < n; ++j)
             if (smax > 0.0 && A1[j + (size_t)j * n] > 1e-14 * smax) sel[r++] = j;
         s_rank = r;
+        info->rank = r;
+        info->fallback = 0;
+        info->cond_E = 0.0;
     }
     __syncthreads();
-    int r = s_rank;
-    // T = V[:, sel] diag(S_sel^{-1/2}), compacted to the left in place (sel[q] >= q): column by column
-    for (int qc = 0; qc < r; ++qc) {
-        const int j = sel[qc];
-        const double sc = rsqrt(A1[j + (size_t)j * n]);
-        __syncthreads();
-        for (int i = threadIdx.x; i < n; i += blockDim.x) V[i + (size_t)qc * n] = V[i + (size_t)j * n] * sc;
+    const int r = s_rank;
+    for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) {
+        const int i = e % n, q = e / n;
+        double v = 0.0;
+        if (q < r) { const int j = sel[q]; v = V[i + (size_t)j * n] * rsqrt(A1[j + (size_t)j * n]); }
+        T[e] = v;
+    }
+}
+
+// Step 2 of the k x k part.  In: E_raw = Zm^T HZm (kp x kp; rows / columns >= rank are zero), T, rank.  Work: 4 kp x kp.
+// Out: E (kp x kp, symmetrised, zero outside the leading rank x rank block), C = E^{-1} (same padding): the coarse solve
+// of eq. (18) in Z coordinates, CW = T E^{-1} T^T: the same solve in W_I coordinates (diagnostics: rd_coarse_setup,
+// rd_energy_fraction), cond_2(E) from a Jacobi eigensolve, rank-zero fallback above 1e10 or if E is not SPD.
+__global__ void __launch_bounds__(1024) k_coarse_E(int kp, const double* Eraw, const double* T, double* work, double* E,
+                                                   double* C, double* CW, CoarseInfo* info)
+{
+    __shared__ DenseShared ds;
+    __shared__ double s_lmin, s_lmax;
+    const int n = kp;
+    const size_t nn = (size_t)n * n;
+    const int r = info->rank;
+    double* A1 = work;            // copy of E for the eigenvalues; later L^{-1}
+    double* A4 = work + nn;       // L (Cholesky of E); later T E^{-1}
+    double* A3 = work + 2 * nn;   // E^{-1} (r x r)
+    for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) {
+        const int i = e % n, j = e / n;
+        E[e] = (i < r && j < r) ? 0.5 * (Eraw[i + (size_t)j * n] + Eraw[j + (size_t)i * n]) : 0.0;
+        C[e] = 0.0;
+        CW[e] = 0.0;
     }
     __syncthreads();
-    bool fallback = false;
-    double cond = 0.0;
-    if (r > 0) {
-        cta_matmul(n, r, n, A3, 1, n, V, 1, n, A4, n);       // A4 = EW T         (n x r)
-        cta_matmul(r, r, n, V, n, 1, A4, 1, n, E, n);        // E  = T^T EW T     (r x r)
-        cta_symmetrize(E, n, r);
-        for (int e = threadIdx.x; e < r * r; e += blockDim.x) A1[(e % r) + (size_t)(e / r) * n] = E[(e % r) + (size_t)(e / r) * n];
-        cta_jacobi_eig(A1, n, r, nullptr, 0, false, ds);
-        if (threadIdx.x == 0) {
-            double lmin = A1[0], lmax = A1[0];
-            for (int j = 1; j < r; ++j) { lmin = fmin(lmin, A1[j + (size_t)j * n]); lmax = fmax(lmax, A1[j + (size_t)j * n]); }
-            s_lmin = lmin; s_lmax = lmax;
-        }
-        __syncthreads();
-        cond = (s_lmin > 0.0) ? s_lmax / s_lmin : INFINITY;
-        for (int e = threadIdx.x; e < r * r; e += blockDim.x) A4[(e % r) + (size_t)(e / r) * n] = E[(e % r) + (size_t)(e / r) * n];
-        bool ok = cta_cholesky(A4, n, r, ds);
-        if (!(cond <= 1e10) || !ok) { fallback = true; }
+    if (r == 0) return;
+    for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) { A1[e] = E[e]; A4[e] = E[e]; }
+    __syncthreads();
+    cta_jacobi_eig(A1, n, r, nullptr, 0, false, ds);
+    if (threadIdx.x == 0) {
+        double lmin = A1[0], lmax = A1[0];
+        for (int j = 1; j < r; ++j) { lmin = fmin(lmin, A1[j + (size_t)j * n]); lmax = fmax(lmax, A1[j + (size_t)j * n]); }
+        s_lmin = lmin; s_lmax = lmax;
     }
-    if (fallback || r == 0) {
-        for (int e = threadIdx.x; e < (int)nn; e += blockDim.x) C[e] = 0.0;
-        if (threadIdx.x == 0) { info->rank = 0; info->fallback = fallback ? 1 : 0; info->cond_E = cond; }
+    __syncthreads();
+    const double cond = (s_lmin > 0.0) ? s_lmax / s_lmin : INFINITY;
+    const bool ok = cta_cholesky(A4, n, r, ds);
+    if (!(cond <= 1e10) || !ok) {
+        if (threadIdx.x == 0) { info->rank = 0; info->fallback = 1; info->cond_E = cond; }
         return;
     }
     cta_tri_inverse_lower(A4, n, r, A1, n);                  // A1 = L^{-1}
-    cta_matmul(r, r, r, A1, n, 1, A1, 1, n, A3, n);          // A3 = L^{-T} L^{-1} = E^{-1}   (sum over k >= max(i,j); zeros above)
-    cta_matmul(n, r, r, V, 1, n, A3, 1, n, A4, n);           // A4 = T E^{-1}     (n x r)
-    cta_matmul(n, n, r, A4, 1, n, V, n, 1, C, n);            // C  = T E^{-1} T^T (n x n)
-    cta_symmetrize(C, n, n);
-    if (threadIdx.x == 0) { info->rank = r; info->fallback = 0; info->cond_E = cond; }
+    cta_matmul(r, r, r, A1, n, 1, A1, 1, n, A3, n);          // A3 = L^{-T} L^{-1} = E^{-1}
+    for (int e = threadIdx.x; e < r * r; e += blockDim.x) {
+        const int i = e % r, j = e / r;
+        C[i + (size_t)j * n] = 0.5 * (A3[i + (size_t)j * n] + A3[j + (size_t)i * n]);
+    }
+    __syncthreads();
+    cta_matmul(n, r, r, T, 1, n, C, 1, n, A4, n);            // A4 = T E^{-1}     (n x r)
+    cta_matmul(n, n, r, A4, 1, n, T, n, 1, CW, n);           // CW = T E^{-1} T^T (n x n)
+    cta_symmetrize(CW, n, n);
+    if (threadIdx.x == 0) { info->fallback = 0; info->cond_E = cond; }
 }
 
 // ---------------------------------------------------------------- eq. (24): energy fraction of the coarse correction

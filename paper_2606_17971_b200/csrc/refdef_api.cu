@@ -66,12 +66,15 @@ struct rd_ctx {
     int* h_nactive = nullptr;
     // reference
     int k = 0, kp = 0;
-    double *W = nullptr, *Wm = nullptr, *HWm = nullptr, *HWt = nullptr, *Wt = nullptr, *Tchunk = nullptr;
+    // W: the stored reference.  Wm = chi_I W (restricted candidate basis).  Zm = Wm T: the basis Z of eq. (18), formed
+    // explicitly; HZm = chi_I H Zm (the cached BZ); Zt / HZt: their tile-major copies for k_alg1_v3's ring.
+    double *W = nullptr, *Wm = nullptr, *Zm = nullptr, *HZm = nullptr, *Zt = nullptr, *HZt = nullptr, *Tchunk = nullptr;
     // S6 compaction: per-slice flags and the two compact lists of live slices of the current active set
     uint8_t* sflags = nullptr;
     int32_t *listA = nullptr, *listB = nullptr, *d_live = nullptr;
     int32_t* h_live = nullptr;
-    double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;
+    double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;  // EW: W_I^T H W_I on request
+    double *T = nullptr, *Eraw = nullptr, *E = nullptr, *CW = nullptr;  // T (W_I -> Z), E = Z^T B Z, C = E^{-1}, CW = T C T^T
     int gram_nparts = 0;
     CoarseInfo* d_cinfo = nullptr;
     CoarseInfo* h_cinfo = nullptr;
@@ -269,9 +272,10 @@ int alloc_reference(rd_ctx* ctx, int k)
     const size_t nk = (size_t)ctx->ldw * kp;
     RDTRY(dalloc(ctx, &ctx->W, nk));
     RDTRY(dalloc(ctx, &ctx->Wm, nk));
-    RDTRY(dalloc(ctx, &ctx->HWm, nk));
-    RDTRY(dalloc(ctx, &ctx->HWt, nk));  // tile-major copy of HWm (k_alg1_v3); pad rows stay zero
-    RDTRY(dalloc(ctx, &ctx->Wt, nk));   // tile-major copy of Wm
+    RDTRY(dalloc(ctx, &ctx->Zm, nk));
+    RDTRY(dalloc(ctx, &ctx->HZm, nk));
+    RDTRY(dalloc(ctx, &ctx->Zt, nk));   // tile-major copies (k_alg1_v3); pad rows stay zero
+    RDTRY(dalloc(ctx, &ctx->HZt, nk));
     RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
     ctx->gram_nparts = ctx->num_sms * 2;
     RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
@@ -279,39 +283,58 @@ int alloc_reference(rd_ctx* ctx, int k)
     RDTRY(dalloc(ctx, &ctx->EW, (size_t)kp * kp));
     RDTRY(dalloc(ctx, &ctx->cwork, (size_t)6 * kp * kp));
     RDTRY(dalloc(ctx, &ctx->C, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->T, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->Eraw, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->E, (size_t)kp * kp));
+    RDTRY(dalloc(ctx, &ctx->CW, (size_t)kp * kp));
     ctx->k = k;
     ctx->kp = kp;
     return RD_OK;
 }
 
-// S1 + S2 for the active set in ctx->act.  Leaves Wm, HWm, C and *h_cinfo (after a stream sync by the caller).
-int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse)
+// S1 + S2 for the active set in ctx->act.  Leaves Zm, HZm (and their tile-major copies), E, C = E^{-1}, CW and *h_cinfo
+// (the stream is synchronised before returning).  want_EW: also form W_I^T H_II W_I in ctx->EW (diagnostics only).
+int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse, bool want_EW = false)
 {
     const int64_t N = ctx->N;
     const int kp = ctx->kp;
+    const bool tiles = ctx->opt.alg1_variant == 0;
     CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     k_restrict<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
-        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm,
-        ctx->opt.alg1_variant == 0 ? ctx->Wt : nullptr);
+        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
     ctx->launches++;
     CU(cudaEventRecord(ctx->ev[1], ctx->stream));
     const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
-    for (int j = 0; j < kp; j += 8) {
-        const double* V = ctx->Wm + (size_t)j * ctx->ldw;
-        k_spmm_K<8><<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->ldw, ctx->minv, V, ctx->ldw, ctx->Tchunk);
-        k_spmm_KT<8><<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->ldw, ctx->m, ctx->sigma, ctx->act, V, ctx->ldw,
-                                                       ctx->Tchunk, ctx->ldw, ctx->HWm + (size_t)j * ctx->ldw,
-                                                       ctx->opt.alg1_variant == 0 ? ctx->HWt : nullptr, kp, j);
-        ctx->launches += 2;
-    }
     dim3 gg(ctx->gram_nparts, (kp + 63) / 64, (kp + 63) / 64);
     const int64_t kk = (int64_t)kp * kp;
-    k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, kp, kp, ctx->Wm, ctx->ldw, ctx->Wm, ctx->ldw, ctx->gram_parts);
-    k_reduce_parts<<<grid_for(kk, kThreads, 64), kThreads, 0, ctx->stream>>>(ctx->gram_nparts, kk, ctx->gram_parts, ctx->G);
-    k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, kp, kp, ctx->Wm, ctx->ldw, ctx->HWm, ctx->ldw, ctx->gram_parts);
-    k_reduce_parts<<<grid_for(kk, kThreads, 64), kThreads, 0, ctx->stream>>>(ctx->gram_nparts, kk, ctx->gram_parts, ctx->EW);
-    k_coarse_small<<<1, 1024, 0, ctx->stream>>>(kp, ctx->G, ctx->EW, ctx->cwork, ctx->C, ctx->d_cinfo);
-    ctx->launches += 5;
+    // H_II V for the kp columns of V, 8 at a time: OUT column-major, OUTT (may be NULL) tile-major
+    auto spmm_H = [&](const double* V, double* OUT, double* OUTT) {
+        for (int j = 0; j < kp; j += 8) {
+            const double* Vj = V + (size_t)j * ctx->ldw;
+            k_spmm_K<8><<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ctx->ldw, ctx->minv, Vj, ctx->ldw, ctx->Tchunk);
+            k_spmm_KT<8><<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ctx->ldw, ctx->m, ctx->sigma, ctx->act, Vj, ctx->ldw,
+                                                           ctx->Tchunk, ctx->ldw, OUT + (size_t)j * ctx->ldw, OUTT, kp, j);
+            ctx->launches += 2;
+        }
+    };
+    auto gram = [&](const double* A, const double* B, double* out) {
+        k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, kp, kp, A, ctx->ldw, B, ctx->ldw, ctx->gram_parts);
+        k_reduce_parts<<<grid_for(kk, kThreads, 64), kThreads, 0, ctx->stream>>>(ctx->gram_nparts, kk, ctx->gram_parts, out);
+        ctx->launches += 2;
+    };
+    gram(ctx->Wm, ctx->Wm, ctx->G);
+    if (want_EW) {  // W_I^T H_II W_I (HZm serves as scratch for H_II W_I; it is overwritten below)
+        spmm_H(ctx->Wm, ctx->HZm, nullptr);
+        gram(ctx->Wm, ctx->HZm, ctx->EW);
+    }
+    k_coarse_T<<<1, 1024, 0, ctx->stream>>>(kp, ctx->G, ctx->cwork, ctx->T, ctx->d_cinfo);
+    k_basis_transform<<<dim3(std::max(1, grid_for(N, 256, big_grid(ctx)) / 2), kp / 8), 256, (size_t)kp * 8 * sizeof(double), ctx->stream>>>(
+        N, ctx->ldw, kp, ctx->Wm, ctx->T, ctx->Zm, tiles ? ctx->Zt : nullptr);
+    ctx->launches += 2;
+    spmm_H(ctx->Zm, ctx->HZm, tiles ? ctx->HZt : nullptr);
+    gram(ctx->Zm, ctx->HZm, ctx->Eraw);
+    k_coarse_E<<<1, 1024, 0, ctx->stream>>>(kp, ctx->Eraw, ctx->T, ctx->cwork, ctx->E, ctx->C, ctx->CW, ctx->d_cinfo);
+    ctx->launches++;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(ctx->h_cinfo, ctx->d_cinfo, sizeof(CoarseInfo), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaEventRecord(ctx->ev[2], ctx->stream));
@@ -348,7 +371,8 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.m = ctx->m; P.minv = ctx->minv; P.dinv = ctx->dinv; P.sigma = ctx->sigma;
     P.act = ctx->act; P.b = ctx->b;
     P.x = ctx->x; P.r = ctx->r; P.p0 = ctx->p0; P.p1 = ctx->p1; P.z = ctx->z; P.w = ctx->w; P.t = ctx->t;
-    P.Wm = ctx->Wm; P.HWm = ctx->HWm; P.HWt = ctx->HWt; P.C = ctx->C; P.EW = ctx->EW;
+    // the kernels work in the coordinates of the explicit basis Z = W_I T: "Wm" = Zm, "HWm" = H_II Zm, C = E^{-1}, "EW" = E
+    P.Wm = ctx->Zm; P.HWm = ctx->HZm; P.HWt = ctx->HZt; P.C = ctx->C; P.EW = ctx->E;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
     P.partial = ctx->partial; P.bar = ctx->bar;
     {   // Part of the H_II W_I stream is requested with L2 evict_last when the whole working set nearly fits the
@@ -369,7 +393,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
                                                                                                ctx->t, ctx->r);
         ctx->launches += 3;
         CU(cudaMemcpyAsync(ctx->h_live, ctx->d_live, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
-        P.listA = ctx->listA; P.listB = ctx->listB; P.live_counts = ctx->d_live; P.Wt = ctx->Wt;
+        P.listA = ctx->listA; P.listB = ctx->listB; P.live_counts = ctx->d_live; P.Wt = ctx->Zt;
     }
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
@@ -1237,7 +1261,7 @@ int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* 
     const uint8_t* da;
     RDTRY(in_dev(ctx, active, ctx->N, ctx->act_stage, &da));
     CU(cudaMemcpyAsync(ctx->act, da, ctx->N, cudaMemcpyDeviceToDevice, ctx->stream));
-    RDTRY(coarse_setup(ctx, method, nullptr, nullptr));
+    RDTRY(coarse_setup(ctx, method, nullptr, nullptr, EW != nullptr));
     const int kp = ctx->kp, k = ctx->k;
     auto copy_kk = [&](double* dst, const double* src) -> int {
         if (!dst) return RD_OK;
@@ -1246,7 +1270,7 @@ int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* 
     };
     RDTRY(copy_kk(G, ctx->G));
     RDTRY(copy_kk(EW, ctx->EW));
-    RDTRY(copy_kk(C, ctx->C));
+    RDTRY(copy_kk(C, ctx->CW));
     CU(cudaStreamSynchronize(ctx->stream));
     if (rank_used) *rank_used = ctx->h_cinfo->rank;
     if (cond_E) *cond_E = ctx->h_cinfo->cond_E;
@@ -1313,7 +1337,7 @@ int rd_energy_fraction(rd_ctx* ctx, int32_t method, const uint8_t* active, const
     const int np = nparts ? nparts : ctx->cg_grid;
     k_energy_parts<<<np, 256, 0, ctx->stream>>>(N, ctx->ldw, kp, ctx->Wm, ctx->b, ctx->x, ctx->w, parts);
     k_reduce_parts<<<1, 128, 0, ctx->stream>>>(np, kp + 1, parts, red);
-    k_energy_fraction<<<1, 64, 0, ctx->stream>>>(kp, use_coarse, ctx->C, red, red + kp + 1);
+    k_energy_fraction<<<1, 64, 0, ctx->stream>>>(kp, use_coarse, ctx->CW, red, red + kp + 1);
     ctx->launches += 3;
     CU(cudaGetLastError());
     double h[3];
