@@ -247,6 +247,16 @@ int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* 
  * y_d, psi, y, lambda: N doubles, host or device (psi_i = +inf allowed).  kkt: 5 host doubles. */
 int rd_kkt(rd_ctx* ctx, const double* y_d, const double* psi, const double* y, const double* lambda, double* kkt);
 
+/* S6, one multiplier / active-set update of PDAS (eq. (7)-(8)) for ANY state y and active set, as
+ * rd_solve_query performs it after every inner solve: lambda = l - H y on the active set and exactly 0 on the inactive
+ * set (reading A4), active_new_i = [psi_i finite and lambda_i + c_i (y_i - psi_i) > 0] with c_i = 1 or H_ii
+ * (rd_options.c_is_diag), margin = min_i |lambda_i + c_i (y_i - psi_i)| over finite psi_i.
+ * y_d, psi, y: N doubles; active: N bytes (non-zero = active); lambda_out: N doubles; active_new_out: N bytes; all host or
+ * device.  changed (number of DOFs whose membership changes), n_active_new, margin: host scalars, may be NULL.
+ * Touches neither the sequence state nor the zero-extension history. */
+int rd_pdas_update(rd_ctx* ctx, const double* y_d, const double* psi, const uint8_t* active, const double* y,
+                   double* lambda_out, uint8_t* active_new_out, int64_t* changed, int64_t* n_active_new, double* margin);
+
 /* Transient variant of the coarse-mesh reference, eq. (14) (section 2.2.2; reading A21).
  * The context holds the all-at-once operator of N = N_s * nt DOFs in the layout id = space + N_s * t.  Phi: N_s x rs
  * spatial vectors, column-major, host or device (e.g. prolonged coarse vectors, or the reference of a steady

@@ -23,7 +23,7 @@ SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
            "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
-           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt"]
+           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
 
 
 class RefDefError(RuntimeError):
@@ -118,6 +118,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_coarse_setup.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl), C.POINTER(i32)]
     lib.rd_energy_fraction.argtypes = [vp, i32, vp, vp, vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(dbl)]
     lib.rd_kkt.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.rd_pdas_update.argtypes = [vp, vp, vp, vp, vp, vp, vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(dbl)]
     _lib = lib
     return lib
 
@@ -364,6 +365,21 @@ class RefDef:
         out = (C.c_double * 5)()
         self._check(self._lib.rd_kkt(self._h, _ptr(y_d), _ptr(psi), _ptr(y), _ptr(lam), out), "rd_kkt")
         return np.array(list(out))
+
+    def pdas_update(self, y_d, psi, active, y):
+        """One multiplier / active-set update (eq. (7)-(8)): returns (lambda, active_new, changed, n_active_new, margin)."""
+        host = isinstance(y, np.ndarray)
+        lam = np.empty(self.N) if host else y.new_empty(self.N)
+        if host:
+            act_new = np.empty(self.N, dtype=np.uint8)
+        else:
+            import torch
+
+            act_new = torch.empty(self.N, dtype=torch.uint8, device=y.device)
+        ch, na, mg = C.c_int64(0), C.c_int64(0), C.c_double(0)
+        self._check(self._lib.rd_pdas_update(self._h, _ptr(y_d), _ptr(psi), _ptr(active), _ptr(y), _ptr(lam), _ptr(act_new),
+                                             C.byref(ch), C.byref(na), C.byref(mg)), "rd_pdas_update")
+        return lam, act_new, ch.value, na.value, mg.value
 
     # ---- the query
     def solve_query(self, method, y_d, psi, J0=None, y=None, u=None, lam=None, want_sets=True):

@@ -1374,6 +1374,40 @@ int rd_kkt(rd_ctx* ctx, const double* y_d, const double* psi, const double* y, c
     return RD_OK;
 }
 
+int rd_pdas_update(rd_ctx* ctx, const double* y_d, const double* psi, const uint8_t* active, const double* y,
+                   double* lambda_out, uint8_t* active_new_out, int64_t* changed, int64_t* n_active_new, double* margin)
+{
+    if (!ctx || !y_d || !psi || !active || !y || !lambda_out || !active_new_out) return RD_EINVAL;
+    const int64_t N = ctx->N;
+    const int g = grid_for(N, kThreads, big_grid(ctx));
+    const double *dyd, *dpsi, *dy;
+    const uint8_t* da;
+    RDTRY(in_dev(ctx, y_d, N, ctx->in0, &dyd));
+    k_ell<<<g, kThreads, 0, ctx->stream>>>(N, ctx->m, dyd, ctx->ell);
+    RDTRY(in_dev(ctx, psi, N, ctx->in1, &dpsi));
+    RDTRY(in_dev(ctx, y, N, ctx->in0, &dy));  // in0 is free again: l has been formed (same stream)
+    RDTRY(in_dev(ctx, active, N, ctx->act_stage, &da));
+    RDTRY(launch_apply_H(ctx, dy, nullptr, ctx->Hy));
+    CU(cudaMemsetAsync(ctx->d_cnt, 0, sizeof(PdasCounters), ctx->stream));
+    {
+        const unsigned long long inf_bits = 0x7ff0000000000000ULL;
+        CU(cudaMemcpyAsync(&ctx->d_cnt->margin_bits, &inf_bits, sizeof inf_bits, cudaMemcpyHostToDevice, ctx->stream));
+    }
+    // lam / act_new / tmp are scratch here: the sequence's own state (ystate, act_seq, hist) is not touched
+    k_pdas_update<<<g, kThreads, 0, ctx->stream>>>(N, da, ctx->ell, ctx->Hy, dy, dpsi, ctx->d, ctx->opt.c_is_diag, ctx->lam, ctx->act_new,
+                                                   ctx->tmp, ctx->d_cnt);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(PdasCounters), cudaMemcpyDeviceToHost, ctx->stream));
+    RDTRY(out_host(ctx, lambda_out, ctx->lam, N));
+    RDTRY(out_host(ctx, active_new_out, ctx->act_new, N));
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (changed) *changed = ctx->h_cnt->changed;
+    if (n_active_new) *n_active_new = ctx->h_cnt->n_active_new;
+    if (margin) memcpy(margin, &ctx->h_cnt->margin_bits, sizeof(double));
+    return RD_OK;
+}
+
 int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double* psi, const uint8_t* J0, double* y, double* u,
                    double* lambda, rd_step_report* steps, uint8_t* J_bits, rd_query_report* rep)
 {

@@ -1,0 +1,84 @@
+"""Writes tests/golden/twin_<name>.json / .npz from the CPU oracle ONLY (never from the CUDA path).
+
+Run:  python tests/golden/make_golden_twins.py [name ...]      (no names: every case; the 256 x 256 case takes the longest)
+
+Complete query sequences of the larger twins of BASELINE.json's configs, too slow to run live inside the GPU tests
+(minutes to an hour of single-threaded oracle time each): the oracle's PDAS active-set sequence (FNV-1a hash of the
+packed set and |I| per step), CG iterations, retained rank, margins and statuses per step (json) and the final y of
+each query (npz, float64).  tests/test_gpu_twins_golden.py runs the same queries through the C ABI and compares.
+
+Settings, identical on both sides: RefDef (direct restriction) with the paper's analytical reference (oracle.sine_reference /
+oracle.spacetime_reference, deterministic closed forms), warm-start policy of PAPER.md:339 over the listed queries,
+eps = eps_c = 1e-12 so that every active-set decision (smallest margins here ~1e-11) is far from the solver's noise and
+the sequence is a property of the method, not of rounding; PDAS cap 400 (the paper's raised cap).
+"""
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+sys.path.insert(0, ROOT)
+
+import oracle  # noqa: E402
+from workloads import make_config  # noqa: E402
+
+# name -> (make_config kwargs, queries)
+CASES = {
+    "c3_32": (dict(twin="c3_32"), [0, 1]),
+    "c2_128": (dict(twin="c2_128"), [0, 1]),
+    "c4_64x8": (dict(twin="c4_64x8"), [0]),
+    "c5_48": (dict(twin="c5_48"), [0, 1]),
+    "c2_256": (dict(config=2, n=256, k=32), [0]),
+}
+EPS = 1e-12
+PDAS_CAP = 400
+
+
+def reference_for(w):
+    if w.nt > 1:
+        return np.asfortranarray(oracle.spacetime_reference(w.dims, w.nt, 1.0 / w.nt, w.k)[-1])
+    return np.asfortranarray(oracle.sine_reference(w.dims, w.k)[-1])
+
+
+def run_case(name):
+    kw, queries = CASES[name]
+    w = make_config(**kw)
+    o = oracle.Oracle.from_workload(w)
+    W = reference_for(w)
+    opt = oracle.OracleOptions(eps=EPS, eps_c=EPS, pdas_cap=PDAS_CAP)
+    out = {"case": name, "make_config": kw, "workload": w.name, "N": w.N, "k": w.k, "operator_sha256": w.operator_hash(),
+           "eps": EPS, "pdas_cap": PDAS_CAP, "method": "refdef", "reference": "analytical (oracle.sine_reference / spacetime_reference)",
+           "queries": []}
+    ys = {}
+    for q in queries:
+        yd, psi = w.target(q)
+        t0 = time.time()
+        r = o.solve_query(oracle.REFDEF, yd, psi, W, opt)
+        dt = time.time() - t0
+        out["queries"].append({
+            "query": q, "status": r["status"], "n_steps": r["n_steps"], "kkt": [float(v) for v in r["kkt"]],
+            "n_inactive": [s["n_inactive"] for s in r["steps"]],
+            "active_hash": [f"{s['active_hash']:016x}" for s in r["steps"]],
+            "cg_iters": [s["cg_iters"] for s in r["steps"]],
+            "rank_used": [s["rank_used"] for s in r["steps"]],
+            "inner_status": [s["status"] for s in r["steps"]],
+            "margin": [float(s["margin"]) for s in r["steps"]],
+            "y_Mnorm": float(np.sqrt((w.m * r["y"] ** 2).sum())),
+            "u_Mnorm": float(np.sqrt((w.m * r["u"] ** 2).sum())),
+            "oracle_seconds": round(dt, 1),
+        })
+        ys[f"y{q}"] = r["y"]
+        print(name, "query", q, "status", r["status"], "steps", r["n_steps"], "iters", sum(out["queries"][-1]["cg_iters"]),
+              f"{dt:.0f} s", flush=True)
+    with open(os.path.join(HERE, f"twin_{name}.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    np.savez_compressed(os.path.join(HERE, f"twin_{name}.npz"), **ys)
+
+
+if __name__ == "__main__":
+    for nm in (sys.argv[1:] or list(CASES)):
+        run_case(nm)
