@@ -42,12 +42,13 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 
 # ----------------------------------------------------------------------------------------------- helpers
 def algorithmic_bytes_per_iter(nnz: int, N: int, n: int, r: int, tall_passes: int = 1) -> float:
-    """HBM bytes one Algorithm-1 loop iteration must move:
-    K and K^T once (8 B value + 4 B index per nonzero), t written and read on all N rows, 14 passes of
-    8 B over the n inactive rows, one mask byte per row, and `tall_passes` passes over an n x r tall-skinny
-    block: ONE (HW_I only) for the default kernel, which carries the projection in coefficient form; two
-    (HW_I and W_I) for the literal recurrence (alg1_variant = 1), which is what SURVEY.md 8(d) counted."""
-    return 24.0 * nnz + 16.0 * N + 112.0 * n + 8.0 * tall_passes * n * r + 1.0 * N
+    """HBM bytes one Algorithm-1 loop iteration must move: the rows of K whose
+    columns reach the inactive set and the rows of K^T in it (8 B value + 4 B index per nonzero: 24 nnz n/N on these
+    stencil operators), t written and read where it can be nonzero (16 N n/N), the mask (N n/N), 14 passes of 8 B over
+    the n inactive rows, and `tall_passes` passes over an n x r tall-skinny block: ONE (H_II Z only) for the default
+    kernel, which carries the projection in coefficient form; two (H_II Z and Z) for the literal recurrence
+    (alg1_variant = 1), which is what SURVEY.md 8(d) counted.  At n = N: 24 nnz + 17 N + 112 N + 8 N r."""
+    return (24.0 * nnz + 17.0 * N) * (n / float(N)) + 112.0 * n + 8.0 * tall_passes * n * r
 
 
 def shard_queries(rank: int, world: int, n_queries: int):
@@ -568,6 +569,63 @@ def run_loop(args):
     return out
 
 
+def run_setup(args):
+    """--mode setup: the once-per-PDAS-step and once-per-sequence parts next to the loop: S1 + S2 (restriction, Gram on the
+    FP64 tensor cores, basis transform, blocked SpMM, k x k factorisation) timed as a whole over --steps repetitions, the
+    FP64 tensor-core peak of the device (probe), and -- with --reference eig -- S0's Chebyshev filter in GB/s
+    (algorithmic bytes 3 nnz + 48 N per column and degree).  Per-kernel times come from an ncu launch list
+    of this command (profiles/)."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    import paper_2606_17971_b200 as pkg
+
+    pkg.load_library()
+    w = make_workload(args)
+    stream = torch.cuda.current_stream()
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap), stream=stream.cuda_stream)
+    peak_tf = g.probe_fp64_tensor_peak()
+    ref = None
+    if args.reference == "eig":
+        _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
+        ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
+    else:
+        build_analytical_reference(g, w)
+        ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
+    act = torch.zeros(w.N, dtype=torch.uint8, device=dev)
+    ms = []
+    info = None
+    for i in range(args.warmup + args.steps):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        info = g.coarse_setup(1, act)
+        e1.record(stream)
+        e1.synchronize()
+        if i >= args.warmup:
+            ms.append(e0.elapsed_time(e1))
+    kp = (w.k + 7) & ~7
+    peak, peak_src = load_peaks()
+    # algorithmic work of S1 + S2 per PDAS step at n = N: restriction 16 N k; two Gram products 2 * 2 N k^2 flop reading
+    # 8 N k (G) and 16 N k (E); transform 2 N k^2 flop, 8 N k read, 16 N k written (column- and tile-major); SpMM
+    # 24 nnz k / 8 + 40 N k
+    flop = 6.0 * w.N * kp * kp
+    nbytes = (16 + 8 + 16 + 24 + 40) * w.N * kp + 3.0 * w.nnz * kp
+    out = {"metric": "coarse setup (S1 + S2) per PDAS step", "value": round(statistics.median(ms), 3), "unit": "ms", "n_gpus": 1,
+           "steps": args.steps, "warmup": args.warmup, "higher_is_better": False, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(args, w), "mode": "setup", "reference": args.reference},
+           "rank": info["rank"], "cond_E": info["cond_E"],
+           "setup_model": {"flop": flop, "bytes": nbytes, "GBs": round(nbytes / (statistics.median(ms) * 1e-3) / 1e9, 1),
+                           "note": "includes the host round trips of rd_coarse_setup (k x k copies out)"},
+           "fp64_tensor_peak_tflops_probe": round(peak_tf, 2), "hbm_peak": peak, "hbm_peak_source": peak_src,
+           "reference": ref}
+    g.close()
+    return out
+
+
 def run_replay(args):
     """--mode replay: the matched-replay protocol of the paper (Table 3 :438-451; NEXT-4 of SURVEY.md 8(f)).
     A query sequence is run once with RefDef under the warm-start policy and every inactive system it meets is
@@ -575,7 +633,8 @@ def run_replay(args):
     initial guesses with direct restriction (eq. (12)), with zero-extension (eq. (13), history accumulating in replay
     order) and with Jacobi-CG, all from the same reference: iterations, retained rank and seconds per transfer, and the
     energy fraction chi of eq. (24) (rd_energy_fraction, x_* = the verified solution of the replayed
-    solve) that the coarse correction removes from a zero initial guess."""
+    solve) that the coarse correction removes from a zero initial guess, and the effective condition number of the
+    Jacobi-scaled deflated operator of eq. (23) (extreme Ritz values of each replayed solve)."""
     import torch
 
     if not torch.cuda.is_available():
@@ -614,9 +673,11 @@ def run_replay(args):
         iters = ranks = 0
         ms = 0.0
         worst = 0.0
-        chis = []
+        chis, kappas = [], []
         for act, b in systems:
             xs, r = g.solve_inactive(METHODS[name], act, b, x0)
+            if r["ritz_min"] > 0.0:
+                kappas.append(r["ritz_max"] / r["ritz_min"])
             iters += r["iters"]
             ranks += r["rank_used"]
             ms += r["t_iter_ms"]
@@ -625,7 +686,11 @@ def run_replay(args):
             chis.append(g.energy_fraction(METHODS[name], act, b, xs)[0])
         out_methods[name] = {"cg_iters": iters, "alg1_s": round(ms * 1e-3, 4), "mean_rank": round(ranks / max(len(systems), 1), 2),
                              "worst_rel_resid": worst, "mean_chi": float(np.mean(chis)) if chis else 0.0,
-                             "min_chi": float(np.min(chis)) if chis else 0.0}
+                             "min_chi": float(np.min(chis)) if chis else 0.0,
+                             # eq. (23): effective condition number of the deflated, Jacobi-preconditioned operator
+                             # (extreme Ritz values of each replayed solve)
+                             "mean_kappa_eff": float(np.mean(kappas)) if kappas else None,
+                             "max_kappa_eff": float(np.max(kappas)) if kappas else None}
     g.close()
     base = out_methods["zeroext"]["cg_iters"]
     return {"metric": "matched replay of the inactive systems of a sequence (PAPER.md:168, Table 3): CG iterations per transfer",
@@ -773,7 +838,7 @@ def build_parser():
     ap.add_argument("--e2e-steps", type=int, default=0, help="host-buffer queries after the timed region; 0 = one full pass of the sequence")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mode", default="query", choices=["query", "loop", "replay"],
+    ap.add_argument("--mode", default="query", choices=["query", "loop", "replay", "setup"],
                     help="query: the metric; loop: the CG loop alone; replay: matched replay of a sequence's inactive systems")
     ap.add_argument("--cg-cap", type=int, default=500000, help="--mode loop: iteration cap of each solve")
     ap.add_argument("--alg1-variant", type=int, default=0, help="rd_options.alg1_variant (0: default kernel; 1: literal recurrence)")
@@ -789,6 +854,8 @@ def main(argv=None):
         out = run_loop(args)
     elif args.mode == "replay":
         out = run_replay(args)
+    elif args.mode == "setup":
+        out = run_setup(args)
     else:
         out = run_ours(args)
     if out is not None:

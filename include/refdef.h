@@ -122,8 +122,16 @@ typedef struct {
                               [2] stage B (K^T product)  [3] grid barrier + reduction  [4] k x k coefficient updates
                               [5] stage C (updates + H_II W_I pass)  [6] grid barrier + reduction  [7] outside the loop;
                               zeros for the other variants */
+    /* eq. (23), alg1_variant 0 through rd_solve_inactive only: extreme Ritz values of the operator the
+     * deflated, Jacobi-preconditioned CG iterates with, D^{-1/2} B P D^{-1/2} = B^ - D^{-1/2} B Z E^{-1} Z^T B D^{-1/2}, from the
+     * Lanczos tridiagonal matrix of the last restart-free run of ritz_count iterations.  They lie inside the nonzero
+     * spectrum of that matrix and converge to its ends: ritz_max / ritz_min estimates the effective condition number.
+     * Zero when nothing was recorded. */
+    double ritz_min, ritz_max;
+    int32_t ritz_count;
     int32_t live_slices_A, live_slices_B; /* S6 compaction: 32-row slices the K product / the K^T product, vector updates
                               and tall-skinny pass of this solve touch (of ceil(N/32)); all others are skipped */
+    int32_t reserved;
 } rd_solve_report;
 
 void rd_default_options(rd_options* opt);
@@ -156,6 +164,15 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
 /* Facts about the last rd_build_reference: block size b, total Chebyshev degree (each degree = one application
  * of H to all b columns), wall milliseconds.  Any pointer may be NULL. */
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms);
+/* Work of the Chebyshev filter of the last rd_build_reference / rd_build_reference_scaled (zeros for the other
+ * constructions): column_applies = the number of (column, degree) pairs H was applied to (locked columns excluded),
+ * filter_ms = CUDA-event time of those applies, bytes_per_column_apply = the algorithmic HBM bytes of one of them,
+ * 3 nnz + 48 N (K and K^T stream once per 8 columns; six vector passes per column).  The filter's GB/s is
+ * column_applies * bytes_per_column_apply / filter_ms.  Any pointer may be NULL. */
+int rd_reference_work(const rd_ctx* ctx, int64_t* column_applies, double* filter_ms, double* bytes_per_column_apply);
+/* Measurement helper: the FP64 tensor-core throughput of this device in TFLOP/s (back-to-back mma.sync m8n8k4 f64 on
+ * registers, best of four timed launches): the denominator for the tensor-pipe share of the S2 Gram kernels. */
+int rd_probe_fp64_tensor_peak(rd_ctx* ctx, double* tflops);
 /* The Jacobi-scaled variant of rd_build_reference (the paper's "generalized eigenproblem M_c phi = mu D_c phi supplies
  * low modes in Jacobi-scaled coordinates ... each column is normalized in the Euclidean norm", here on the
  * fine operator): the k lowest pairs of H w = mu D w, D = diag(H), by the same block method applied to
@@ -182,9 +199,23 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
  * eq. (17); capacity c_0 = 1, W_t = I); the candidate pairs are ordered by (s, i, j) and the k lowest retained;
  * column c of the reference is q_{i,j} (x) phi_i, each q with its largest-magnitude component positive.
  * s_out: host, k doubles (reference eigenvalue nu = h^d (1 + sigma s)), may be NULL.  pairs_out: host, k x (ndim + 1)
- * int32 (q_1..q_d of the spatial mode, then j), may be NULL.  Build time charged to the next query. */
+ * int32 (q_1..q_d of the spatial mode, then j), may be NULL.  Build time charged to the next query.
+ * Stored compactly (rd_reference_storage): the r_s distinct sine products used and the k temporal vectors. */
 int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt,
                                  double* s_out, int32_t* pairs_out);
+/* Complete temporal coverage ("The timed Cartesian trajectories keep all temporal factors of S spatial
+ * modes ... which pairs each retained mode with every time level"; :210): the reference of rd_build_reference_spacetime
+ * restricted to the first S spatial sine modes, ALL nt temporal eigenvectors of each: rank k = S * nt (<= 64, else
+ * RD_EINVAL), columns in the order (s, i, j) as above.  s_out: k doubles, pairs_out: k x (ndim + 1) int32, may be NULL. */
+int rd_build_reference_spacetime_cover(rd_ctx* ctx, int32_t S, int32_t ndim, const int64_t* dims, int32_t nt, double dt,
+                                       double* s_out, int32_t* pairs_out);
+/* How the reference is held ("If the selected pairs use r_s distinct spatial modes, the reference stores
+ * N_s r_s + N_t r floating-point values and r spatial-column indices.  Restriction evaluates a selected product at its
+ * inactive space-time entries.").  kind: -1 none, 0 dense N x k block, 1 compact space-time factors (the two
+ * rd_build_reference_spacetime* calls and rd_build_reference_transient): no dense copy exists on the device, S1 forms
+ * the restricted candidate W_I from the factors and rd_get_reference forms the dense block for the caller only.
+ * n_values: doubles stored (N k, or N_s r_s + N_t k); n_indices: int32 stored (0 or k).  Any pointer may be NULL. */
+int rd_reference_storage(const rd_ctx* ctx, int32_t* kind, int64_t* n_values, int64_t* n_indices);
 /* The paper's coarse-mesh reference (section 2.2.2): "P1 prolongation maps these vectors to the full
  * fine mesh, where each column is normalized in the Euclidean norm."  Wc: N_c x k column-major (ld N_c), host or
  * device: vectors on a coarser Cartesian grid of dims_c cells of the same unit box, typically the Jacobi-scaled low

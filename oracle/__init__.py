@@ -14,6 +14,7 @@ from .oracle import (  # noqa: F401
     prolong_p1,
     prolonged_reference,
     transient_reference,
+    deflated_spectrum,
     JACOBI_CG,
     REFDEF,
     ZEROEXT,

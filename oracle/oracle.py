@@ -386,7 +386,7 @@ def temporal_sign(q):
     return q if q[j] > 0 else -q
 
 
-def spacetime_reference(dims, nt, dt, k):
+def spacetime_reference(dims, nt, dt, k, cover=None):
     """Mode-dependent temporal reference (NEXT-2 of SURVEY.md 8(f)): section 2.2.4, eq. (16)-(17),
     for the backward-Euler all-at-once operator of workloads/ (K_st = I (x) K_s + L (x) M_s, L lower bidiagonal with
     1/dt and -1/dt, capacity c_0 = 1, W_t = I).
@@ -400,11 +400,19 @@ def spacetime_reference(dims, nt, dt, k):
     total space-time rank r.  A fixed ordering resolves repeated eigenvalues": sorted by
     (s, i, j), i the position of the spatial mode in sine_reference's order, j the index of s within S_i ascending.
 
+    cover = S (k is then ignored and set to S nt): complete temporal coverage, "The timed Cartesian
+    trajectories keep all temporal factors of S spatial modes (Table 1), which pairs each retained mode with every time
+    level": every pair (i, j) with i < S, in the same (s, i, j) order.
+
     Layout id = space + N_s * t: column = kron(q, phi).  Returns (pairs, s, W): pairs int (k, d + 1) = (q_1..q_d, j),
     s (k,), W (N_s nt, k) column-major, orthonormal columns."""
     dims = [int(n) for n in dims]
     Ns = int(np.prod(dims))
-    rs = min(k, Ns)
+    if cover is not None:
+        rs = int(cover)
+        k = rs * nt
+    else:
+        rs = min(k, Ns)
     modes, mu, Phi = sine_reference(dims, rs)
     L = (np.eye(nt) - np.eye(nt, k=-1)) / dt
     cand = []
@@ -576,3 +584,38 @@ def transient_reference(Phi, st, nt, k):
         col = np.kron(temporal_sign(Q[i][:, j]), Phi[:, i])
         W[:, c] = col / np.linalg.norm(col)
     return pairs, nus, W
+
+
+def deflated_spectrum(orc: "Oracle", idx, Zt, jacobi: bool = True):
+    """Jacobi-scaled diagnostic of the paper (NEXT-3 of SURVEY.md 8(f)): eq. (23).  "For
+    Jacobi-preconditioned CG, the relevant matrix is B^ = D^{-1/2} B D^{-1/2} and the relevant coarse space is
+    range(D^{1/2} Z) ... We measure the nonzero spectrum of
+        B^ - D^{-1/2} B Z (Z^T B Z)^{-1} Z^T B D^{-1/2}
+    on the small replay systems."  Written out densely: B = H_II from n operator applies on unit vectors, D = diag(B),
+    Z, BZ, E = the factors of the coarse space the oracle builds from the restricted candidate basis Zt (QR + SVD,
+    threshold 1e-12, cond(E) guard), the symmetric n x n matrix above, a library eigensolver.  The
+    matrix has exactly r = rank(Z) zero eigenvalues (it annihilates D^{1/2} Z); they are dropped.
+
+    Returns (lam, r): the n - r nonzero eigenvalues ascending, and r.  The effective condition number that the
+    deflated, Jacobi-preconditioned CG of Algorithm 1 sees is lam[-1] / lam[0].  jacobi = False: D = I.
+    Small systems only (dense n x n)."""
+    idx = np.ascontiguousarray(idx, dtype=np.int64)
+    n = len(idx)
+    B = np.empty((n, n))
+    e = np.zeros(n)
+    for j in range(n):
+        e[j] = 1.0
+        B[:, j] = orc.apply_B(idx, e)
+        e[j] = 0.0
+    B = 0.5 * (B + B.T)
+    cs = orc.coarse(idx, Zt if Zt is not None else np.zeros((n, 0)))
+    r = cs.rank
+    A = B.copy()
+    if r:
+        Z, BZ, E = cs.factors()
+        A -= BZ @ np.linalg.solve(E, BZ.T)
+    if jacobi:
+        s = 1.0 / np.sqrt(np.diag(B))
+        A = A * s[:, None] * s[None, :]
+    lam = np.linalg.eigvalsh(0.5 * (A + A.T))
+    return lam[r:].copy(), r

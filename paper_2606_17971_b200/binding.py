@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
 
 
@@ -54,7 +54,8 @@ class _SolveReport(C.Structure):
     _fields_ = [("iters", C.c_int32), ("rank_used", C.c_int32), ("coarse_fallback", C.c_int32),
                 ("replacements", C.c_int32), ("status", C.c_int32), ("rel_resid_verified", C.c_double),
                 ("cond_E", C.c_double), ("t_iter_ms", C.c_double), ("bytes_per_iter", C.c_double),
-                ("t_stage_us", C.c_double * 8), ("live_slices_A", C.c_int32), ("live_slices_B", C.c_int32)]
+                ("t_stage_us", C.c_double * 8), ("ritz_min", C.c_double), ("ritz_max", C.c_double), ("ritz_count", C.c_int32),
+                ("live_slices_A", C.c_int32), ("live_slices_B", C.c_int32), ("reserved", C.c_int32)]
 
 
 @dataclass
@@ -103,9 +104,13 @@ def load_library(path: Optional[str] = None):
     lib.rd_build_reference_scaled.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
+    lib.rd_build_reference_spacetime_cover.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
+    lib.rd_reference_storage.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(i64)]
     lib.rd_build_reference_prolonged.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.rd_build_reference_transient.argtypes = [vp, i32, i32, i32, vp, vp, vp]
     lib.rd_reference_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), C.POINTER(dbl)]
+    lib.rd_probe_fp64_tensor_peak.argtypes = [vp, C.POINTER(dbl)]
+    lib.rd_reference_work.argtypes = [vp, C.POINTER(i64), C.POINTER(dbl), C.POINTER(dbl)]
     lib.rd_set_reference.argtypes = [vp, i32, vp]
     lib.rd_get_reference.argtypes = [vp, vp, C.POINTER(i32)]
     lib.rd_solve_query.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, C.POINTER(_StepReport), vp, C.POINTER(_QueryReport)]
@@ -251,6 +256,23 @@ class RefDef:
         self.k = k
         return s, pairs
 
+    def build_reference_spacetime_cover(self, S, dims, nt, dt):
+        """Complete temporal coverage: all nt temporal factors of the first S spatial modes, k = S nt."""
+        dims = np.ascontiguousarray(dims, dtype=np.int64)
+        k = S * nt
+        s = np.zeros(k)
+        pairs = np.zeros((k, len(dims) + 1), dtype=np.int32)
+        self._check(self._lib.rd_build_reference_spacetime_cover(self._h, S, len(dims), dims.ctypes.data, nt, dt, s.ctypes.data,
+                                                                 pairs.ctypes.data), "rd_build_reference_spacetime_cover")
+        self.k = k
+        return s, pairs
+
+    def reference_storage(self):
+        """(kind, doubles stored, int32 stored): kind -1 none, 0 dense, 1 compact space-time factors."""
+        kind, nv, ni = C.c_int32(0), C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.rd_reference_storage(self._h, C.byref(kind), C.byref(nv), C.byref(ni)), "rd_reference_storage")
+        return kind.value, nv.value, ni.value
+
     def build_reference_prolonged(self, Wc, dims_c, dims_f):
         """Coarse-mesh reference: P1 prolongation of Wc (N_c x k numpy, or a column-major device tensor of
         shape (k, N_c)) from the grid dims_c to the grid dims_f, unit columns.  Returns the norms before normalisation."""
@@ -291,7 +313,19 @@ class RefDef:
     def reference_info(self):
         b, deg, ms = C.c_int32(0), C.c_int64(0), C.c_double(0)
         self._check(self._lib.rd_reference_info(self._h, C.byref(b), C.byref(deg), C.byref(ms)), "rd_reference_info")
-        return dict(block=b.value, total_degree=deg.value, build_ms=ms.value)
+        ca, fms, bpc = C.c_int64(0), C.c_double(0), C.c_double(0)
+        self._check(self._lib.rd_reference_work(self._h, C.byref(ca), C.byref(fms), C.byref(bpc)), "rd_reference_work")
+        d = dict(block=b.value, total_degree=deg.value, build_ms=ms.value)
+        if ca.value > 0 and fms.value > 0:
+            # S0's Chebyshev filter: algorithmic bytes (3 nnz + 48 N per column and degree) over its CUDA-event time
+            d.update(filter_column_applies=ca.value, filter_ms=fms.value, filter_bytes_per_column_apply=bpc.value,
+                     filter_GBs=ca.value * bpc.value / (fms.value * 1e-3) / 1e9)
+        return d
+
+    def probe_fp64_tensor_peak(self):
+        t = C.c_double(0)
+        self._check(self._lib.rd_probe_fp64_tensor_peak(self._h, C.byref(t)), "rd_probe_fp64_tensor_peak")
+        return t.value
 
     def set_reference(self, W):
         """W: N x k, numpy (any order; copied column-major) or a column-major device tensor of shape (k, N)."""

@@ -49,6 +49,8 @@ struct CgParams {
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]
     GridBarrier* bar;
+    double2* coef;        // NULL or coef_cap entries: (a_it, beta_it) of every loop iteration (CG-Lanczos coefficients; eq. (23) diagnostic)
+    int32_t coef_cap;
     int32_t hw_res_tiles; // tiles per CTA of the H_II W_I stream requested with L2 evict_last (kept resident)
     CgDevReport* rep;
 };

@@ -715,6 +715,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
         if (!(pw > 0.0) || !(rho > 0.0)) { status = RD_ENOTSPD_DEV; break; }
         // line 10
         const double a = rho / pw;
+        if (P.coef && blockIdx.x == 0 && threadIdx.x == 0 && iters <= P.coef_cap) P.coef[iters - 1] = make_double2(a, beta);
         if (coarse) {
             cta.coef_step(a);
             x_split = true;

@@ -195,6 +195,25 @@ __global__ void __launch_bounds__(256) k_gram_dmma(int64_t N, int p, int q, cons
     }
 }
 
+// Measurement helper (no arithmetic of the method): back-to-back m8n8k4 FP64 tensor-core operations on registers, eight
+// independent accumulator tiles per warp -- the peak the Gram kernels' tensor-pipe utilisation is quoted against.
+__global__ void __launch_bounds__(256) k_dmma_peak_probe(int iters, double seed, double* sink)
+{
+    double acc[8][2];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) acc[t][0] = acc[t][1] = 0.0;
+    double a = seed + 1e-3 * (threadIdx.x & 31), b = seed - 1e-3 * (threadIdx.x & 7);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int t = 0; t < 8; ++t) dmma_m8n8k4(acc[t][0], acc[t][1], a, b);
+        a = -a;  // keeps the accumulators bounded
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int t = 0; t < 8; ++t) s += acc[t][0] + acc[t][1];
+    if (s == 123.456) sink[0] = s;  // never true: keeps the loop alive
+}
+
 // out[e] = sum over parts of part[part][e], fixed order (deterministic)
 __global__ void k_reduce_parts(int nparts, int64_t len, const double* parts, double* out)
 {
@@ -298,6 +317,94 @@ __global__ void __launch_bounds__(1024) k_coarse_E(int kp, const double* Eraw, c
     cta_matmul(n, n, r, A4, 1, n, T, n, 1, CW, n);           // CW = T E^{-1} T^T (n x n)
     cta_symmetrize(CW, n, n);
     if (threadIdx.x == 0) { info->fallback = 0; info->cond_E = cond; }
+}
+
+// ---------------------------------------------------------------- eq. (23): spectrum the deflated, Jacobi-preconditioned CG sees
+// The step lengths a_j and direction coefficients beta_j of a CG run define the Lanczos tridiagonal matrix of the
+// operator CG iterates with -- for Algorithm 1 that is D^{-1/2} B P D^{-1/2} = B^ - D^{-1/2} B Z E^{-1} Z^T B D^{-1/2}, the
+// matrix of eq. (23), on the complement of its null space:
+//     T_jj = 1/a_j + beta_j / a_{j-1},    T_{j,j-1} = sqrt(beta_j) / a_{j-1}        (beta = 0 where the direction restarts)
+// Its eigenvalues (Ritz values) lie inside the nonzero spectrum and the extreme ones converge to its ends.  One CTA:
+// the last restart-free segment of the m recorded pairs, extreme eigenvalues by multisection on Sturm counts.
+// out[0] = smallest, out[1] = largest Ritz value, out[2] = segment length.
+__global__ void __launch_bounds__(1024) k_ritz_extremes(int m, const double2* coef, double* out)
+{
+    __shared__ int s_start;
+    __shared__ double s_lo[2], s_hi[2];
+    __shared__ int s_pick[2];
+    if (threadIdx.x == 0) {
+        int st = 0;
+        for (int j = m - 1; j > 0; --j)
+            if (coef[j].y == 0.0) { st = j; break; }
+        // a trailing restart (the replacement branch that ends a solve) leaves a segment of length one: take the one before
+        if (m - st < 3) {
+            const int end = st;
+            st = 0;
+            for (int j = end - 1; j > 0; --j)
+                if (coef[j].y == 0.0) { st = j; break; }
+            m = end;
+        }
+        s_start = st;
+        s_pick[0] = m;  // reuse: segment end
+    }
+    __syncthreads();
+    const int j0 = s_start, j1 = s_pick[0], len = j1 - j0;
+    __syncthreads();
+    if (len < 1) {
+        if (threadIdx.x == 0) { out[0] = 0.0; out[1] = 0.0; out[2] = 0.0; }
+        return;
+    }
+    auto diag = [&](int j) { return 1.0 / coef[j].x + (j > j0 ? coef[j].y / coef[j - 1].x : 0.0); };
+    auto off2 = [&](int j) { return coef[j].y / (coef[j - 1].x * coef[j - 1].x); };  // T_{j,j-1}^2, j > j0
+    if (threadIdx.x == 0) {  // Gershgorin bounds
+        double lo = 1e300, hi = -1e300;
+        for (int j = j0; j < j1; ++j) {
+            const double d = diag(j);
+            const double r = (j > j0 ? sqrt(off2(j)) : 0.0) + (j + 1 < j1 ? sqrt(off2(j + 1)) : 0.0);
+            lo = fmin(lo, d - r);
+            hi = fmax(hi, d + r);
+        }
+        lo = fmax(lo, 0.0);  // the operator is positive semidefinite
+        s_lo[0] = s_lo[1] = lo;
+        s_hi[0] = s_hi[1] = hi * (1.0 + 1e-12) + 1e-300;
+    }
+    __syncthreads();
+    // number of eigenvalues of T below x (Sturm sequence of the LDL^T pivots)
+    auto count_below = [&](double x) {
+        int cnt = 0;
+        double q = 1.0;
+        for (int j = j0; j < j1; ++j) {
+            q = diag(j) - x - (j > j0 ? off2(j) / q : 0.0);
+            if (q == 0.0) q = -1e-300;
+            cnt += q < 0.0;
+        }
+        return cnt;
+    };
+    for (int which = 0; which < 2; ++which) {  // 0: smallest (first x with count >= 1), 1: largest (first x with count >= len)
+        const int want = which == 0 ? 1 : len;
+        for (int round = 0; round < 7; ++round) {
+            const double lo = s_lo[which], hi = s_hi[which];
+            const double x = lo + (hi - lo) * (double)(threadIdx.x + 1) / (double)(blockDim.x + 1);
+            const bool ok = count_below(x) >= want;
+            if (threadIdx.x == 0) s_pick[1] = blockDim.x;
+            __syncthreads();
+            if (ok) atomicMin(&s_pick[1], (int)threadIdx.x);
+            __syncthreads();
+            const int t = s_pick[1];
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const double w = (hi - lo) / (double)(blockDim.x + 1);
+                s_lo[which] = lo + w * t;          // count(lo + w t) < want (or t = 0: lo itself)
+                s_hi[which] = lo + w * (t + 1);    // count >= want (or t = blockDim: hi itself)
+            }
+            __syncthreads();
+        }
+    }
+    if (threadIdx.x == 0) {
+        out[0] = 0.5 * (s_lo[0] + s_hi[0]);
+        out[1] = 0.5 * (s_lo[1] + s_hi[1]);
+        out[2] = (double)len;
+    }
 }
 
 // ---------------------------------------------------------------- eq. (24): energy fraction of the coarse correction

@@ -73,6 +73,19 @@ struct rd_ctx {
     uint8_t* sflags = nullptr;
     int32_t *listA = nullptr, *listB = nullptr, *d_live = nullptr;
     int32_t* h_live = nullptr;
+    // compact (Kronecker-factored) reference: W[x + Ns t, c] = kQc[t + nt c] * kPhi[x + Ns ksp[c]]
+    bool have_ref = false;
+    int ref_kind = 0;  // 0: dense N x k block in W; 1: factors (kPhi, kQc, ksp), no dense copy is kept
+    double *kPhi = nullptr, *kQc = nullptr;
+    int32_t* ksp = nullptr;
+    int64_t kNs = 0, kPhi_cap = 0;
+    int knt = 0, krs = 0, kQc_cap = 0;
+    int work_kp = 0;   // padded rank the work buffers (Wm, Zm, ...) were allocated for
+    int dense_kp = 0;  // padded rank the dense block W was allocated for
+    double2* coef = nullptr;  // CG-Lanczos coefficients of the last rd_solve_inactive (eq. (23) diagnostic)
+    int32_t coef_cap = 0;
+    bool want_ritz = false;
+    double* d_ritz = nullptr;
     double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;  // EW: W_I^T H W_I on request
     double *T = nullptr, *Eraw = nullptr, *E = nullptr, *CW = nullptr;  // T (W_I -> Z), E = Z^T B Z, C = E^{-1}, CW = T C T^T
     int gram_nparts = 0;
@@ -91,6 +104,8 @@ struct rd_ctx {
     double ref_ms_pending = 0.0, ref_ms_last = 0.0;
     int64_t ref_degree = 0;  // total Chebyshev degree of the last rd_build_reference
     int ref_block = 0;       // its block size b
+    int64_t ref_col_applies = 0;  // sum over filter degrees of the columns H was applied to (locked columns excluded)
+    double ref_filter_ms = 0.0;   // CUDA-event time of all filter applies of the last build
     int64_t launches = 0;  // kernels launched so far (rd_kernel_launches)
 };
 
@@ -264,31 +279,42 @@ int launch_apply_H(rd_ctx* ctx, const double* v, const uint8_t* act, double* out
     return RD_OK;
 }
 
-int alloc_reference(rd_ctx* ctx, int k)
+// Buffers for a reference of k columns: the work blocks of S1 / S2 always; the dense N x k block W only for the dense
+// kind (a compact reference never materialises it).  Buffers of an earlier, smaller reference stay allocated until destroy.
+int alloc_reference(rd_ctx* ctx, int k, bool need_dense = true)
 {
     const int kp = (k + 7) & ~7;
-    if (ctx->kp >= kp && ctx->W) { ctx->k = k; return RD_OK; }
-    // (buffers of an earlier, smaller reference stay allocated until destroy)
     const size_t nk = (size_t)ctx->ldw * kp;
-    RDTRY(dalloc(ctx, &ctx->W, nk));
-    RDTRY(dalloc(ctx, &ctx->Wm, nk));
-    RDTRY(dalloc(ctx, &ctx->Zm, nk));
-    RDTRY(dalloc(ctx, &ctx->HZm, nk));
-    RDTRY(dalloc(ctx, &ctx->Zt, nk));   // tile-major copies (k_alg1_v3); pad rows stay zero
-    RDTRY(dalloc(ctx, &ctx->HZt, nk));
-    RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
-    ctx->gram_nparts = ctx->num_sms * 2;
-    RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
-    RDTRY(dalloc(ctx, &ctx->G, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->EW, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->cwork, (size_t)6 * kp * kp));
-    RDTRY(dalloc(ctx, &ctx->C, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->T, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->Eraw, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->E, (size_t)kp * kp));
-    RDTRY(dalloc(ctx, &ctx->CW, (size_t)kp * kp));
+    if (ctx->work_kp < kp) {
+        RDTRY(dalloc(ctx, &ctx->Wm, nk));
+        RDTRY(dalloc(ctx, &ctx->Zm, nk));
+        RDTRY(dalloc(ctx, &ctx->HZm, nk));
+        RDTRY(dalloc(ctx, &ctx->Zt, nk));   // tile-major copies (k_alg1_v3); pad rows stay zero
+        RDTRY(dalloc(ctx, &ctx->HZt, nk));
+        RDTRY(dalloc(ctx, &ctx->Tchunk, (size_t)ctx->ldw * 8));
+        ctx->gram_nparts = ctx->num_sms * 2;
+        RDTRY(dalloc(ctx, &ctx->gram_parts, (size_t)ctx->gram_nparts * kp * kp));
+        RDTRY(dalloc(ctx, &ctx->G, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->EW, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->cwork, (size_t)6 * kp * kp));
+        RDTRY(dalloc(ctx, &ctx->C, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->T, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->Eraw, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->E, (size_t)kp * kp));
+        RDTRY(dalloc(ctx, &ctx->CW, (size_t)kp * kp));
+        ctx->work_kp = kp;
+    } else if (ctx->kp != kp) {
+        // a narrower reference in wider buffers: the tile-major blocks are addressed with the new kp; clear the old layout
+        CU(cudaMemsetAsync(ctx->Zt, 0, (size_t)ctx->ldw * ctx->work_kp * sizeof(double), ctx->stream));
+        CU(cudaMemsetAsync(ctx->HZt, 0, (size_t)ctx->ldw * ctx->work_kp * sizeof(double), ctx->stream));
+    }
+    if (need_dense && ctx->dense_kp < kp) {
+        RDTRY(dalloc(ctx, &ctx->W, nk));
+        ctx->dense_kp = kp;
+    }
     ctx->k = k;
     ctx->kp = kp;
+    ctx->have_ref = false;  // the caller sets it once the reference is in place
     return RD_OK;
 }
 
@@ -300,8 +326,12 @@ int coarse_setup(rd_ctx* ctx, int method, float* ms_restrict, float* ms_coarse, 
     const int kp = ctx->kp;
     const bool tiles = ctx->opt.alg1_variant == 0;
     CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-    k_restrict<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
-        N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
+    if (ctx->ref_kind == 1)  // compact reference: the selected products are evaluated at the inactive entries
+        k_restrict_kron<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+            ctx->kNs, ctx->knt, ctx->ldw, ctx->k, kp, ctx->kPhi, ctx->kQc, ctx->ksp, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
+    else
+        k_restrict<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+            N, ctx->ldw, ctx->k, kp, ctx->W, ctx->act, ctx->hist, method == RD_ZEROEXT ? 1 : 0, ctx->Wm);
     ctx->launches++;
     CU(cudaEventRecord(ctx->ev[1], ctx->stream));
     const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
@@ -353,7 +383,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     if (ms_coarse) *ms_coarse = 0;
     int use_coarse = 0;
     if (method != RD_JACOBI_CG) {
-        if (!ctx->W || ctx->k <= 0) return fail(ctx, RD_ENOREF, "method %d needs a reference (rd_build_reference / rd_set_reference)", method);
+        if (!ctx->have_ref || ctx->k <= 0) return fail(ctx, RD_ENOREF, "method %d needs a reference (rd_build_reference / rd_set_reference)", method);
         RDTRY(coarse_setup(ctx, method, ms_restrict, ms_coarse));
         rep->rank_used = ctx->h_cinfo->rank;
         rep->coarse_fallback = ctx->h_cinfo->fallback;
@@ -395,6 +425,16 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
         CU(cudaMemcpyAsync(ctx->h_live, ctx->d_live, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
         P.listA = ctx->listA; P.listB = ctx->listB; P.live_counts = ctx->d_live; P.Wt = ctx->Zt;
     }
+    if (ctx->want_ritz && variant == 0) {  // eq. (23) diagnostic (rd_solve_inactive): record (a, beta) of every iteration
+        const int32_t want = (int32_t)std::min<int64_t>(std::max(ctx->opt.cg_cap, 1), 1 << 20);
+        if (ctx->coef_cap < want) {
+            RDTRY(dalloc(ctx, &ctx->coef, (size_t)want));
+            if (!ctx->d_ritz) RDTRY(dalloc(ctx, &ctx->d_ritz, 4));
+            ctx->coef_cap = want;
+        }
+        P.coef = ctx->coef;
+        P.coef_cap = ctx->coef_cap;
+    }
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
@@ -419,10 +459,19 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     // 14 vector passes over the n inactive rows, the two n x r passes over HW_I and W_I, the mask.
     const double rnk = use_coarse ? (double)rep->rank_used : 0.0;
     // k_alg1_v3 (default) passes over HW_I only: 8 n r instead of 16 n r.
-    rep->bytes_per_iter = 24.0 * (double)ctx->nnz + 16.0 * (double)N + 112.0 * (double)n_inactive +
-                          (variant == 0 ? 8.0 : 16.0) * (double)n_inactive * rnk + (double)N;
+    rep->bytes_per_iter = (24.0 * (double)ctx->nnz + 17.0 * (double)N) * ((double)n_inactive / (double)N) + 112.0 * (double)n_inactive +
+                          (variant == 0 ? 8.0 : 16.0) * (double)n_inactive * rnk;
     rep->live_slices_A = ctx->h_live[0];
     rep->live_slices_B = ctx->h_live[1];
+    if (P.coef && rep->iters > 0) {
+        double h[3];
+        k_ritz_extremes<<<1, 1024, 0, ctx->stream>>>(std::min(rep->iters, ctx->coef_cap), ctx->coef, ctx->d_ritz);
+        ctx->launches++;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(h, ctx->d_ritz, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        rep->ritz_min = h[0]; rep->ritz_max = h[1]; rep->ritz_count = (int32_t)h[2];
+    }
     return RD_OK;
 }
 
@@ -463,6 +512,32 @@ void select_sine_modes(int ndim, const int64_t* dims, int count, std::vector<Sin
     });
     cand.resize(std::min<size_t>(cand.size(), (size_t)count));
     if (qmax_out) *qmax_out = qmax;
+}
+
+// Stores a compact reference: Phi_used (Ns x rs_used, device, column-major ld Ns) is copied into the
+// context; Qc (nt x k) and sp (k) are packed from the per-vector temporal eigenvectors Q[(i * nt + j) * nt + t] and the
+// selection sel (k pairs (i, j)); cols[] lists the rs_used distinct spatial indices i in the order of Phi_used's columns.
+int store_kron(rd_ctx* ctx, int k, int64_t Ns, int nt, int rs_used, const double* d_Phi_used, const std::vector<int32_t>& cols,
+               const int32_t* d_sel, const double* d_Q, int normalise, const double* d_phin2)
+{
+    const int64_t need_phi = Ns * rs_used;
+    if (ctx->kPhi_cap < need_phi) { RDTRY(dalloc(ctx, &ctx->kPhi, (size_t)need_phi, false)); ctx->kPhi_cap = need_phi; }
+    if (ctx->kQc_cap < nt * k) {
+        RDTRY(dalloc(ctx, &ctx->kQc, (size_t)nt * k, false));
+        RDTRY(dalloc(ctx, &ctx->ksp, (size_t)k + RD_MAX_K, false));
+        ctx->kQc_cap = nt * k;
+    }
+    CU(cudaMemcpyAsync(ctx->kPhi, d_Phi_used, (size_t)need_phi * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    int32_t* d_cols = ctx->ksp + k;  // scratch behind sp
+    CU(cudaMemcpyAsync(d_cols, cols.data(), (size_t)rs_used * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+    k_kron_pack<<<1, RD_MAX_K, 0, ctx->stream>>>(nt, k, rs_used, d_cols, d_sel, d_Q, normalise, d_phin2, ctx->kQc, ctx->ksp);
+    ctx->launches++;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->kNs = Ns; ctx->knt = nt; ctx->krs = rs_used;
+    ctx->ref_kind = 1;
+    ctx->have_ref = true;
+    return RD_OK;
 }
 
 }  // namespace
@@ -765,7 +840,11 @@ int rd_build_reference_prolonged(rd_ctx* ctx, int32_t k, int32_t ndim, const int
             ctx->k = 0;  // no usable reference
             return fail(ctx, RD_EINVAL, "column %d of the prolonged reference has norm %g", c, norms[c]);
         }
+    ctx->have_ref = true;
+    ctx->ref_kind = 0;
     ctx->ref_degree = 0;
+    ctx->ref_col_applies = 0;
+    ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
@@ -780,6 +859,8 @@ int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W)
     CU(cudaMemcpy2DAsync(ctx->W, ctx->ldw * sizeof(double), W, ctx->N * sizeof(double), ctx->N * sizeof(double), k,
                          cudaMemcpyDefault, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_ref = true;
+    ctx->ref_kind = 0;
     ctx->ref_ms_pending = 0.0;
     return RD_OK;
 }
@@ -787,12 +868,31 @@ int rd_set_reference(rd_ctx* ctx, int32_t k, const double* W)
 int rd_get_reference(rd_ctx* ctx, double* W_out, int32_t* k_out)
 {
     if (!ctx) return RD_EINVAL;
-    if (k_out) *k_out = ctx->W ? ctx->k : 0;
-    if (W_out && ctx->W && ctx->k > 0) {
-        CU(cudaMemcpy2DAsync(W_out, ctx->N * sizeof(double), ctx->W, ctx->ldw * sizeof(double), ctx->N * sizeof(double), ctx->k,
-                             cudaMemcpyDefault, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));
+    if (k_out) *k_out = ctx->have_ref ? ctx->k : 0;
+    if (!W_out || !ctx->have_ref || ctx->k <= 0) return RD_OK;
+    if (ctx->ref_kind == 1) {  // compact reference: the dense block is formed for the caller only
+        double* dst = W_out;
+        double* tmp = nullptr;
+        if (!is_device_ptr(W_out)) {
+            if (cudaMalloc(&tmp, (size_t)ctx->N * ctx->k * sizeof(double)) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(ctx, RD_ENOMEM, "cudaMalloc of the dense copy of a compact reference");
+            }
+            dst = tmp;
+        }
+        k_kron_dense<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(ctx->kNs, ctx->knt, ctx->N, ctx->k, ctx->kPhi,
+                                                                                           ctx->kQc, ctx->ksp, dst);
+        ctx->launches++;
+        cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(W_out, tmp, (size_t)ctx->N * ctx->k * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (tmp) cudaFree(tmp);
+        if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "rd_get_reference: %s", cudaGetErrorString(e));
+        return RD_OK;
     }
+    CU(cudaMemcpy2DAsync(W_out, ctx->N * sizeof(double), ctx->W, ctx->ldw * sizeof(double), ctx->N * sizeof(double), ctx->k,
+                         cudaMemcpyDefault, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
     return RD_OK;
 }
 
@@ -852,6 +952,8 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     if (!(beta > 0.0) || !std::isfinite(beta)) return fail(ctx, RD_ENOTSPD, "spectrum bound %g", beta);
     beta *= 1.0 + 1e-10;
 
+    int64_t col_applies = 0;
+    float filter_ms = 0.0f;
     // columns [col0, b) of the block (col0 a multiple of the chunk width): the leading col0 columns are locked
     auto block_apply = [&](const double* Y, double c1, double cshift, double c2, const double* Yprev, double* Ynext, int col0 = 0) {
         const int nch = nchunk - col0 / RD_EIG_CB;
@@ -861,6 +963,7 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
         k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o,
                                                    Yprev ? Yprev + o : nullptr, Ynext + o);
         ctx->launches += 2;
+        col_applies += (int64_t)nch * RD_EIG_CB;
     };
     auto gram = [&](const double* A, const double* B, double* out) {
         k_gram_dmma<<<ggram, 256, 0, ctx->stream>>>(N, b, b, A, ld, B, ld, parts);
@@ -939,12 +1042,20 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
         while (nlock < k && resid[nlock] <= tol) ++nlock;
         nlock = std::min((nlock / RD_EIG_CB) * RD_EIG_CB, b - RD_EIG_CB);
         const double* Xlocked = Y0;
+        CU(cudaEventRecord(ctx->ev[0], ctx->stream));
         block_apply(Y0, sg / e, c, 0.0, nullptr, Y1, nlock);
         for (int j = 2; j <= deg; ++j) {
             const double sn = 1.0 / (tau - sg);
             block_apply(Y1, 2.0 * sn / e, c, -sg * sn, Y0, Y2, nlock);
             double* tmp = Y0; Y0 = Y1; Y1 = Y2; Y2 = tmp;
             sg = sn;
+        }
+        CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+        CU(cudaEventSynchronize(ctx->ev[1]));
+        {
+            float ms1 = 0.0f;
+            CU(cudaEventElapsedTime(&ms1, ctx->ev[0], ctx->ev[1]));
+            filter_ms += ms1;
         }
         if (nlock > 0 && Y1 != Xlocked)
             CU(cudaMemcpyAsync(Y1, Xlocked, (size_t)nlock * ld * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
@@ -956,11 +1067,15 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     CU(cudaMemsetAsync(ctx->W, 0, (size_t)ld * ctx->kp * sizeof(double), ctx->stream));
     CU(cudaMemcpyAsync(ctx->W, P[cur], (size_t)ld * k * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    ctx->have_ref = true;
+    ctx->ref_kind = 0;
     if (theta_out) memcpy(theta_out, theta.data(), k * sizeof(double));
     if (resid_out) memcpy(resid_out, resid.data(), k * sizeof(double));
     if (iters_out) *iters_out = sweeps;
     ctx->ref_degree = total_degree;
     ctx->ref_block = b;
+    ctx->ref_col_applies = col_applies;
+    ctx->ref_filter_ms = filter_ms;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
     if (status != RD_OK) fail(ctx, status, "reference not converged to tol %g in %d sweeps (worst residual %g)", tol, sweeps,
@@ -1013,17 +1128,22 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
     cudaFree(d_modes);
     cudaFree(d_tab);
     if (e != cudaSuccess) return fail(ctx, RD_ECUDA, "sine reference: %s", cudaGetErrorString(e));
+    ctx->have_ref = true;
+    ctx->ref_kind = 0;
     ctx->ref_degree = 0;
+    ctx->ref_col_applies = 0;
+    ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
     return RD_OK;
 }
 
-int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt, double* s_out,
-                                 int32_t* pairs_out)
+// Shared by rd_build_reference_spacetime (ordered selection of k pairs among the first min(k, N_s) spatial modes) and
+// rd_build_reference_spacetime_cover (every temporal factor of the first S spatial modes, k = S nt).
+static int build_spacetime(rd_ctx* ctx, int32_t k, int32_t pool, int32_t ndim, const int64_t* dims, int32_t nt, double dt, double* s_out,
+                           int32_t* pairs_out)
 {
-    if (!ctx || !dims || k < 1 || k > RD_MAX_K || ndim < 1 || ndim > 3 || nt < 1 || nt > RD_DENSE_MAXN || !(dt > 0.0)) return RD_EINVAL;
     int64_t Ns = 1;
     for (int a = 0; a < ndim; ++a) {
         if (dims[a] < 1 || dims[a] > (1 << 20)) return fail(ctx, RD_EINVAL, "dims[%d] = %lld", a, (long long)dims[a]);
@@ -1032,8 +1152,9 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     if (Ns * nt != ctx->N) return fail(ctx, RD_EINVAL, "product of dims x nt = %lld is not N = %lld", (long long)(Ns * nt), (long long)ctx->N);
     if (k > ctx->N) return fail(ctx, RD_EINVAL, "k = %d exceeds N = %lld", k, (long long)ctx->N);
     const auto t_begin = std::chrono::steady_clock::now();
-    // ---- the first min(k, N_s) spatial modes and their Laplacian eigenvalues
-    const int rs = (int)std::min<int64_t>(k, Ns);
+    // ---- the candidate spatial modes and their Laplacian eigenvalues
+    const int rs = (int)std::min<int64_t>(pool, Ns);
+    if ((int64_t)k > (int64_t)rs * nt) return fail(ctx, RD_EINVAL, "k = %d exceeds the %d x %d candidates", k, rs, nt);
     int qmax = 1;
     std::vector<SineCand> cand;
     select_sine_modes(ndim, dims, rs, cand, &qmax);
@@ -1043,7 +1164,7 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
         for (int a = 0; a < 3; ++a) modes[(size_t)i * 3 + a] = cand[i].q[a];
         mu[i] = cand[i].mu;
     }
-    RDTRY(alloc_reference(ctx, k));
+    RDTRY(alloc_reference(ctx, k, /*need_dense=*/false));
     int nmax = 1;
     for (int a = 0; a < ndim; ++a) nmax = std::max<int>(nmax, (int)dims[a]);
     const size_t tab_count = (size_t)ndim * qmax * nmax, tt = (size_t)rs * nt * nt;
@@ -1057,8 +1178,8 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
         return RD_OK;
     };
     int32_t *d_modes = nullptr, *d_sel = nullptr;
-    double *d_tab = nullptr, *d_mu = nullptr, *d_A = nullptr, *d_V = nullptr, *d_s = nullptr, *d_Q = nullptr;
-    RDTRY(salloc((void**)&d_modes, modes.size() * sizeof(int32_t)));
+    double *d_tab = nullptr, *d_mu = nullptr, *d_A = nullptr, *d_V = nullptr, *d_s = nullptr, *d_Q = nullptr, *d_Phi = nullptr;
+    RDTRY(salloc((void**)&d_modes, (size_t)RD_MAX_K * 3 * sizeof(int32_t)));
     RDTRY(salloc((void**)&d_sel, (size_t)2 * k * sizeof(int32_t)));
     RDTRY(salloc((void**)&d_tab, tab_count * sizeof(double)));
     RDTRY(salloc((void**)&d_mu, rs * sizeof(double)));
@@ -1066,7 +1187,6 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     RDTRY(salloc((void**)&d_V, tt * sizeof(double)));
     RDTRY(salloc((void**)&d_s, (size_t)rs * nt * sizeof(double)));
     RDTRY(salloc((void**)&d_Q, tt * sizeof(double)));
-    CU(cudaMemcpyAsync(d_modes, modes.data(), modes.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(d_mu, mu.data(), rs * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     const int n0 = (int)dims[0], n1 = ndim > 1 ? (int)dims[1] : 1, n2 = ndim > 2 ? (int)dims[2] : 1;
     k_sine_tables<<<grid_for((int64_t)tab_count, kThreads, 1024), kThreads, 0, ctx->stream>>>(ndim, qmax, nmax, n0, n1, n2, d_tab);
@@ -1077,7 +1197,8 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     CU(cudaMemcpyAsync(s_all.data(), d_s, s_all.size() * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     // ---- ordered selection of the k lowest pairs: (s, i, j) ("order the candidate pairs by nu ... A
-    // fixed ordering resolves repeated eigenvalues"; nu = h^d (1 + alpha s) is increasing in s)
+    // fixed ordering resolves repeated eigenvalues"; nu = h^d (1 + alpha s) is increasing in s).  With k = rs * nt
+    // (complete coverage) every pair is kept, in the same order.
     struct Pair { double s; int i, j; };
     std::vector<Pair> pr;
     pr.reserve(s_all.size());
@@ -1088,26 +1209,62 @@ int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int
         if (x.i != y.i) return x.i < y.i;
         return x.j < y.j;
     });
-    std::vector<int32_t> sel((size_t)2 * k);
+    std::vector<int32_t> sel((size_t)2 * k), cols;
     for (int c = 0; c < k; ++c) {
         sel[2 * c] = pr[c].i;
         sel[2 * c + 1] = pr[c].j;
+        if (std::find(cols.begin(), cols.end(), pr[c].i) == cols.end()) cols.push_back(pr[c].i);
         if (s_out) s_out[c] = pr[c].s;
         if (pairs_out) {
             for (int a = 0; a < ndim; ++a) pairs_out[(size_t)c * (ndim + 1) + a] = modes[(size_t)pr[c].i * 3 + a];
             pairs_out[(size_t)c * (ndim + 1) + ndim] = pr[c].j;
         }
     }
+    std::sort(cols.begin(), cols.end());
+    const int rs_used = (int)cols.size();  // r_s: the distinct spatial modes the selected pairs use
+    // ---- the compact reference: Phi (N_s x r_s: the selected sine products), Qc (nt x k), sp (k)
+    std::vector<int32_t> used_modes((size_t)rs_used * 3);
+    for (int q = 0; q < rs_used; ++q)
+        for (int a = 0; a < 3; ++a) used_modes[(size_t)q * 3 + a] = modes[(size_t)cols[q] * 3 + a];
+    RDTRY(salloc((void**)&d_Phi, (size_t)Ns * rs_used * sizeof(double)));
+    CU(cudaMemcpyAsync(d_modes, used_modes.data(), used_modes.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaMemcpyAsync(d_sel, sel.data(), sel.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
-    k_kron_product<<<grid_for(ctx->N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(Ns, nt, ctx->ldw, ndim, qmax, nmax, n0, n1, k, ctx->kp,
-                                                                                           d_modes, d_sel, d_tab, d_Q, ctx->W);
+    k_sine_product<<<grid_for(Ns, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(Ns, Ns, ndim, qmax, nmax, n0, n1, rs_used, rs_used, d_modes,
+                                                                                      d_tab, d_Phi);
     ctx->launches++;
     CU(cudaGetLastError());
-    CU(cudaStreamSynchronize(ctx->stream));
+    RDTRY(store_kron(ctx, k, Ns, nt, rs_used, d_Phi, cols, d_sel, d_Q, /*normalise=*/0, nullptr));
     ctx->ref_degree = 0;
+    ctx->ref_col_applies = 0;
+    ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
+    return RD_OK;
+}
+
+int rd_build_reference_spacetime(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t* dims, int32_t nt, double dt, double* s_out,
+                                 int32_t* pairs_out)
+{
+    if (!ctx || !dims || k < 1 || k > RD_MAX_K || ndim < 1 || ndim > 3 || nt < 1 || nt > RD_DENSE_MAXN || !(dt > 0.0)) return RD_EINVAL;
+    return build_spacetime(ctx, k, /*pool=*/k, ndim, dims, nt, dt, s_out, pairs_out);
+}
+
+int rd_build_reference_spacetime_cover(rd_ctx* ctx, int32_t S, int32_t ndim, const int64_t* dims, int32_t nt, double dt, double* s_out,
+                                       int32_t* pairs_out)
+{
+    if (!ctx || !dims || S < 1 || ndim < 1 || ndim > 3 || nt < 1 || nt > RD_DENSE_MAXN || !(dt > 0.0)) return RD_EINVAL;
+    if ((int64_t)S * nt > RD_MAX_K) return fail(ctx, RD_EINVAL, "S x nt = %lld exceeds the rank limit %d", (long long)S * nt, RD_MAX_K);
+    return build_spacetime(ctx, S * nt, /*pool=*/S, ndim, dims, nt, dt, s_out, pairs_out);
+}
+
+int rd_reference_storage(const rd_ctx* ctx, int32_t* kind, int64_t* n_values, int64_t* n_indices)
+{
+    if (!ctx) return RD_EINVAL;
+    const bool kron = ctx->have_ref && ctx->ref_kind == 1;
+    if (kind) *kind = ctx->have_ref ? ctx->ref_kind : -1;
+    if (n_values) *n_values = !ctx->have_ref ? 0 : kron ? ctx->kNs * ctx->krs + (int64_t)ctx->knt * ctx->k : ctx->N * (int64_t)ctx->k;
+    if (n_indices) *n_indices = kron ? ctx->k : 0;
     return RD_OK;
 }
 
@@ -1118,7 +1275,7 @@ int rd_build_reference_transient(rd_ctx* ctx, int32_t k, int32_t rs, int32_t nt,
     if ((int64_t)k > (int64_t)rs * nt) return fail(ctx, RD_EINVAL, "k = %d exceeds the %d x %d candidates", k, rs, nt);
     const int64_t N = ctx->N, Ns = N / nt;
     const auto t_begin = std::chrono::steady_clock::now();
-    RDTRY(alloc_reference(ctx, k));
+    RDTRY(alloc_reference(ctx, k, /*need_dense=*/false));
     struct Scratch {
         std::vector<void*> p;
         ~Scratch() { for (void* q : p) cudaFree(q); }
@@ -1179,22 +1336,31 @@ int rd_build_reference_transient(rd_ctx* ctx, int32_t k, int32_t rs, int32_t nt,
         if (x.i != y.i) return x.i < y.i;
         return x.j < y.j;
     });
-    std::vector<int32_t> sel((size_t)2 * k);
+    std::vector<int32_t> sel((size_t)2 * k), cols;
     for (int c = 0; c < k; ++c) {
         sel[2 * c] = pr[c].i;
         sel[2 * c + 1] = pr[c].j;
+        if (std::find(cols.begin(), cols.end(), pr[c].i) == cols.end()) cols.push_back(pr[c].i);
         if (nu_out) nu_out[c] = pr[c].nu;
         if (pairs_out) { pairs_out[2 * c] = pr[c].i; pairs_out[2 * c + 1] = pr[c].j; }
     }
+    std::sort(cols.begin(), cols.end());
+    const int rs_used = (int)cols.size();
     CU(cudaMemcpyAsync(d_sel, sel.data(), sel.size() * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
-    CU(cudaMemsetAsync(ctx->W, 0, (size_t)ctx->ldw * ctx->kp * sizeof(double), ctx->stream));  // pad rows stay zero
-    k_kron_vectors<<<g, kThreads, 0, ctx->stream>>>(Ns, nt, ctx->ldw, k, ctx->kp, d_sel, d_Phi, d_Q, ctx->W);
-    k_col_sumsq_parts<<<dim3(nparts, k), kThreads, 0, ctx->stream>>>(N, ctx->ldw, ctx->W, d_parts);
-    k_col_normalise<<<dim3(std::max(1, g / 8), k), kThreads, 0, ctx->stream>>>(N, ctx->ldw, nparts, d_parts, ctx->W, d_norms);
-    ctx->launches += 3;
+    // ---- compact storage: the r_s spatial vectors the selection uses, the k temporal vectors scaled so that
+    // every column q (x) phi_i has unit Euclidean norm (||q (x) phi|| = ||q|| ||phi||), and the spatial-column indices
+    double *d_used = nullptr, *d_phin2 = nullptr;
+    RDTRY(salloc((void**)&d_used, (size_t)Ns * rs_used * sizeof(double)));
+    RDTRY(salloc((void**)&d_phin2, (size_t)rs * sizeof(double)));
+    for (int q = 0; q < rs_used; ++q)
+        CU(cudaMemcpyAsync(d_used + (size_t)q * Ns, d_Phi + (size_t)cols[q] * Ns, (size_t)Ns * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    k_col_norm2<<<rs, 256, 0, ctx->stream>>>(Ns, d_Phi, d_phin2);
+    ctx->launches++;
     CU(cudaGetLastError());
-    CU(cudaStreamSynchronize(ctx->stream));
+    RDTRY(store_kron(ctx, k, Ns, nt, rs_used, d_used, cols, d_sel, d_Q, /*normalise=*/1, d_phin2));
     ctx->ref_degree = 0;
+    ctx->ref_col_applies = 0;
+    ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
@@ -1244,6 +1410,38 @@ int rd_build_reference_scaled(rd_ctx* ctx, int32_t k, double tol, int32_t max_bl
     return rc;
 }
 
+int rd_probe_fp64_tensor_peak(rd_ctx* ctx, double* tflops)
+{
+    if (!ctx || !tflops) return RD_EINVAL;
+    const int iters = 1 << 15, blocks = ctx->num_sms * 8, threads = 256;
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+        k_dmma_peak_probe<<<blocks, threads, 0, ctx->stream>>>(iters, 0.5, ctx->tmp);
+        CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+        CU(cudaEventSynchronize(ctx->ev[1]));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, ctx->ev[0], ctx->ev[1]));
+        if (rep > 0) best = std::min(best, ms);
+        ctx->launches++;
+    }
+    CU(cudaGetLastError());
+    const double flop = (double)blocks * (threads / 32) * (double)iters * 8.0 * 512.0;  // m8n8k4: 2 * 8 * 8 * 4 flop
+    *tflops = flop / (best * 1e-3) / 1e12;
+    return RD_OK;
+}
+
+int rd_reference_work(const rd_ctx* ctx, int64_t* column_applies, double* filter_ms, double* bytes_per_column_apply)
+{
+    if (!ctx) return RD_EINVAL;
+    if (column_applies) *column_applies = ctx->ref_col_applies;
+    if (filter_ms) *filter_ms = ctx->ref_filter_ms;
+    // K and K^T stream once per 8 columns (12 B per stored entry each); per column Y is read by the gathers
+    // and once directly, T written and read, Yprev read, Ynext written: 48 N
+    if (bytes_per_column_apply) *bytes_per_column_apply = 3.0 * (double)ctx->nnz + 48.0 * (double)ctx->N;
+    return RD_OK;
+}
+
 int rd_reference_info(const rd_ctx* ctx, int32_t* block, int64_t* total_degree, double* build_ms)
 {
     if (!ctx) return RD_EINVAL;
@@ -1257,7 +1455,7 @@ int rd_coarse_setup(rd_ctx* ctx, int32_t method, const uint8_t* active, double* 
                     double* cond_E, int32_t* fallback)
 {
     if (!ctx || !active) return RD_EINVAL;
-    if (!ctx->W || ctx->k <= 0) return fail(ctx, RD_ENOREF, "no reference set");
+    if (!ctx->have_ref || ctx->k <= 0) return fail(ctx, RD_ENOREF, "no reference set");
     const uint8_t* da;
     RDTRY(in_dev(ctx, active, ctx->N, ctx->act_stage, &da));
     CU(cudaMemcpyAsync(ctx->act, da, ctx->N, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -1298,7 +1496,10 @@ int rd_solve_inactive(rd_ctx* ctx, int32_t method, const uint8_t* active, const 
     CU(cudaMemcpyAsync(ctx->h_nactive, ctx->d_nactive, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     float msr = 0, msc = 0;
-    RDTRY(run_alg1(ctx, method, N - *ctx->h_nactive, rep, &msr, &msc));
+    ctx->want_ritz = true;
+    const int rc_alg = run_alg1(ctx, method, N - *ctx->h_nactive, rep, &msr, &msc);
+    ctx->want_ritz = false;
+    RDTRY(rc_alg);
     RDTRY(out_host(ctx, x, ctx->x, N));
     CU(cudaStreamSynchronize(ctx->stream));
     return rep->status;
@@ -1311,7 +1512,7 @@ int rd_energy_fraction(rd_ctx* ctx, int32_t method, const uint8_t* active, const
     if (method < RD_JACOBI_CG || method > RD_ZEROEXT) return RD_EINVAL;
     const int64_t N = ctx->N;
     int use_coarse = 0;
-    if (method != RD_JACOBI_CG && (!ctx->W || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
+    if (method != RD_JACOBI_CG && (!ctx->have_ref || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
     const uint8_t* da;
     const double *db, *dx;
     RDTRY(in_dev(ctx, active, N, ctx->act_stage, &da));
@@ -1414,7 +1615,7 @@ int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double*
     if (!ctx || !y_d || !psi || !y || !u || !steps || !rep) return RD_EINVAL;
     if (method < RD_JACOBI_CG || method > RD_ZEROEXT) return RD_EINVAL;
     if (ctx->opt.init == RD_INIT_GIVEN && !J0) return RD_EINVAL;
-    if (method != RD_JACOBI_CG && (!ctx->W || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
+    if (method != RD_JACOBI_CG && (!ctx->have_ref || ctx->k <= 0)) return fail(ctx, RD_ENOREF, "method %d needs a reference", method);
     const auto t_begin = std::chrono::steady_clock::now();
     const int64_t N = ctx->N;
     const int64_t nbytes = (N + 7) / 8;

@@ -9,8 +9,10 @@ each query (npz, float64).  tests/test_gpu_twins_golden.py runs the same queries
 
 Settings, identical on both sides: RefDef (direct restriction) with the paper's analytical reference (oracle.sine_reference /
 oracle.spacetime_reference, deterministic closed forms), warm-start policy of PAPER.md:339 over the listed queries,
-eps = eps_c = 1e-12 so that every active-set decision (smallest margins here ~1e-11) is far from the solver's noise and
-the sequence is a property of the method, not of rounding; PDAS cap 400 (the paper's raised cap).
+the paper's own accuracy (verified relative residual 1e-10, recurrence trigger 1e-11) so that the
+active-set decisions (smallest margins here ~1e-11 in absolute terms, on states of size ~1e-1) sit well above the
+solver's noise; PDAS cap 400 (the paper's raised cap).  (1e-12 is below what the recurrence attains on
+the 2-D twins, cond(H) ~ 1e6: the oracle then spends its time in residual replacements.)
 """
 import json
 import os
@@ -34,7 +36,7 @@ CASES = {
     "c5_48": (dict(twin="c5_48"), [0, 1]),
     "c2_256": (dict(config=2, n=256, k=32), [0]),
 }
-EPS = 1e-12
+EPS, EPS_C = 1e-10, 1e-11
 PDAS_CAP = 400
 
 
@@ -49,9 +51,9 @@ def run_case(name):
     w = make_config(**kw)
     o = oracle.Oracle.from_workload(w)
     W = reference_for(w)
-    opt = oracle.OracleOptions(eps=EPS, eps_c=EPS, pdas_cap=PDAS_CAP)
+    opt = oracle.OracleOptions(eps=EPS, eps_c=EPS_C, pdas_cap=PDAS_CAP)
     out = {"case": name, "make_config": kw, "workload": w.name, "N": w.N, "k": w.k, "operator_sha256": w.operator_hash(),
-           "eps": EPS, "pdas_cap": PDAS_CAP, "method": "refdef", "reference": "analytical (oracle.sine_reference / spacetime_reference)",
+           "eps": EPS, "eps_c": EPS_C, "pdas_cap": PDAS_CAP, "method": "refdef", "reference": "analytical (oracle.sine_reference / spacetime_reference)",
            "queries": []}
     ys = {}
     for q in queries:

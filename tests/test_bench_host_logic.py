@@ -57,9 +57,11 @@ def test_bytes_model():
     a = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=0)
     b = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=8)
     c = bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=150, r=8, tall_passes=2)
-    assert a == 24 * 1000 + 16 * 200 + 112 * 150 + 200
+    assert a == (24 * 1000 + 17 * 200) * (150 / 200) + 112 * 150
     assert b - a == 8 * 150 * 8
     assert c - a == 16 * 150 * 8
+    # at n = N the model is round 1's: both matrices once, t on all rows, the mask, 14 vector passes, one tall pass
+    assert bench.algorithmic_bytes_per_iter(nnz=1000, N=200, n=200, r=8) == 24 * 1000 + 17 * 200 + 112 * 200 + 8 * 200 * 8
 
 
 def test_reference_arm_runs_on_cpu(capsys):

@@ -4,7 +4,8 @@ CPU oracle alone (tests/golden/make_golden_twins.py; minutes to an hour of oracl
 
 Compared per query: the whole active-set sequence (FNV-1a hash of the packed set and |I| at every PDAS step: bit-exact),
 status, retained rank and CG iterations per step (5 %), y and u = M^-1 K y to 1e-6 in the M-norm (north_star's bar),
-KKT measures.  Both sides run RefDef with the analytical reference at eps = eps_c = 1e-12 (see the generator's header)."""
+KKT measures.  Both sides run RefDef with the analytical reference at the paper's accuracy, eps = 1e-10 and eps_c = 1e-11
+(see the generator's header)."""
 import json
 import os
 
@@ -37,7 +38,7 @@ def test_twin_sequence_matches_oracle_golden(oracle_mod, case):
         W = oracle_mod.spacetime_reference(w.dims, w.nt, 1.0 / w.nt, w.k)[-1]
     else:
         W = oracle_mod.sine_reference(w.dims, w.k)[-1]
-    g = pkg.RefDef.from_workload(w, pkg.Options(eps=gold["eps"], eps_c=gold["eps"], pdas_cap=gold["pdas_cap"]))
+    g = pkg.RefDef.from_workload(w, pkg.Options(eps=gold["eps"], eps_c=gold["eps_c"], pdas_cap=gold["pdas_cap"]))
     g.set_reference(np.asfortranarray(W))
     o = oracle_mod.Oracle.from_workload(w)
     nrm = lambda v: float(np.sqrt((w.m * v * v).sum()))

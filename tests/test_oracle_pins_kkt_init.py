@@ -259,3 +259,54 @@ def test_K4_c_is_diag_and_margin(c_is_diag):
     assert np.allclose(got, margins, rtol=1e-6, atol=1e-14), (got, margins)
     other = pdas_dense(H, ell, psi, np.ones(N, dtype=bool), c=None if c_is_diag else d)[3]
     assert not np.allclose(margins, other, rtol=1e-3), "the two choices of c must give different margins here"
+
+
+# ------------------------------------------------------------------------------------------------------ K5: eq. (23)
+def test_K5_deflated_spectrum_eq23():
+    """eq. (23).  Pins: (a) with Z = the k lowest eigenvectors of the pencil (B, D) the nonzero spectrum
+    is exactly the rest of the pencil's spectrum (deflation removes what Z spans and nothing else); (b) rank zero gives
+    the whole pencil; (c) for a generic Z the matrix annihilates D^{1/2} Z (r zeros), its nonzero eigenvalues interlace
+    the pencil's: mu_j <= lam_j <= mu_{j+r}; (d) Algorithm 1's iteration count obeys the classical CG bound for the
+    effective condition number.  Mutations this fails under: D^{-1} in place of D^{-1/2}, Z^T B Z replaced by Z^T Z,
+    the r zeros not dropped, B Z taken as Z, D = diag(H) on all N rows instead of diag(B) on I (same here) -- and a
+    transposed or unsymmetrised B."""
+    import scipy.linalg as sla
+
+    w, K, m = small_problem(9)
+    N, sigma = w.N, 1e-4
+    H = dense_H(K, m, sigma)
+    o = oracle.Oracle(w.rowptr, w.colidx, w.val, m, sigma)
+    rng = np.random.default_rng(4)
+    idx = np.flatnonzero(rng.random(N) > 0.25).astype(np.int64)
+    n = len(idx)
+    B = H[np.ix_(idx, idx)]
+    D = np.diag(np.diag(B))
+    mu, V = sla.eigh(B, D)  # B v = mu D v, ascending
+    k = 5
+    lam, r = oracle.deflated_spectrum(o, idx, V[:, :k])
+    assert r == k and len(lam) == n - k
+    assert np.allclose(lam, mu[k:], rtol=1e-9)
+    lam0, r0 = oracle.deflated_spectrum(o, idx, None)
+    assert r0 == 0 and np.allclose(lam0, mu, rtol=1e-10)
+    # generic basis: Cauchy interlacing of the compression to the B-orthogonal complement
+    Zt = rng.standard_normal((n, 4))
+    lam_g, r_g = oracle.deflated_spectrum(o, idx, Zt)
+    assert r_g == 4 and len(lam_g) == n - 4
+    assert (lam_g >= mu[: n - 4] * (1 - 1e-9)).all() and (lam_g <= mu[4:] * (1 + 1e-9)).all()
+    assert lam_g[0] > 1e-6 * lam_g[-1], "the r zero eigenvalues must have been dropped"
+    # independent dense evaluation of the matrix of eq. (23) for the generic basis
+    Q, _ = np.linalg.qr(Zt)
+    Ssc = np.diag(1.0 / np.sqrt(np.diag(B)))
+    A = Ssc @ (B - B @ Q @ np.linalg.solve(Q.T @ B @ Q, Q.T @ B)) @ Ssc
+    ref = np.linalg.eigvalsh(0.5 * (A + A.T))[4:]
+    assert np.allclose(lam_g, ref, rtol=1e-8)
+    # the solver sees this spectrum: iterations <= the CG bound for kappa_eff = lam_max / lam_min
+    b = rng.standard_normal(n)
+    eps = 1e-10
+    _, rep = o.alg1(idx, b, np.zeros(n), Zt, eps=eps)
+    kappa = lam_g[-1] / lam_g[0]
+    # energy-norm bound 2 ((sqrt(k)-1)/(sqrt(k)+1))^m, converted to the residual with sqrt(kappa(B^)) slack
+    bound = np.ceil(0.5 * np.sqrt(kappa) * np.log(2.0 * np.sqrt(mu[-1] / mu[0]) / eps)) + 1
+    assert rep["status"] == 0 and rep["iters"] <= bound
+    _, rep_j = o.alg1(idx, b, np.zeros(n), None, eps=eps)
+    assert rep["iters"] <= rep_j["iters"]
