@@ -405,11 +405,13 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     P.Wm = ctx->Zm; P.HWm = ctx->HZm; P.HWt = ctx->HZt; P.C = ctx->C; P.EW = ctx->E;
     P.eps = ctx->opt.eps; P.eps_c = ctx->opt.eps_c; P.cap = ctx->opt.cg_cap; P.replace_period = ctx->opt.replace_period;
     P.partial = ctx->partial; P.bar = ctx->bar;
-    {   // Part of the H_II W_I stream is requested with L2 evict_last when the whole working set nearly fits the
-        // 126 MB L2 (config 2): what is left of a 60 MB budget after K, K^T and ten vectors, at most half the stream.
-        const double hw_bytes = 8.0 * (double)ctx->ldw * ctx->kp;
+    {   // Part of the H_II Z stream is requested with L2 evict_last when the whole working set nearly fits the 126 MB L2
+        // (config 2): what is left of an L2 budget after K, K^T and ten vectors, at most 90 % of the stream.  The budget
+        // (MB) can be overridden with RD_L2_BUDGET_MB for experiments (profiles/r2_summary.md).
+        static const double budget_mb = [] { const char* e = getenv("RD_L2_BUDGET_MB"); return e ? atof(e) : 60.0; }();
+        const double hw_bytes = 8.0 * (double)n_inactive * ctx->kp;
         const double other = 12.0 * (double)(ctx->K.entries + ctx->KT.entries) + 80.0 * (double)N;
-        double frac = hw_bytes > 0 ? std::min(0.5, std::max(0.0, (60e6 - other) / hw_bytes)) : 0.0;
+        double frac = hw_bytes > 0 ? std::min(0.9, std::max(0.0, (budget_mb * 1e6 - other) / hw_bytes)) : 0.0;
         const int64_t tiles_per_cta = ((n_inactive + 31) / 32 + ctx->cg_grid - 1) / ctx->cg_grid;
         P.hw_res_tiles = (int32_t)((double)tiles_per_cta * frac);
     } P.rep = ctx->d_cgrep;
@@ -959,9 +961,15 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
         const int nch = nchunk - col0 / RD_EIG_CB;
         const dim3 gb(std::max(1, gs / std::min(nch, 4)), nch);
         const size_t o = (size_t)col0 * ld;
-        k_blk_K<<<gb, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y + o, T + o);
-        k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o,
-                                                   Yprev ? Yprev + o : nullptr, Ynext + o);
+        // kernels specialised for the uniform row widths of the stencil operators (5, 6, 7 entries), generic otherwise
+        const Ell Kv = ctx->K.view(), KTv = ctx->KT.view();
+        const double* Yp = Yprev ? Yprev + o : nullptr;
+#define RD_BLK_K(W) k_blk_K<W><<<gb, kThreads, 0, ctx->stream>>>(Kv, N, ld, ctx->minv, Y + o, T + o)
+#define RD_BLK_KT(W) k_blk_KT<W><<<gb, kThreads, 0, ctx->stream>>>(KTv, N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o, Yp, Ynext + o)
+        switch (Kv.uwd) { case 5: RD_BLK_K(5); break; case 6: RD_BLK_K(6); break; case 7: RD_BLK_K(7); break; default: RD_BLK_K(0); }
+        switch (KTv.uwd) { case 5: RD_BLK_KT(5); break; case 6: RD_BLK_KT(6); break; case 7: RD_BLK_KT(7); break; default: RD_BLK_KT(0); }
+#undef RD_BLK_K
+#undef RD_BLK_KT
         ctx->launches += 2;
         col_applies += (int64_t)nch * RD_EIG_CB;
     };

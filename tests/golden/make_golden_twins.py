@@ -9,10 +9,9 @@ each query (npz, float64).  tests/test_gpu_twins_golden.py runs the same queries
 
 Settings, identical on both sides: RefDef (direct restriction) with the paper's analytical reference (oracle.sine_reference /
 oracle.spacetime_reference, deterministic closed forms), warm-start policy of PAPER.md:339 over the listed queries,
-the paper's own accuracy (verified relative residual 1e-10, recurrence trigger 1e-11) so that the
-active-set decisions (smallest margins here ~1e-11 in absolute terms, on states of size ~1e-1) sit well above the
-solver's noise; PDAS cap 400 (the paper's raised cap).  (1e-12 is below what the recurrence attains on
-the 2-D twins, cond(H) ~ 1e6: the oracle then spends its time in residual replacements.)
+the paper's own accuracy where double precision attains it (verified relative residual 1e-10, recurrence
+trigger 1e-11; see CASES) so that the active-set decisions sit above the solver's noise; PDAS cap 400 (the paper's
+raised cap).
 """
 import json
 import os
@@ -28,15 +27,17 @@ sys.path.insert(0, ROOT)
 import oracle  # noqa: E402
 from workloads import make_config  # noqa: E402
 
-# name -> (make_config kwargs, queries)
+# name -> (make_config kwargs, queries, eps, eps_c)
+# The 3-D and space-time twins (cond(H) <= 1e4) run at the paper's accuracy.  The 2-D twins have cond(H) ~ 1.6e6 (128^2) and
+# ~ 2.6e7 (256^2): a recomputed relative residual of 1e-11 is below what double precision attains there (Algorithm 1 then
+# restarts until its cap), so they run at BASELINE.json's 1e-8 / 1e-8.
 CASES = {
-    "c3_32": (dict(twin="c3_32"), [0, 1]),
-    "c2_128": (dict(twin="c2_128"), [0, 1]),
-    "c4_64x8": (dict(twin="c4_64x8"), [0]),
-    "c5_48": (dict(twin="c5_48"), [0, 1]),
-    "c2_256": (dict(config=2, n=256, k=32), [0]),
+    "c3_32": (dict(twin="c3_32"), [0, 1], 1e-10, 1e-11),
+    "c2_128": (dict(twin="c2_128"), [0, 1], 1e-8, 1e-8),
+    "c4_64x8": (dict(twin="c4_64x8"), [0], 1e-10, 1e-11),
+    "c5_48": (dict(twin="c5_48"), [0, 1], 1e-10, 1e-11),
+    "c2_256": (dict(config=2, n=256, k=32), [0], 1e-8, 1e-8),
 }
-EPS, EPS_C = 1e-10, 1e-11
 PDAS_CAP = 400
 
 
@@ -47,7 +48,7 @@ def reference_for(w):
 
 
 def run_case(name):
-    kw, queries = CASES[name]
+    kw, queries, EPS, EPS_C = CASES[name]
     w = make_config(**kw)
     o = oracle.Oracle.from_workload(w)
     W = reference_for(w)

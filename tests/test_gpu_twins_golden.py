@@ -51,9 +51,17 @@ def test_twin_sequence_matches_oracle_golden(oracle_mod, case):
             n_in = [s["n_inactive"] for s in r["steps"]]
             if hashes != gq["active_hash"]:
                 first = next(i for i, (a, b) in enumerate(zip(hashes, gq["active_hash"])) if a != b)
-                pytest.fail(f"{case} query {gq['query']}: active sets differ first at step {first} of {gq['n_steps']} "
-                            f"(|I| {n_in[first]} vs {gq['n_inactive'][first]}); oracle margin of the deciding step "
-                            f"{gq['margin'][first - 1]:.2e}")
+                # A decision of eq. (8) is a threshold on an inexact solve: the two sides may part
+                # only where the oracle's own distance to a tie is below the solver's noise, eps * |y|; anything else
+                # is a bug.  Both sequences must still end at the unique solution of the QP (checked below).
+                noise = 10.0 * gold["eps"] * float(np.abs(ys[f"y{gq['query']}"]).max())
+                assert gq["margin"][first - 1] <= noise, (
+                    f"{case} query {gq['query']}: active sets differ first at step {first} of {gq['n_steps']} "
+                    f"(|I| {n_in[first]} vs {gq['n_inactive'][first]}); oracle margin of the deciding step "
+                    f"{gq['margin'][first - 1]:.2e} is not a near-tie (noise level {noise:.1e})")
+                y_o = ys[f"y{gq['query']}"]
+                assert nrm(r["y"] - y_o) <= 1e-6 * nrm(y_o) and max(r["kkt"]) <= 1e-8
+                continue
             assert r["n_steps"] == gq["n_steps"] and n_in == gq["n_inactive"]
             assert r["worst_inner_status"] == 0 and all(s == 0 for s in gq["inner_status"])
             for s, it_o, rk_o in zip(r["steps"], gq["cg_iters"], gq["rank_used"]):
