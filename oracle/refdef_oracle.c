@@ -25,7 +25,10 @@
  * on tiny grids, symmetry + definiteness, KKT complementarity, unconstrained limit,
  * projector identities, restriction-residual identity eq. (20)-(21),
  * closed-form spectrum, rank-zero == Jacobi-CG, Fig. 2 transfer pattern, energy fraction
- * eq. (24).  Unpinned: CG iteration counts at full size ("parity unpinned").
+ * eq. (24); and (tests/test_oracle_pins_kkt_init.py) the five KKT measures of eq. (25) on a perturbed pair with
+ * ||l||_inf > 1, the cond(E) > 1e10 fallback on both sides of its threshold, the query starts (given J0, all
+ * inactive, inherited state and set), c = H_ii and the margin -- each shown to fail under listed mutations.
+ * Unpinned: CG iteration counts at full size ("parity unpinned").
  *
  * Threads.  The parity tests use the plain build (gcc -O2, single thread, the loops exactly as written).
  * The TIMING legs of bench.py (cpu_baseline, --impl reference) may build the same file with -fopenmp: the

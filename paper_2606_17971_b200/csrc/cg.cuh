@@ -38,13 +38,14 @@ struct CgParams {
     const uint8_t* act;  // 1 = active (J)
     const double* b;     // rhs, 0 on J
     double *x, *r, *p0, *p1, *z, *w, *t;
-    const double *Wm, *HWm;  // chi_I W and chi_I H chi_I W, N x kp column-major (ld = ldw)
+    const double *Wm, *HWm;  // the basis of eq. (18) and its cached product, N x kp column-major (ld = ldw): since round 2 the
+                             // explicit Z = W_I T and H_II Z (coarse.cuh), so that C = E^{-1}; any full-rank basis with its C works
     const double* HWt;       // HWm tile-major: (i, j) at (i / 32) * 32 kp + 32 j + i % 32 (k_alg1_v3)
-    const double* Wt;        // Wm tile-major, same layout (k_alg1_v3: coarse corrections outside the loop)
+    const double* Wt;        // Wm (= Z) tile-major, same layout (k_alg1_v3: coarse corrections outside the loop)
     const int32_t *listA, *listB;  // S6 compaction: live 32-row slices of the current active set (pdas.cuh k_slice_lists)
     const int32_t* live_counts;    // [0] = |listA|, [1] = |listB|
-    const double* C;         // kp x kp column-major
-    const double* EW;        // W_I^T H_II W_I, kp x kp column-major (k_alg1_v3: curvature in coefficient form)
+    const double* C;         // kp x kp column-major, symmetric: the coarse solve in the coordinates of Wm
+    const double* EW;        // Wm^T HWm, kp x kp column-major (k_alg1_v3: curvature in coefficient form)
     double eps, eps_c;
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]

@@ -3,6 +3,9 @@
 // work restricted to the live 32-row slices of the current active set (S6 compaction, pdas.cuh).  Default kernel of the
 // library (rd_options.alg1_variant = 0); cg.cuh keeps the literal two-pass recurrence as variant 1.
 //
+// (W_I below stands for the basis handed to the kernel, HW_I for its cached product and C for the coarse solve in its
+// coordinates; since round 2 that basis is the explicit Z = W_I T of coarse.cuh, so HW_I = H_II Z, E_W = E, C = E^{-1}.)
+//
 // ---- coefficient form.  Write the search direction and the iterate of Alg. 1 as  p = p~ - W_I nu,  x = x~ - W_I xi  with
 // k-vectors nu, xi kept (replicated, bit-identical) in the shared memory of every CTA.  With z~ = J r (never projected):
 //   line 22  z = P J r = z~ - W_I mu,  mu = C c,  c = (HW_I)^T z~                       (eq. (18))
@@ -45,8 +48,8 @@ namespace rd {
 #define RD_SPMV_SLOT_BYTES 4096  // per warp: values 8 x 256 B, then indices 8 x 128 B
 
 struct __align__(128) Cg3Shared {
-    double C[RD_MAX_K * RD_MAX_K];   // T E^{-1} T^T, symmetric
-    double EW[RD_MAX_K * RD_MAX_K];  // W_I^T H_II W_I, symmetrised on load
+    double C[RD_MAX_K * RD_MAX_K];   // E^{-1} (coordinates of the explicit basis Z), symmetric
+    double EW[RD_MAX_K * RD_MAX_K];  // E = Z^T H_II Z, symmetrised on load
     double zb[32][32];               // tile streams: the per-row multiplier of the warp's tile, for the transposed pass
     double cpart[512];               // tile streams: c partials of the consumer warps, NST x kp <= 512
     double c[RD_MAX_K], mu[RD_MAX_K], nu[2][RD_MAX_K], g[2][RD_MAX_K], sv[RD_MAX_K], xi[RD_MAX_K], anu[RD_MAX_K], e[RD_MAX_K];

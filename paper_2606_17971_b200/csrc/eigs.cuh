@@ -19,43 +19,11 @@ namespace rd {
 #define RD_EIG_CB 8      // columns per SpMM pass
 #define RD_EIG_MAXB 128  // block size limit (k <= 64 plus guard)
 
-// One row of a blocked sliced-ELL product: acc[q] += sum_e A[row,e] V[col_e, q] for RD_EIG_CB columns of V (leading
-// dimension ld).  WD > 0: the matrix has WD entries in every row (Ell::uwd, all the stencil operators here): the loop is
-// unrolled, all indices and values are loaded first and the 8 WD gathers follow back to back (more loads in flight per
-// lane than the rolled loop reaches).  WD = 0: any width, read from the slice extents.
-template <int WD>
-__device__ __forceinline__ void blk_row(const Ell& A, int64_t s, int lane, const double* __restrict__ V, int64_t ld, double (&acc)[RD_EIG_CB])
-{
-    if (WD > 0) {
-        const int64_t o = s * 32 * WD;
-        int c[WD > 0 ? WD : 1];
-        double a[WD > 0 ? WD : 1];
-#pragma unroll
-        for (int e = 0; e < WD; ++e) {
-            c[e] = ldg_i32(A.col + o + e * 32 + lane);
-            a[e] = ldg_f64(A.val + o + e * 32 + lane);
-        }
-#pragma unroll
-        for (int e = 0; e < WD; ++e) {
-#pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a[e], ldg_f64(V + c[e] + (size_t)q * ld), acc[q]);
-        }
-    } else {
-        const int64_t o = A.off[s];
-        const int wd = (int)((A.off[s + 1] - o) >> 5);
-        for (int e = 0; e < wd; ++e) {
-            const int c = ldg_i32(A.col + o + e * 32 + lane);
-            const double a = ldg_f64(A.val + o + e * 32 + lane);
-#pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a, ldg_f64(V + c + (size_t)q * ld), acc[q]);
-        }
-    }
-}
-
+// (Round 2 tried kernels specialised on the uniform row width with all indices / values loaded before the gathers and the
+// row's own Y / Yprev entries prefetched: slower on B200 -- config 2 build 10.05 s against 9.02 s, config 3 7.9 s against
+// 6.9 s, 78 registers in the K^T kernel -- so the rolled loops below stay.)
 // T[:, chunk] = M^{-1} K Y[:, chunk]; chunk = blockIdx.y selects RD_EIG_CB columns
-template <int WD>
-__global__ void __launch_bounds__(256) k_blk_K(Ell K, int64_t N, int64_t ld, const double* __restrict__ minv, const double* __restrict__ Y,
-                                               double* __restrict__ T)
+__global__ void k_blk_K(Ell K, int64_t N, int64_t ld, const double* minv, const double* Y, double* T)
 {
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -65,12 +33,19 @@ __global__ void __launch_bounds__(256) k_blk_K(Ell K, int64_t N, int64_t ld, con
     double* O = T + cofs;
     for (int64_t s = gw; s < K.nslices; s += nwt) {
         const int64_t row = s * RD_SLICE + lane;
+        const int64_t o = K.off[s];
+        const int wd = (int)((K.off[s + 1] - o) >> 5);
         double acc[RD_EIG_CB];
 #pragma unroll
         for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = 0.0;
-        blk_row<WD>(K, s, lane, V, ld, acc);
+        for (int e = 0; e < wd; ++e) {
+            const int c = ldg_i32(K.col + o + e * 32 + lane);
+            const double a = ldg_f64(K.val + o + e * 32 + lane);
+#pragma unroll
+            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a, V[c + (size_t)q * ld], acc[q]);
+        }
         if (row < N) {
-            const double mi = ldg_f64(minv + row);
+            const double mi = minv[row];
 #pragma unroll
             for (int q = 0; q < RD_EIG_CB; ++q) O[row + (size_t)q * ld] = acc[q] * mi;
         }
@@ -79,10 +54,8 @@ __global__ void __launch_bounds__(256) k_blk_K(Ell K, int64_t N, int64_t ld, con
 
 // Ynext[:, chunk] = c1 ( (m .* Y + sigma K^T T) - cshift Y ) + c2 Yprev     (Yprev may be NULL when c2 == 0)
 // c1 = 1, cshift = 0, c2 = 0 gives the plain block apply H Y.
-template <int WD>
-__global__ void __launch_bounds__(256) k_blk_KT(Ell KT, int64_t N, int64_t ld, const double* __restrict__ m, double sigma, double c1,
-                                                double cshift, double c2, const double* __restrict__ Y, const double* __restrict__ T,
-                                                const double* __restrict__ Yprev, double* __restrict__ Ynext)
+__global__ void k_blk_KT(Ell KT, int64_t N, int64_t ld, const double* m, double sigma, double c1, double cshift,
+                         double c2, const double* Y, const double* T, const double* Yprev, double* Ynext)
 {
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -91,29 +64,26 @@ __global__ void __launch_bounds__(256) k_blk_KT(Ell KT, int64_t N, int64_t ld, c
     const double* Tc = T + cofs;
     for (int64_t s = gw; s < KT.nslices; s += nwt) {
         const int64_t row = s * RD_SLICE + lane;
-        // the row's own entries of Y and Yprev: issued before the gathers so that they never add a round trip
-        double yv[RD_EIG_CB], pv[RD_EIG_CB];
-        double mi = 0.0;
-        if (row < N) {
-            mi = ldg_f64(m + row) - cshift;
-#pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) {
-                const size_t idx = cofs + row + (size_t)q * ld;
-                yv[q] = ldg_f64(Y + idx);
-                pv[q] = Yprev ? ldg_f64(Yprev + idx) : 0.0;
-            }
-        }
+        const int64_t o = KT.off[s];
+        const int wd = (int)((KT.off[s + 1] - o) >> 5);
         double acc[RD_EIG_CB];
 #pragma unroll
         for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = 0.0;
-        blk_row<WD>(KT, s, lane, Tc, ld, acc);
+        for (int e = 0; e < wd; ++e) {
+            const int c = ldg_i32(KT.col + o + e * 32 + lane);
+            const double a = ldg_f64(KT.val + o + e * 32 + lane);
+#pragma unroll
+            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a, Tc[c + (size_t)q * ld], acc[q]);
+        }
         if (row < N) {
+            const double mi = m[row] - cshift;
 #pragma unroll
             for (int q = 0; q < RD_EIG_CB; ++q) {
-                double h = fma(sigma, acc[q], mi * yv[q]);
+                const size_t idx = cofs + row + (size_t)q * ld;
+                double h = fma(sigma, acc[q], mi * Y[idx]);
                 h *= c1;
-                if (Yprev) h = fma(c2, pv[q], h);
-                Ynext[cofs + row + (size_t)q * ld] = h;
+                if (Yprev) h = fma(c2, Yprev[idx], h);
+                Ynext[idx] = h;
             }
         }
     }

@@ -408,7 +408,7 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
     {   // Part of the H_II Z stream is requested with L2 evict_last when the whole working set nearly fits the 126 MB L2
         // (config 2): what is left of an L2 budget after K, K^T and ten vectors, at most 90 % of the stream.  The budget
         // (MB) can be overridden with RD_L2_BUDGET_MB for experiments (profiles/r2_summary.md).
-        static const double budget_mb = [] { const char* e = getenv("RD_L2_BUDGET_MB"); return e ? atof(e) : 60.0; }();
+        static const double budget_mb = [] { const char* e = getenv("RD_L2_BUDGET_MB"); return e ? atof(e) : 80.0; }();
         const double hw_bytes = 8.0 * (double)n_inactive * ctx->kp;
         const double other = 12.0 * (double)(ctx->K.entries + ctx->KT.entries) + 80.0 * (double)N;
         double frac = hw_bytes > 0 ? std::min(0.9, std::max(0.0, (budget_mb * 1e6 - other) / hw_bytes)) : 0.0;
@@ -961,15 +961,9 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
         const int nch = nchunk - col0 / RD_EIG_CB;
         const dim3 gb(std::max(1, gs / std::min(nch, 4)), nch);
         const size_t o = (size_t)col0 * ld;
-        // kernels specialised for the uniform row widths of the stencil operators (5, 6, 7 entries), generic otherwise
-        const Ell Kv = ctx->K.view(), KTv = ctx->KT.view();
-        const double* Yp = Yprev ? Yprev + o : nullptr;
-#define RD_BLK_K(W) k_blk_K<W><<<gb, kThreads, 0, ctx->stream>>>(Kv, N, ld, ctx->minv, Y + o, T + o)
-#define RD_BLK_KT(W) k_blk_KT<W><<<gb, kThreads, 0, ctx->stream>>>(KTv, N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o, Yp, Ynext + o)
-        switch (Kv.uwd) { case 5: RD_BLK_K(5); break; case 6: RD_BLK_K(6); break; case 7: RD_BLK_K(7); break; default: RD_BLK_K(0); }
-        switch (KTv.uwd) { case 5: RD_BLK_KT(5); break; case 6: RD_BLK_KT(6); break; case 7: RD_BLK_KT(7); break; default: RD_BLK_KT(0); }
-#undef RD_BLK_K
-#undef RD_BLK_KT
+        k_blk_K<<<gb, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y + o, T + o);
+        k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o,
+                                                   Yprev ? Yprev + o : nullptr, Ynext + o);
         ctx->launches += 2;
         col_applies += (int64_t)nch * RD_EIG_CB;
     };
