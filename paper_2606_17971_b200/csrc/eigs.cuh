@@ -22,63 +22,66 @@ namespace rd {
 // (Round 2 tried kernels specialised on the uniform row width with all indices / values loaded before the gathers and the
 // row's own Y / Yprev entries prefetched: slower on B200 -- config 2 build 10.05 s against 9.02 s, config 3 7.9 s against
 // 6.9 s, 78 registers in the K^T kernel -- so the rolled loops below stay.)
-// T[:, chunk] = M^{-1} K Y[:, chunk]; chunk = blockIdx.y selects RD_EIG_CB columns
+// T[:, chunk] = M^{-1} K Y[:, chunk]; chunk = blockIdx.y selects CB columns (CB = 8 or 16: the wider pass streams K
+// once per 16 columns and halves the matrix traffic per column)
+template <int CB>
 __global__ void k_blk_K(Ell K, int64_t N, int64_t ld, const double* minv, const double* Y, double* T)
 {
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
-    const size_t cofs = (size_t)blockIdx.y * RD_EIG_CB * ld;
+    const size_t cofs = (size_t)blockIdx.y * CB * ld;
     const double* V = Y + cofs;
     double* O = T + cofs;
     for (int64_t s = gw; s < K.nslices; s += nwt) {
         const int64_t row = s * RD_SLICE + lane;
         const int64_t o = K.off[s];
         const int wd = (int)((K.off[s + 1] - o) >> 5);
-        double acc[RD_EIG_CB];
+        double acc[CB];
 #pragma unroll
-        for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = 0.0;
+        for (int q = 0; q < CB; ++q) acc[q] = 0.0;
         for (int e = 0; e < wd; ++e) {
             const int c = ldg_i32(K.col + o + e * 32 + lane);
             const double a = ldg_f64(K.val + o + e * 32 + lane);
 #pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a, V[c + (size_t)q * ld], acc[q]);
+            for (int q = 0; q < CB; ++q) acc[q] = fma(a, V[c + (size_t)q * ld], acc[q]);
         }
         if (row < N) {
             const double mi = minv[row];
 #pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) O[row + (size_t)q * ld] = acc[q] * mi;
+            for (int q = 0; q < CB; ++q) O[row + (size_t)q * ld] = acc[q] * mi;
         }
     }
 }
 
 // Ynext[:, chunk] = c1 ( (m .* Y + sigma K^T T) - cshift Y ) + c2 Yprev     (Yprev may be NULL when c2 == 0)
 // c1 = 1, cshift = 0, c2 = 0 gives the plain block apply H Y.
+template <int CB>
 __global__ void k_blk_KT(Ell KT, int64_t N, int64_t ld, const double* m, double sigma, double c1, double cshift,
                          double c2, const double* Y, const double* T, const double* Yprev, double* Ynext)
 {
     const int lane = threadIdx.x & 31;
     const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
-    const size_t cofs = (size_t)blockIdx.y * RD_EIG_CB * ld;
+    const size_t cofs = (size_t)blockIdx.y * CB * ld;
     const double* Tc = T + cofs;
     for (int64_t s = gw; s < KT.nslices; s += nwt) {
         const int64_t row = s * RD_SLICE + lane;
         const int64_t o = KT.off[s];
         const int wd = (int)((KT.off[s + 1] - o) >> 5);
-        double acc[RD_EIG_CB];
+        double acc[CB];
 #pragma unroll
-        for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = 0.0;
+        for (int q = 0; q < CB; ++q) acc[q] = 0.0;
         for (int e = 0; e < wd; ++e) {
             const int c = ldg_i32(KT.col + o + e * 32 + lane);
             const double a = ldg_f64(KT.val + o + e * 32 + lane);
 #pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) acc[q] = fma(a, Tc[c + (size_t)q * ld], acc[q]);
+            for (int q = 0; q < CB; ++q) acc[q] = fma(a, Tc[c + (size_t)q * ld], acc[q]);
         }
         if (row < N) {
             const double mi = m[row] - cshift;
 #pragma unroll
-            for (int q = 0; q < RD_EIG_CB; ++q) {
+            for (int q = 0; q < CB; ++q) {
                 const size_t idx = cofs + row + (size_t)q * ld;
                 double h = fma(sigma, acc[q], mi * Y[idx]);
                 h *= c1;
