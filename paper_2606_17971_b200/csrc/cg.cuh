@@ -50,10 +50,6 @@ struct CgParams {
     int32_t cap, replace_period;
     double* partial;  // [2][SL_NSLOT][gridDim.x]
     GridBarrier* bar;
-    unsigned int* stage_flags;  // NULL or gridDim.x counters (zero at launch): CTA c publishes "my K product of direction
-                                // number q is done"; stands in for the grid barrier between stages A and B when the
-                                // operator's bandwidth keeps every CTA's K^T gathers inside a few neighbouring shares
-    int64_t bandwidth;          // max |column - row| over the entries of K (rows); used with stage_flags
     double2* coef;        // NULL or coef_cap entries: (a_it, beta_it) of every loop iteration (CG-Lanczos coefficients; eq. (23) diagnostic)
     int32_t coef_cap;
     int32_t hw_res_tiles; // tiles per CTA of the H_II W_I stream requested with L2 evict_last (kept resident)

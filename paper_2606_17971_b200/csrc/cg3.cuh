@@ -88,10 +88,8 @@ struct Cg3Cta {
     uint32_t ph;    // phase parity of this warp's mbarrier (uniform in the warp)
     int par;        // which copy of nu / g is current
     double ng, ne;  // nu^T g, nu^T E_W nu of the current direction (every thread holds them)
-    int dep_lo, dep_n;     // neighbour synchronisation between stages A and B: the CTAs whose t rows this CTA's K^T rows gather
-    unsigned int aseq;     // stage-A completions published so far
 
-    __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : P(p), sh(s), nbar(0), ph(0), par(0), ng(0.0), ne(0.0), dep_lo(0), dep_n(0), aseq(0)
+    __device__ Cg3Cta(const CgParams& p, Cg3Shared& s) : P(p), sh(s), nbar(0), ph(0), par(0), ng(0.0), ne(0.0)
     {
         G = gridDim.x;
         const int64_t nA = P.live_counts[0], nB = P.live_counts[1];
@@ -100,14 +98,6 @@ struct Cg3Cta {
         b0 = (int64_t)blockIdx.x * nB / G;
         b1 = (int64_t)(blockIdx.x + 1) * nB / G;
         dense = (nB == P.K.nslices);  // listA contains listB
-        if (dense && P.stage_flags && b1 > b0) {
-            // rows this CTA's K^T product gathers t from: its own rows widened by the bandwidth; their owners in stage A
-            // (dense: CTA c owns the slices [c nA / G, (c + 1) nA / G), so slice s belongs to ceil((s + 1) G / nA) - 1)
-            const int64_t smin = max((int64_t)0, (b0 * 32 - P.bandwidth) >> 5);
-            const int64_t smax = min(nA - 1, ((b1 * 32 - 1 + P.bandwidth) >> 5));
-            dep_lo = (int)(((smin + 1) * G + nA - 1) / nA - 1);
-            dep_n = (int)(((smax + 1) * G + nA - 1) / nA - 1) - dep_lo + 1;
-        }
         if (threadIdx.x == 0) {
             for (int w = 0; w < 32; ++w) mbar_init(&sh.full[w], 1);
             mbar_fence_init();
@@ -139,23 +129,10 @@ struct Cg3Cta {
         for (int q = 0; q < 8; ++q) rep->t_stage_us[q] = us_per_cycle * (double)sh.tacc[q];
     }
 
-    // ---- neighbour synchronisation between stage A and stage B (dense lists, banded operator): instead of a grid
-    // barrier, every CTA publishes the number of K products it has finished (release store after a CTA barrier) and
-    // waits only for the few CTAs whose rows of t its own K^T rows gather (acquire loads: they also invalidate this SM's
-    // L1, as the grid barrier's acquire does).  Cooperative launch keeps all CTAs resident, so the waits terminate.
-    __device__ bool neighbour_sync_on() const { return dense && P.stage_flags != nullptr; }
-    __device__ void publish_and_wait_neighbours()
-    {
-        aseq++;
-        __syncthreads();
-        if (threadIdx.x == 0) st_release_u32(P.stage_flags + blockIdx.x, aseq);
-        if ((int)threadIdx.x < dep_n) {
-            const unsigned int* f = P.stage_flags + dep_lo + threadIdx.x;
-            while (ld_acquire_u32(f) < aseq) {}
-        }
-        __syncthreads();
-    }
-
+    // (Round 2 also tried per-CTA flags instead of the grid barrier between stages A and B -- a CTA's K^T rows gather t only
+    // from a few neighbouring shares on these banded operators; commit d22bb87, RD_NEIGHBOUR_SYNC.  Config 5: 566.3 against
+    // 567.0 us per iteration (the wait moves to the next barrier), config 4 293.8 against 289.1, config 2 35.6 against 32.7:
+    // removed.)
     // ---- grid barrier + all-reduce.  Every CTA has written one partial per reduced quantity; the barrier is the
     // single-hop counter barrier of common.cuh (arrival = release reduction on one monotone counter, everybody polls
     // that counter); then every CTA sums all partials in the same fixed order (deterministic, identical branches).
@@ -728,8 +705,7 @@ __global__ void __launch_bounds__(RD_CG_THREADS, 1) k_alg1_v3(const CgParams P)
         else cta.opK<true, false>(P.z, pold, beta, pnew);
         cur ^= 1;
         cta.tick(0);
-        if (cta.neighbour_sync_on()) cta.publish_and_wait_neighbours();
-        else cta.sync_fetch(false, false);
+        cta.sync_fetch(false, false);
         cta.tick(1);
         // ---- stage B
         {

@@ -22,9 +22,11 @@ namespace rd {
 // (Round 2 tried kernels specialised on the uniform row width with all indices / values loaded before the gathers and the
 // row's own Y / Yprev entries prefetched: slower on B200 -- config 2 build 10.05 s against 9.02 s, config 3 7.9 s against
 // 6.9 s, 78 registers in the K^T kernel -- so the rolled loops below stay.)
-// T[:, chunk] = M^{-1} K Y[:, chunk]; chunk = blockIdx.y selects CB columns (CB = 8 or 16: the wider pass streams K
-// once per 16 columns and halves the matrix traffic per column)
-template <int CB>
+// (Also tried in round 2, commit d22bb87: 4 and 16 columns per pass.  Build times 8 / 4 / 16 columns: config 2 9.05 / 10.08 /
+// 9.95 s, config 3 6.69 / 6.31 / 5.91 s, config 5 123.4 / 127.0 / 128.0 s: 8 stays.  ncu: the two kernels run at 35-43 % of
+// the DRAM peak with 54 % warp occupancy -- bound by the latency of the gathers, not by bytes; profiles/r2_summary.md.)
+// T[:, chunk] = M^{-1} K Y[:, chunk]; chunk = blockIdx.y selects RD_EIG_CB columns
+#define CB RD_EIG_CB
 __global__ void k_blk_K(Ell K, int64_t N, int64_t ld, const double* minv, const double* Y, double* T)
 {
     const int lane = threadIdx.x & 31;
@@ -56,7 +58,6 @@ __global__ void k_blk_K(Ell K, int64_t N, int64_t ld, const double* minv, const 
 
 // Ynext[:, chunk] = c1 ( (m .* Y + sigma K^T T) - cshift Y ) + c2 Yprev     (Yprev may be NULL when c2 == 0)
 // c1 = 1, cshift = 0, c2 = 0 gives the plain block apply H Y.
-template <int CB>
 __global__ void k_blk_KT(Ell KT, int64_t N, int64_t ld, const double* m, double sigma, double c1, double cshift,
                          double c2, const double* Y, const double* T, const double* Yprev, double* Ynext)
 {
@@ -91,6 +92,8 @@ __global__ void k_blk_KT(Ell KT, int64_t N, int64_t ld, const double* m, double 
         }
     }
 }
+
+#undef CB
 
 // Upper bound of the spectrum (Gershgorin on |H| <= M + sigma |K|^T M^{-1} |K|):
 //   s_r = (1/m_r) sum_c |K_rc|,   bound = max_i ( m_i + sigma sum_r |K_ri| s_r )

@@ -85,8 +85,6 @@ struct rd_ctx {
     double2* coef = nullptr;  // CG-Lanczos coefficients of the last rd_solve_inactive (eq. (23) diagnostic)
     int32_t coef_cap = 0;
     bool want_ritz = false;
-    int64_t bandwidth = 0;            // max |column - row| over the entries of K
-    unsigned int* stage_flags = nullptr;  // one counter per CTA of the persistent kernel (neighbour synchronisation A -> B)
     double* d_ritz = nullptr;
     double *gram_parts = nullptr, *G = nullptr, *EW = nullptr, *cwork = nullptr, *C = nullptr;  // EW: W_I^T H W_I on request
     double *T = nullptr, *Eraw = nullptr, *E = nullptr, *CW = nullptr;  // T (W_I -> Z), E = Z^T B Z, C = E^{-1}, CW = T C T^T
@@ -439,18 +437,6 @@ int run_alg1(rd_ctx* ctx, int method, int64_t n_inactive, rd_solve_report* rep, 
         P.coef = ctx->coef;
         P.coef_cap = ctx->coef_cap;
     }
-    {   // Between the K product and the K^T product a CTA needs t only on its own rows widened by the bandwidth of K: when
-        // that reaches a few neighbouring shares, the grid barrier between the two stages is replaced by per-CTA flags
-        // (cg3.cuh publish_and_wait_neighbours).  RD_NEIGHBOUR_SYNC=0 keeps the grid barrier.
-        static const int nsync = [] { const char* e = getenv("RD_NEIGHBOUR_SYNC"); return e ? atoi(e) : 1; }();
-        const int64_t rows_per_cta = 32 * std::max<int64_t>(1, ctx->K.nslices / ctx->cg_grid);
-        const int64_t ndeps = 2 * ((ctx->bandwidth + rows_per_cta - 1) / rows_per_cta) + 2;
-        if (nsync && variant == 0 && ctx->K.nslices >= ctx->cg_grid && ndeps <= 32) {
-            CU(cudaMemsetAsync(ctx->stage_flags, 0, sizeof(unsigned int) * ctx->cg_grid, ctx->stream));
-            P.stage_flags = ctx->stage_flags;
-            P.bandwidth = ctx->bandwidth;
-        }
-    }
     CU(cudaMemsetAsync(ctx->bar, 0, sizeof(GridBarrier), ctx->stream));
     CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     void* args[] = {(void*)&P};
@@ -652,8 +638,6 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
         }
     }
     ctx->nnz = rp2[N];
-    for (int64_t r = 0; r < N; ++r)
-        for (int64_t e = rp2[r]; e < rp2[r + 1]; ++e) ctx->bandwidth = std::max<int64_t>(ctx->bandwidth, std::llabs((long long)ci2[e] - (long long)r));
     // transpose (counting sort: rows of K^T come out with ascending column = ascending row of K)
     std::vector<int64_t> tp(N + 1, 0);
     for (int64_t e = 0; e < ctx->nnz; ++e) tp[ci2[e] + 1]++;
@@ -721,7 +705,6 @@ int rd_create(rd_ctx** out, int64_t N, const int64_t* rowptr, const int32_t* col
     if (occ < 1) return fail(ctx, RD_ECUDA, "k_alg1_v3 does not fit an SM (occupancy 0)");
     ctx->cg_grid = ctx->num_sms;
     RDTRY(dalloc(ctx, &ctx->partial, (size_t)2 * SL_NSLOT * ctx->cg_grid));
-    RDTRY(dalloc(ctx, &ctx->stage_flags, (size_t)ctx->cg_grid));
     // d = diag(H), dinv
     k_diag_H<<<grid_for(ctx->KT.nslices * 32, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
         ctx->KT.view(), N, ctx->m, ctx->minv, ctx->sigma, ctx->opt.jacobi, ctx->d, ctx->dinv);
@@ -973,39 +956,15 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
 
     int64_t col_applies = 0;
     float filter_ms = 0.0f;
-    static const int wide_cb = [] { const char* e = getenv("RD_EIG_CB"); return e ? atoi(e) : 8; }();  // 16: experiment
     // columns [col0, b) of the block (col0 a multiple of the chunk width): the leading col0 columns are locked
     auto block_apply = [&](const double* Y, double c1, double cshift, double c2, const double* Yprev, double* Ynext, int col0 = 0) {
-        const int nch = nchunk - col0 / RD_EIG_CB;  // 8-column chunks to apply H to
+        const int nch = nchunk - col0 / RD_EIG_CB;
+        const dim3 gb(std::max(1, gs / std::min(nch, 4)), nch);
         const size_t o = (size_t)col0 * ld;
-        const Ell Kv = ctx->K.view(), KTv = ctx->KT.view();
-        const double* Yp = Yprev ? Yprev + o : nullptr;
-        // pairs of chunks go through the 16-column kernels (K and K^T stream once per 16 columns), an odd last chunk
-        // through the 8-column ones
-        if (wide_cb == 4) {  // experiment: 4 columns per thread, twice the warps
-            const dim3 gb(std::max(1, gs / std::min(2 * nch, 8)), 2 * nch);
-            k_blk_K<4><<<gb, kThreads, 0, ctx->stream>>>(Kv, N, ld, ctx->minv, Y + o, T + o);
-            k_blk_KT<4><<<gb, kThreads, 0, ctx->stream>>>(KTv, N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o, Yp, Ynext + o);
-            ctx->launches += 2;
-            col_applies += (int64_t)nch * RD_EIG_CB;
-            return;
-        }
-        const int wide = (wide_cb == 16) ? nch / 2 : 0;
-        if (wide > 0) {
-            const dim3 gb(std::max(1, gs / std::min(wide, 4)), wide);
-            k_blk_K<16><<<gb, kThreads, 0, ctx->stream>>>(Kv, N, ld, ctx->minv, Y + o, T + o);
-            k_blk_KT<16><<<gb, kThreads, 0, ctx->stream>>>(KTv, N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o, Yp, Ynext + o);
-            ctx->launches += 2;
-        }
-        const int rest = nch - 2 * wide;
-        if (rest > 0) {
-            const size_t o2 = o + (size_t)wide * 16 * ld;
-            const dim3 gb(std::max(1, gs / std::min(rest, 4)), rest);
-            k_blk_K<8><<<gb, kThreads, 0, ctx->stream>>>(Kv, N, ld, ctx->minv, Y + o2, T + o2);
-            k_blk_KT<8><<<gb, kThreads, 0, ctx->stream>>>(KTv, N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o2, T + o2,
-                                                          Yprev ? Yprev + o2 : nullptr, Ynext + o2);
-            ctx->launches += 2;
-        }
+        k_blk_K<<<gb, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y + o, T + o);
+        k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, c1, cshift, c2, Y + o, T + o,
+                                                   Yprev ? Yprev + o : nullptr, Ynext + o);
+        ctx->launches += 2;
         col_applies += (int64_t)nch * RD_EIG_CB;
     };
     auto gram = [&](const double* A, const double* B, double* out) {
