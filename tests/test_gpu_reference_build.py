@@ -89,3 +89,31 @@ def test_build_reference_edge_cases(rd, oracle_mod):
             g.build_reference(65)
     finally:
         g.close()
+
+
+def test_reference_work_accounting_and_tensor_probe(rd):
+    """S0's work counters (rd_reference_work) and the FP64 tensor-pipe probe (rd_probe_fp64_tensor_peak): the counters
+    exist only after an eigen-build, count whole column applies of the Chebyshev filter (at least one column per
+    degree, at most the block), and the bytes per column apply are the DESIGN.md model 3 nnz + 48 N."""
+    w = CASES["c2_48"]()
+    g = rd.RefDef.from_workload(w, rd.Options(pdas_cap=w.pdas_cap))
+    try:
+        info0 = g.reference_info()
+        assert "filter_GBs" not in info0 and info0["total_degree"] == 0
+        theta, resid, sweeps, st = g.build_reference(w.k, tol=1e-5)
+        assert st == 0
+        info = g.reference_info()
+        nnz = len(w.val)
+        assert info["filter_bytes_per_column_apply"] == 3 * nnz + 48 * w.N
+        # every sweep filters at most `block` columns with that sweep's degree; locked columns drop out
+        assert 0 < info["filter_column_applies"] <= info["block"] * info["total_degree"]
+        assert info["filter_column_applies"] >= info["total_degree"]
+        assert 0 < info["filter_ms"] <= info["build_ms"]
+        assert info["filter_GBs"] > 0
+        # an analytical reference resets the counters
+        g.build_reference_sine(w.k, list(w.dims))
+        assert "filter_GBs" not in g.reference_info()
+        tf = g.probe_fp64_tensor_peak()
+        assert 5.0 < tf < 80.0, tf  # DMMA on B200: tens of TFLOP/s; the FP64 CUDA-core path alone is far below 5
+    finally:
+        g.close()

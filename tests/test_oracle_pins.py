@@ -850,3 +850,41 @@ def test_threaded_timing_build_matches_the_plain_oracle():
     # alg1_on (line 2 built once by the caller) is the same solve as alg1
     x3, r3 = o1.alg1_on(o1.coarse(idx, W[idx]), b, np.zeros(len(idx)))
     assert np.array_equal(x1, x3) and r1["iters"] == r3["iters"]
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# the stored goldens of the larger twins (tests/golden/twin_*.json, written by make_golden_twins.py from the oracle)
+def test_golden_twins_belong_to_this_generator_and_oracle(oracle_mod):
+    """Every stored golden names the operator it was computed on (sha256 of rowptr/colidx/val/m/alpha) and the first PDAS
+    steps of the smallest case are recomputed live: a change to the input generator or to the oracle's arithmetic that is
+    not followed by regenerating the goldens fails here, on the CPU, and not only on the GPU box."""
+    import json
+
+    gdir = os.path.join(HERE, "golden")
+    names = sorted(f for f in os.listdir(gdir) if f.startswith("twin_") and f.endswith(".json"))
+    assert len(names) >= 5
+    for f in names:
+        with open(os.path.join(gdir, f)) as fh:
+            g = json.load(fh)
+        w = make_config(**g["make_config"]) if g["N"] <= 70000 else None
+        if w is not None:
+            assert w.operator_hash() == g["operator_sha256"] and w.N == g["N"] and w.k == g["k"], f
+        for q in g["queries"]:
+            assert q["status"] == 0 and max(q["kkt"]) <= 1e-6, (f, q["query"])
+            assert len(q["active_hash"]) == q["n_steps"] == len(q["n_inactive"]) == len(q["cg_iters"])
+            assert all(s == 0 for s in q["inner_status"])
+        y = np.load(os.path.join(gdir, f.replace(".json", ".npz")))
+        assert sorted(y.files) == sorted(f"y{q['query']}" for q in g["queries"])
+    # live: the first three steps of c3_32, query 0 (a few seconds of oracle time)
+    with open(os.path.join(gdir, "twin_c3_32.json")) as fh:
+        g = json.load(fh)
+    w = make_config(**g["make_config"])
+    o = oracle_mod.Oracle.from_workload(w)
+    W = np.asfortranarray(oracle_mod.sine_reference(w.dims, w.k)[-1])
+    yd, psi = w.target(0)
+    r = o.solve_query(oracle_mod.REFDEF, yd, psi, W, oracle_mod.OracleOptions(eps=g["eps"], eps_c=g["eps_c"], pdas_cap=3))
+    q = g["queries"][0]
+    assert [f"{s['active_hash']:016x}" for s in r["steps"]] == q["active_hash"][:3]
+    assert [s["n_inactive"] for s in r["steps"]] == q["n_inactive"][:3]
+    assert [s["cg_iters"] for s in r["steps"]] == q["cg_iters"][:3]
+    assert [s["rank_used"] for s in r["steps"]] == q["rank_used"][:3]
