@@ -255,6 +255,21 @@ int rd_apply_KT(rd_ctx* ctx, const double* v, double* out);
  * operator of eq. (7), out_i = (H (chi_I v))_i on I and 0 on J. */
 int rd_apply_H(rd_ctx* ctx, const double* v, const uint8_t* active, double* out);
 int rd_diag_H(rd_ctx* ctx, double* d_out);
+/* S3 without any allocation (callers under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * out = H v, or with active != NULL the masked operator of eq. (7) exactly as rd_apply_H computes it (same kernels'
+ * order of sums: bit-identical results).  The intermediate t = M^-1 K (chi_I v) lives in a file-scope
+ * `static __device__` array of RD_NOALLOC_MAX_N doubles (8 MiB, held by every GPU that loads the library until the
+ * process exits) instead of a context buffer.
+ *   v, out : N doubles, DEVICE pointers, out must not alias v; active: NULL or N bytes, DEVICE pointer.  The caller owns
+ *            all three; host pointers are RD_EINVAL (they would need a staging copy).
+ *   N > RD_NOALLOC_MAX_N is RD_EINVAL with a message in rd_last_error; rd_apply_H has no such limit.
+ * The call enqueues two kernels on the context's stream and returns WITHOUT synchronising; it calls no cudaMalloc,
+ * cudaFree or allocating library routine (the first call on a device resolves the array's address with
+ * cudaGetSymbolAddress: make that call outside a capture).  Every call on a device shares the one array, which keeps
+ * the previous call's contents: each call rewrites all N entries it reads, so nothing needs clearing, but two calls
+ * that overlap on the GPU (different streams, or two contexts) race on it.  The device of the context must be current. */
+#define RD_NOALLOC_MAX_N (1 << 20)
+int rd_apply_H_noalloc(rd_ctx* ctx, const double* v, const uint8_t* active, double* out);
 /* Algorithm 1 on one inactive system (S1-S5): active = N bytes; b, x: N doubles in full-domain indexing
  * (entries on J are ignored on input and 0 on output); x holds x0 on entry.  Deflated methods use the
  * stored reference and, for RD_ZEROEXT, update the zero-extension history. */

@@ -6,5 +6,5 @@ importing works anywhere, creating a context without the library or without a CU
 """
 from .binding import (  # noqa: F401
     RefDef, RefDefError, Options, JACOBI_CG, REFDEF, ZEROEXT, INIT_PAPER, INIT_ALL_ACTIVE,
-    INIT_ALL_INACTIVE, INIT_GIVEN, STATUS_NAMES, load_library, exported_symbols, LIB_PATH,
+    INIT_ALL_INACTIVE, INIT_GIVEN, STATUS_NAMES, load_library, exported_symbols, LIB_PATH, NOALLOC_MAX_N,
 )

@@ -23,7 +23,10 @@ SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
            "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
-           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
+           "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_apply_H_noalloc", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
+
+
+NOALLOC_MAX_N = 1 << 20  # RD_NOALLOC_MAX_N of include/refdef.h
 
 
 class RefDefError(RuntimeError):
@@ -118,6 +121,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_apply_K.argtypes = [vp, vp, vp]
     lib.rd_apply_KT.argtypes = [vp, vp, vp]
     lib.rd_apply_H.argtypes = [vp, vp, vp, vp]
+    lib.rd_apply_H_noalloc.argtypes = [vp, vp, vp, vp]
     lib.rd_diag_H.argtypes = [vp, vp]
     lib.rd_solve_inactive.argtypes = [vp, i32, vp, vp, vp, C.POINTER(_SolveReport)]
     lib.rd_coarse_setup.argtypes = [vp, i32, vp, vp, vp, vp, C.POINTER(i32), C.POINTER(dbl), C.POINTER(i32)]
@@ -360,6 +364,12 @@ class RefDef:
 
     def apply_H(self, v, active=None, out=None):
         return self._apply(self._lib.rd_apply_H, v, out, _ptr(active))
+
+    def apply_H_noalloc(self, v, active, out):
+        """rd_apply_H_noalloc: device tensors only, `out` given by the caller, nothing allocated, NOT synchronised
+        (N <= NOALLOC_MAX_N; the scratch is a static device array shared by every call on the device)."""
+        self._check(self._lib.rd_apply_H_noalloc(self._h, _ptr(v), _ptr(active), _ptr(out)), "rd_apply_H_noalloc")
+        return out
 
     def diag_H(self):
         d = np.empty(self.N)

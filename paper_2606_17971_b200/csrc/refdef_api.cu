@@ -1747,3 +1747,84 @@ int rd_solve_query(rd_ctx* ctx, int32_t method, const double* y_d, const double*
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// rd_apply_H_noalloc: S3 for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc).  The intermediate t = M^{-1} K (chi_I v) of eq. (5) lives in a file-scope device array instead of a
+// context buffer; the mask chi_I is applied inside the gather, so no masked copy of v is needed either.
+//
+// g_noalloc_t is a DEVICE symbol: in host code its name is a host-side stand-in, not a device address.  The address the
+// kernels get comes from cudaGetSymbolAddress, taken once per device with that device current (noalloc_scratch below).
+namespace {
+
+__device__ __align__(256) double g_noalloc_t[RD_NOALLOC_MAX_N];  // 8 MiB on every GPU that loads the library, until exit
+
+constexpr int kMaxDevices = 64;
+double* g_noalloc_ptr[kMaxDevices];  // per device: the address of g_noalloc_t on it, NULL until resolved
+
+// t_r = (1/m_r) sum_c K_rc (act_c ? 0 : v_c): k_apply_K with chi_I folded into the gather.  Same order of the sums as
+// ell_row_dot (groups of four entries, one fma chain), so the result equals k_mask_copy + k_apply_K bit for bit.
+__global__ void k_apply_K_masked(Ell K, int64_t N, const double* __restrict__ minv, const uint8_t* __restrict__ act,
+                                 const double* __restrict__ v, double* __restrict__ t)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t gw = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwt = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t s = gw; s < K.nslices; s += nwt) {
+        const int64_t row = s * RD_SLICE + lane;
+        const int64_t o = K.off[s];
+        const int wd = (int)((K.off[s + 1] - o) >> 5);
+        const int32_t* cp = K.col + o + lane;
+        const double* vp = K.val + o + lane;
+        double acc = 0.0;
+        for (int e = 0; e < wd; ++e) {
+            const int c = ldg_i32(cp + e * 32);
+            const double a = ldg_f64(vp + e * 32);
+            const double x = (act && act[c]) ? 0.0 : v[c];
+            acc = fma(a, x, acc);
+        }
+        if (row < N) t[row] = acc * ldg_f64(minv + row);
+    }
+}
+
+// The device address of g_noalloc_t on `device` (which must be current).  No allocation: the array is part of the module.
+int noalloc_scratch(rd_ctx* ctx, int device, double** out)
+{
+    if (device < 0 || device >= kMaxDevices) return fail(ctx, RD_EINVAL, "device ordinal %d is outside 0..%d", device, kMaxDevices - 1);
+    if (!g_noalloc_ptr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_t);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(ctx, RD_ECUDA, "cudaGetSymbolAddress(g_noalloc_t) on device %d: %s", device, cudaGetErrorString(e));
+        }
+        g_noalloc_ptr[device] = (double*)p;  // the same value whichever thread stores it
+    }
+    *out = g_noalloc_ptr[device];
+    return RD_OK;
+}
+
+}  // namespace
+
+extern "C" int rd_apply_H_noalloc(rd_ctx* ctx, const double* v, const uint8_t* active, double* out)
+{
+    if (!ctx || !v || !out) return RD_EINVAL;
+    if (ctx->N > (int64_t)RD_NOALLOC_MAX_N)
+        return fail(ctx, RD_EINVAL, "rd_apply_H_noalloc: N = %lld exceeds RD_NOALLOC_MAX_N = %lld (the static scratch); use rd_apply_H",
+                    (long long)ctx->N, (long long)RD_NOALLOC_MAX_N);
+    if (v == out) return fail(ctx, RD_EINVAL, "rd_apply_H_noalloc: out must not alias v");
+    if (!is_device_ptr(v) || !is_device_ptr(out) || (active && !is_device_ptr(active)))
+        return fail(ctx, RD_EINVAL, "rd_apply_H_noalloc takes device pointers only (a host buffer would need a staging copy)");
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev != ctx->device) return fail(ctx, RD_EINVAL, "rd_apply_H_noalloc: device %d is current, the context lives on device %d", dev, ctx->device);
+    double* t = nullptr;
+    RDTRY(noalloc_scratch(ctx, dev, &t));
+    // every row of t below N is rewritten by the first kernel before the second reads it: nothing has to start at zero
+    const int g = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    k_apply_K_masked<<<g, kThreads, 0, ctx->stream>>>(ctx->K.view(), ctx->N, ctx->minv, active, v, t);
+    k_apply_KT_H<<<g, kThreads, 0, ctx->stream>>>(ctx->KT.view(), ctx->N, ctx->m, ctx->sigma, active, v, t, out);
+    ctx->launches += 2;
+    CU(cudaGetLastError());
+    return RD_OK;
+}
