@@ -162,6 +162,28 @@ def build_analytical_reference(g, w):
 _COARSE = {}
 
 
+KAPPA_REF = 1.0  # conductivity of the homogeneous comparison medium of the LOBPCG preconditioner: the generator's solid
+DEFAULT_EIG_SOLVER = "lobpcg"  # steady Cartesian grids; everything else takes the filter (eig_solver_for)
+
+
+def eig_solver_for(w, reference):
+    """Which of the two eigensolvers of S0 builds the 'eig' reference: the sine-preconditioned LOBPCG needs a steady
+    Cartesian grid (csrc/lobpcg.cuh); everything else, and 'eig-filter', takes the Chebyshev-filtered subspace iteration."""
+    if reference == "eig-filter" or w.nt != 1:
+        return "filter"
+    if reference == "eig-lobpcg":
+        return "lobpcg"
+    return DEFAULT_EIG_SOLVER
+
+
+def build_eig_reference(g, w, reference, ref_tol, sweeps=60):
+    """The k lowest eigenvectors of H (BASELINE.json's reference) to ||H w - theta w|| <= ref_tol theta.
+    Returns (theta, residuals, iterations or sweeps, status)."""
+    if eig_solver_for(w, reference) == "lobpcg":
+        return g.build_reference_lobpcg(w.k, w.dims, kappa_ref=KAPPA_REF, tol=ref_tol, max_iters=600)
+    return g.build_reference(w.k, tol=ref_tol, max_block_iters=sweeps)
+
+
 def build_coarse_reference(g, w, ref_tol, coarsen=2):
     """The paper's coarse-mesh reference (section 2.2.2): Jacobi-scaled low modes of the operator on a grid
     with 1/coarsen of the cells per axis (a second context, rd_build_reference_scaled), P1 prolongation and column
@@ -249,7 +271,7 @@ class Sequence:
             elif self.reference == "eig-scaled":  # Jacobi-scaled generalized problem
                 _, _, _, st = self.g.build_reference_scaled(self.w.k, tol=self.ref_tol, max_block_iters=60)
             else:
-                _, _, _, st = self.g.build_reference(self.w.k, tol=self.ref_tol, max_block_iters=60)
+                _, _, _, st = build_eig_reference(self.g, self.w, self.reference, self.ref_tol)
             info = self.g.reference_info()
             self.ref_builds += 1
             self.ref_ms += info["build_ms"] + extra_ms
@@ -451,7 +473,9 @@ def run_ours(args):
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(mx_total / args.steps, 3),
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args, w, cap), "method": args.method, "parallelism": f"replicas x{world}",
-                       "alg1_variant": args.alg1_variant, "reference": args.reference, "reference_tol": args.ref_tol, "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
+                       "alg1_variant": args.alg1_variant, "reference": args.reference, "reference_tol": args.ref_tol,
+                       "eig_solver": (eig_solver_for(w, args.reference) if args.reference in ("eig", "eig-filter", "eig-lobpcg") else None),
+                       "sigma": "alpha (DESIGN.md reading A1)", "eps": 1e-8,
                        "l2": "flushed between steps (256 MiB write)" + ("; the loop's working set is far larger than the 126 MB L2" if w.N > 1000000 else
                                                                           "; the loop's working set (HW, K, K^T, vectors: about 120 MB) is the size of the L2")},
             # time-to-solution bookkeeping: a query counts as converged only if PDAS stopped on a repeated
@@ -521,9 +545,12 @@ def run_loop(args):
             st, ms_c = build_coarse_reference(g, w, args.ref_tol)
             ref = dict(g.reference_info(), kind="coarse eigenproblem + P1 prolongation (PAPER.md:176)", status=st, coarse_eig_ms=ms_c)
         else:
-            build = g.build_reference_scaled if args.reference == "eig-scaled" else g.build_reference
-            _, resid, sweeps, st = build(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
-            ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
+            if args.reference == "eig-scaled":
+                _, resid, sweeps, st = g.build_reference_scaled(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
+            else:
+                _, resid, sweeps, st = build_eig_reference(g, w, args.reference, args.ref_tol, args.ref_sweeps)
+            ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()),
+                       solver=eig_solver_for(w, args.reference))
     yd = w._target(1000 * w.config)
     b = torch.from_numpy(w.m * yd).to(dev)
     act = torch.zeros(w.N, dtype=torch.uint8, device=dev)
@@ -589,9 +616,10 @@ def run_setup(args):
     g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap), stream=stream.cuda_stream)
     peak_tf = g.probe_fp64_tensor_peak()
     ref = None
-    if args.reference == "eig":
-        _, resid, sweeps, st = g.build_reference(w.k, tol=args.ref_tol, max_block_iters=args.ref_sweeps)
-        ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()))
+    if args.reference in ("eig", "eig-filter", "eig-lobpcg"):
+        _, resid, sweeps, st = build_eig_reference(g, w, args.reference, args.ref_tol, args.ref_sweeps)
+        ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()),
+                   solver=eig_solver_for(w, args.reference))
     else:
         build_analytical_reference(g, w)
         ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
@@ -652,7 +680,7 @@ def run_replay(args):
     elif args.reference == "eig-scaled":
         g.build_reference_scaled(w.k, tol=args.ref_tol, max_block_iters=60)
     else:
-        g.build_reference(w.k, tol=args.ref_tol, max_block_iters=60)
+        build_eig_reference(g, w, args.reference, args.ref_tol)
     ref = g.reference_info()
     systems = []
     nq = min(w.n_queries, args.steps)
@@ -831,8 +859,10 @@ def build_parser():
     ap.add_argument("--twin", default=None)
     ap.add_argument("--method", default="refdef", choices=list(METHODS))
     ap.add_argument("--ref-tol", type=float, default=1e-3)
-    ap.add_argument("--reference", default="eig", choices=["eig", "eig-scaled", "sine", "coarse"],
-                    help="eig: k lowest eigenvectors of H (rd_build_reference, BASELINE.json); sine: the paper's analytical "
+    ap.add_argument("--reference", default="eig", choices=["eig", "eig-filter", "eig-lobpcg", "eig-scaled", "sine", "coarse"],
+                    help="eig: k lowest eigenvectors of H (BASELINE.json) by the default eigensolver; eig-filter: by Chebyshev-filtered "
+                         "subspace iteration (rd_build_reference); eig-lobpcg: by sine-preconditioned LOBPCG (rd_build_reference_lobpcg, "
+                         "steady Cartesian grids); sine: the paper's analytical "
                          "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4); "
                          "coarse: Jacobi-scaled modes of the half-resolution operator, P1-prolonged (PAPER.md:176)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="host-buffer queries after the timed region; 0 = one full pass of the sequence")

@@ -181,6 +181,17 @@ int rd_probe_fp64_tensor_peak(rd_ctx* ctx, double* tflops);
  * receives the generalized eigenvalues, the residual test is ||H w - mu D w|| in the scaled coordinates. */
 int rd_build_reference_scaled(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_iters, double* mu_out,
                               double* resid_out, int32_t* iters_out);
+/* rd_build_reference for operators on a Cartesian grid of the unit box (dims as in rd_build_reference_sine): the same
+ * k lowest eigenpairs of H (same tolerance test, same outputs, same stored reference) by a locally optimal block
+ * preconditioned CG (LOBPCG) whose preconditioner is the exact inverse of the HOMOGENEOUS operator of that grid,
+ * T = S^T diag(1 / (mbar (1 + sigma kappa_ref^2 mu^2))) S, with S the products of the 1-D sine vectors of eq. (15)
+ * and mu their Laplacian eigenvalues, mbar the mean of m; S is applied axis by axis as dense
+ * products on the FP64 tensor cores.  kappa_ref > 0: the conductivity of the homogeneous comparison medium (the
+ * background conductivity of the problem; it changes the number of iterations, never the result).  max_iters: cap on
+ * LOBPCG iterations (RD_ECAP as a soft status, the best block so far stays as the reference); iters_out: iterations
+ * used.  The result is checked with a freshly applied H before RD_OK is returned.  3 (k + guard) <= 256 and <= N. */
+int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int32_t max_iters, int32_t ndim, const int64_t* dims,
+                              double kappa_ref, double* theta_out, double* resid_out, int32_t* iters_out);
 /* The analytical Cartesian spatial reference of the paper (section 2.2.3, eq. (15)) for steady
  * problems on a Cartesian grid of dims[0] x ... x dims[ndim-1] cells (ndim <= 3, x = dims[0] fastest, product = N,
  * else RD_EINVAL): the k lowest products of the 1-D sine modes of the constant-coefficient Dirichlet Laplacian,

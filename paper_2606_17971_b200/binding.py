@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_lobpcg", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_apply_H_noalloc", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
 
 
@@ -105,6 +105,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
     lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_scaled.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
+    lib.rd_build_reference_lobpcg.argtypes = [vp, i32, dbl, i32, i32, vp, dbl, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
     lib.rd_build_reference_spacetime_cover.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
@@ -239,6 +240,19 @@ class RefDef:
                          soft_ok=True)
         self.k = k
         return mu, resid, it.value, st
+
+    def build_reference_lobpcg(self, k, dims, kappa_ref=1.0, tol=1e-3, max_iters=500):
+        """k lowest eigenvectors of H by LOBPCG with the sine-transform preconditioner of the homogeneous grid operator.
+        Returns (theta, relative residuals, iterations, status); status -6 = not converged within max_iters."""
+        dims = np.ascontiguousarray(dims, dtype=np.int64)
+        theta = np.zeros(k)
+        resid = np.zeros(k)
+        it = C.c_int32(0)
+        st = self._check(self._lib.rd_build_reference_lobpcg(self._h, k, tol, max_iters, len(dims), dims.ctypes.data,
+                                                             float(kappa_ref), theta.ctypes.data, resid.ctypes.data,
+                                                             C.byref(it)), "rd_build_reference_lobpcg", soft_ok=True)
+        self.k = k
+        return theta, resid, it.value, st
 
     def build_reference_sine(self, k, dims):
         """Analytical Cartesian reference: dims = cells per axis, x first.  Returns (mu, modes)."""

@@ -144,11 +144,14 @@ __device__ __forceinline__ void dmma_m8n8k4(double& d0, double& d1, double a, do
                  : "d"(a), "d"(b));
 }
 
+// upper_only: the product is symmetric (A^T B with B = A or B = H A) and only the 64 x 64 tiles on or above the diagonal
+// are formed; the caller mirrors them (k_mirror_upper_tiles).
 __global__ void __launch_bounds__(256) k_gram_dmma(int64_t N, int p, int q, const double* A, int64_t lda,
-                                                   const double* B, int64_t ldb, double* Cpart)
+                                                   const double* B, int64_t ldb, double* Cpart, int upper_only = 0)
 {
     __shared__ double sA[64 * RD_GRAM_LD];
     __shared__ double sB[64 * RD_GRAM_LD];
+    if (upper_only && blockIdx.z < blockIdx.y) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int i0 = blockIdx.y * 64, j0 = blockIdx.z * 64;
     const int pa = min(64, p - i0), qb = min(64, q - j0);
@@ -212,6 +215,15 @@ __global__ void __launch_bounds__(256) k_dmma_peak_probe(int iters, double seed,
 #pragma unroll
     for (int t = 0; t < 8; ++t) s += acc[t][0] + acc[t][1];
     if (s == 123.456) sink[0] = s;  // never true: keeps the loop alive
+}
+
+// G (p x p): the 64 x 64 tiles below the diagonal <- the transposes of the tiles above it
+__global__ void k_mirror_upper_tiles(int p, double* G)
+{
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < p * p; e += gridDim.x * blockDim.x) {
+        const int i = e % p, j = e / p;
+        if ((i >> 6) > (j >> 6)) G[e] = G[j + (size_t)i * p];
+    }
 }
 
 // out[e] = sum over parts of part[part][e], fixed order (deterministic)

@@ -21,6 +21,7 @@
 #include "transient.cuh"
 #include "coarse.cuh"
 #include "eigs.cuh"
+#include "lobpcg.cuh"
 #include "pdas.cuh"
 
 using namespace rd;
@@ -1827,4 +1828,355 @@ extern "C" int rd_apply_H_noalloc(rd_ctx* ctx, const double* v, const uint8_t* a
     ctx->launches += 2;
     CU(cudaGetLastError());
     return RD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// S0, second eigensolver: LOBPCG preconditioned by the inverse of the homogeneous grid operator (lobpcg.cuh).
+namespace {
+
+struct SineAxis {
+    int n = 0;
+    int64_t rs = 1;  // stride of this axis in the vector (product of the faster dims)
+    double *S = nullptr, *St = nullptr, *mu = nullptr;
+};
+
+template <bool AM, bool BN>
+void launch_gemm(cudaStream_t st, int tn, int M, int Nn, int Kk, int nb1, int nb2, GemmOp A, GemmOp B, GemmOp E, GemmOp D)
+{
+    if (tn == 10) {
+        const dim3 g((M + 63) / 64, (Nn + 79) / 80, nb1 * nb2);
+        k_dgemm_dmma<AM, BN, 10><<<g, 256, 0, st>>>(M, Nn, Kk, nb2, A, B, E, D);
+    } else {
+        const dim3 g((M + 63) / 64, (Nn + 63) / 64, nb1 * nb2);
+        k_dgemm_dmma<AM, BN, 8><<<g, 256, 0, st>>>(M, Nn, Kk, nb2, A, B, E, D);
+    }
+}
+inline int tile_for(int n) { return (((n + 79) / 80) * 80 < ((n + 63) / 64) * 64) ? 10 : 8; }
+
+// Y[:, 0:ncols] <- transform along one axis (forward: coefficients S y; inverse: S^T y), from `in` to `out`
+int sine_axis_pass(rd_ctx* ctx, const SineAxis& ax, bool inverse, int64_t N, int64_t ld, int ncols, const double* in, double* out)
+{
+    const double* Mat = inverse ? ax.St : ax.S;  // Mat[o][i], row-major
+    const int n = ax.n;
+    const GemmOp none{nullptr, 0, 0, 0, 0};
+    if (ax.rs == 1) {
+        // D[l, o] = sum_i In[l n + i] Mat[o][i]: lines are the m index, both operands contiguous along the contraction
+        const int64_t L = N / n;
+        const GemmOp A{in, n, 1, ld, 0}, B{Mat, 1, n, 0, 0}, D{out, n, 1, ld, 0};
+        launch_gemm<false, false>(ctx->stream, tile_for(n), (int)L, n, n, ncols, 1, A, B, none, D);
+    } else {
+        // D[o, l] = sum_i Mat[o][i] In[i rs + l] for every slab of rs n entries
+        const int64_t slab = ax.rs * n, nslab = N / slab;
+        if ((int64_t)ncols * nslab > 65535) return fail(ctx, RD_EINVAL, "sine preconditioner: %lld batches exceed the grid limit", (long long)(ncols * nslab));
+        const GemmOp A{Mat, n, 1, 0, 0}, B{in, ax.rs, 1, ld, slab}, D{out, ax.rs, 1, ld, slab};
+        launch_gemm<false, true>(ctx->stream, tile_for((int)std::min<int64_t>(ax.rs, 1 << 20)), n, (int)ax.rs, n, ncols, (int)nslab, A, B, none, D);
+    }
+    ctx->launches++;
+    return RD_OK;
+}
+
+}  // namespace
+
+extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int32_t max_iters, int32_t ndim, const int64_t* dims,
+                                         double kappa_ref, double* theta_out, double* resid_out, int32_t* iters_out)
+{
+    if (!ctx || !dims || k < 1 || k > RD_MAX_K || !(tol > 0.0) || max_iters < 1 || ndim < 1 || ndim > 3 || !(kappa_ref > 0.0))
+        return RD_EINVAL;
+    const int64_t N = ctx->N, ld = ctx->ldw;
+    int64_t prod = 1;
+    for (int a = 0; a < ndim; ++a) {
+        if (dims[a] < 2 || dims[a] > 4096) return fail(ctx, RD_EINVAL, "dims[%d] = %lld", a, (long long)dims[a]);
+        prod *= dims[a];
+    }
+    if (prod != N) return fail(ctx, RD_EINVAL, "prod(dims) = %lld but N = %lld", (long long)prod, (long long)N);
+    int b = (k + std::max(8, k / 4) + 7) & ~7;
+    while (b - 8 >= k && 3 * b > N) b -= 8;
+    if (3 * b > N || 3 * b > RD_DENSE_MAXN) return fail(ctx, RD_EINVAL, "block of %d vectors: 3 b must not exceed min(N, %d)", b, RD_DENSE_MAXN);
+    const auto t_begin = std::chrono::steady_clock::now();
+
+    struct Scratch {
+        std::vector<void*> p;
+        ~Scratch() { for (void* q : p) cudaFree(q); }
+    } scratch;
+    auto salloc = [&](double** out, size_t count) -> int {
+        void* q = nullptr;
+        cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, RD_ENOMEM, "cudaMalloc(%zu doubles): %s", count, cudaGetErrorString(e)); }
+        scratch.p.push_back(q);
+        cudaMemsetAsync(q, 0, std::max<size_t>(count, 1) * sizeof(double), ctx->stream);
+        *out = (double*)q;
+        return RD_OK;
+    };
+    const size_t nb = (size_t)ld * b;
+    const int ns_max = 3 * b;
+    double *S, *HS, *Xn, *HXn, *Pn, *HPn, *tmp, *parts, *Gs, *Gh, *work, *Cm, *d_theta, *rparts, *rsum, *d_info;
+    RDTRY(salloc(&S, 3 * nb));
+    RDTRY(salloc(&HS, 3 * nb));
+    RDTRY(salloc(&Xn, nb));
+    RDTRY(salloc(&HXn, nb));
+    RDTRY(salloc(&Pn, nb));
+    RDTRY(salloc(&HPn, nb));
+    RDTRY(salloc(&tmp, nb));
+    const int nparts = ctx->num_sms * 2;
+    RDTRY(salloc(&parts, (size_t)nparts * ns_max * ns_max));
+    RDTRY(salloc(&Gs, (size_t)ns_max * ns_max));
+    RDTRY(salloc(&Gh, (size_t)ns_max * ns_max));
+    RDTRY(salloc(&work, (size_t)7 * ns_max * ns_max + 1024));
+    RDTRY(salloc(&Cm, (size_t)ns_max * b));
+    RDTRY(salloc(&d_theta, b));
+    const int rgrid = ctx->num_sms * 2;
+    RDTRY(salloc(&rparts, (size_t)rgrid * b));
+    RDTRY(salloc(&rsum, b));
+    RDTRY(salloc(&d_info, 4));  // four ints (kept, kept rounded up to even, Cholesky flag, unused), then the grid barrier of k_jacobi_grid
+    // the preconditioner: per-axis sine tables, the mean lumped mass
+    SineAxis ax[3];
+    {
+        int64_t rs = 1;
+        for (int a = 0; a < ndim; ++a) {
+            ax[a].n = (int)dims[a];
+            ax[a].rs = rs;
+            rs *= dims[a];
+            RDTRY(salloc(&ax[a].S, (size_t)dims[a] * dims[a]));
+            RDTRY(salloc(&ax[a].St, (size_t)dims[a] * dims[a]));
+            RDTRY(salloc(&ax[a].mu, (size_t)dims[a]));
+            k_sine_axis_tables<<<grid_for(dims[a] * dims[a], kThreads, 1024), kThreads, 0, ctx->stream>>>(ax[a].n, ax[a].S, ax[a].St, ax[a].mu);
+            ctx->launches++;
+        }
+    }
+    double mbar = 0.0;
+    {
+        std::vector<double> mh(N);
+        CU(cudaMemcpyAsync(mh.data(), ctx->m, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        long double s = 0.0L;
+        for (int64_t i = 0; i < N; ++i) s += mh[i];
+        mbar = (double)(s / (long double)N);
+    }
+    const double sk2 = ctx->sigma * kappa_ref * kappa_ref;
+    std::vector<double> theta(b), res2(b), resid(b, INFINITY);
+    const int gs = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
+    int64_t col_applies = 0;
+    int64_t prec_applies = 0;
+
+    auto block_apply = [&](const double* Y, double* HY, int nc) {  // HY = H Y for nc columns (a multiple of 8); tmp holds M^{-1} K Y
+        const int nch = nc / RD_EIG_CB;
+        const dim3 gb(std::max(1, gs / std::min(nch, 4)), nch);
+        k_blk_K<<<gb, kThreads, 0, ctx->stream>>>(ctx->K.view(), N, ld, ctx->minv, Y, tmp);
+        k_blk_KT<<<gb, kThreads, 0, ctx->stream>>>(ctx->KT.view(), N, ld, ctx->m, ctx->sigma, 1.0, 0.0, 0.0, Y, tmp, nullptr, HY);
+        ctx->launches += 2;
+        col_applies += nc;
+    };
+    auto precondition = [&](double* Y, int nc) -> int {  // Y <- T Y in place (nc columns), tmp is the other buffer of the ping-pong
+        double* cur = Y;
+        double* oth = tmp;
+        for (int a = 0; a < ndim; ++a) {
+            RDTRY(sine_axis_pass(ctx, ax[a], false, N, ld, nc, cur, oth));
+            std::swap(cur, oth);
+        }
+        k_sine_scale<<<grid_for(N, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(
+            N, ld, nc, ax[0].n, ndim > 1 ? ax[1].n : 1, ax[0].mu, ndim > 1 ? ax[1].mu : nullptr, ndim > 2 ? ax[2].mu : nullptr, mbar, sk2, cur);
+        ctx->launches++;
+        for (int a = ndim - 1; a >= 0; --a) {
+            RDTRY(sine_axis_pass(ctx, ax[a], true, N, ld, nc, cur, oth));
+            std::swap(cur, oth);
+        }
+        // 2 ndim passes: the result is back in Y
+        prec_applies += nc;
+        return RD_OK;
+    };
+    auto gram = [&](int p, const double* A, const double* B, double* out) {  // out (p x p) = A^T B
+        const dim3 gg(nparts, (p + 63) / 64, (p + 63) / 64);
+        k_gram_dmma<<<gg, 256, 0, ctx->stream>>>(N, p, p, A, ld, B, ld, parts, 1);  // symmetric products only: upper tiles
+        k_reduce_parts<<<grid_for((int64_t)p * p, kThreads, 64), kThreads, 0, ctx->stream>>>(nparts, (int64_t)p * p, parts, out);
+        k_mirror_upper_tiles<<<grid_for((int64_t)p * p, kThreads, 64), kThreads, 0, ctx->stream>>>(p, out);
+        ctx->launches += 3;
+    };
+    // Out (N x nout) = A[:, 0:kk] Cs (kk x nout, column-major with leading dimension ldc) (+ Add)
+    auto tall_mult = [&](const double* A, int kk, const double* Cs, int ldc, const double* Add, double* Out, int nout) {
+        const GemmOp a{A, 1, ld, 0, 0}, c{Cs, 1, ldc, 0, 0}, e{Add, 1, ld, 0, 0}, d{Out, 1, ld, 0, 0};
+        launch_gemm<true, false>(ctx->stream, 10, (int)N, nout, kk, 1, 1, a, c, e, d);
+        ctx->launches++;
+    };
+    auto copy_cols = [&](double* dst, const double* src, int nc) -> int {
+        if (nc > 0) CU(cudaMemcpyAsync(dst, src, (size_t)nc * ld * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+        return RD_OK;
+    };
+    double* X = S;
+    double* HX = HS;
+    // the ns x ns part: two grid-parallel Jacobi eigensolves and the small products between them (lobpcg.cuh)
+    auto small_rr = [&](int ns) -> int {
+        const size_t nn = (size_t)ns_max * ns_max;
+        double *A0 = work, *A1 = work + nn, *Vj = work + 2 * nn, *Tm = work + 3 * nn, *GhS = work + 4 * nn, *Q = work + 5 * nn;
+        double* dsc = work + 6 * nn;
+        double* jpart = work + 6 * nn + 512;
+        GridBarrier* bar = (GridBarrier*)(d_info + 2);  // zero-initialised, returns to its idle state after every launch
+        int* info = (int*)d_info;
+        const int gsm = grid_for((int64_t)ns * ns, kThreads, 256);
+        k_rr_scale<<<gsm, kThreads, 0, ctx->stream>>>(ns, Gs, Gh, dsc, A0, GhS);
+        CU(cudaMemcpyAsync(A1, A0, (size_t)ns * ns * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));  // the Cholesky works on a copy
+        k_rr_chol<<<1, 1024, 0, ctx->stream>>>(ns, A1, dsc, Q, Tm, info);
+        int n_arg = ns;
+        const int* n_ptr = nullptr;
+        const int* skip1 = info + 2;
+        void* args1[] = {&n_arg, &n_ptr, &A0, &A1, &Vj, &bar, &jpart, &skip1};
+        CU(cudaLaunchCooperativeKernel((const void*)k_jacobi_grid, dim3(ns / 2), dim3(256), args1, 0, ctx->stream));
+        k_rr_select<<<1, 1024, 0, ctx->stream>>>(ns, A0, Vj, dsc, Tm, info);
+        k_rr_q<<<gsm, kThreads, 0, ctx->stream>>>(ns, info, GhS, Tm, Q);
+        k_rr_a<<<gsm, kThreads, 0, ctx->stream>>>(ns, info, Tm, Q, A0);
+        int n_zero = 0;
+        const int* n_ptr2 = info + 1;
+        const int* skip2 = nullptr;
+        void* args2[] = {&n_zero, &n_ptr2, &A0, &A1, &Vj, &bar, &jpart, &skip2};
+        CU(cudaLaunchCooperativeKernel((const void*)k_jacobi_grid, dim3(ns / 2), dim3(256), args2, 0, ctx->stream));
+        k_rr_finish<<<1, 1024, 0, ctx->stream>>>(ns, b, info, A0, Vj, Tm, Cm, d_theta);
+        ctx->launches += 8;
+        return RD_OK;
+    };
+
+    // ---- start: T applied to a seeded random block (smooth), orthonormalised twice, Rayleigh-Ritz
+    k_rand_block<<<grid_for(N * b, kThreads, big_grid(ctx)), kThreads, 0, ctx->stream>>>(N, ld, b, 0x5EEDULL, X);
+    ctx->launches++;
+    RDTRY(precondition(X, b));
+    auto orthonormalise = [&]() -> int {
+        gram(b, X, X, Gs);
+        k_orth_small<<<1, 1024, 0, ctx->stream>>>(b, Gs, work, Cm);
+        ctx->launches++;
+        tall_mult(X, b, Cm, b, nullptr, Xn, b);
+        return copy_cols(X, Xn, b);
+    };
+    RDTRY(orthonormalise());
+    RDTRY(orthonormalise());
+    auto fresh_ritz = [&]() -> int {  // HX = H X, then X <- X V, HX <- HX V with V from X^T H X; theta on the device
+        block_apply(X, HX, b);
+        gram(b, X, HX, Gs);
+        k_rr_small<<<1, 1024, 0, ctx->stream>>>(b, Gs, work, Cm, d_theta);
+        ctx->launches++;
+        tall_mult(X, b, Cm, b, nullptr, Xn, b);
+        tall_mult(HX, b, Cm, b, nullptr, HXn, b);
+        RDTRY(copy_cols(X, Xn, b));
+        return copy_cols(HX, HXn, b);
+    };
+    RDTRY(fresh_ritz());
+    int iters = 0, status = RD_ECAP;
+    const bool dbg = std::getenv("RD_LOBPCG_DEBUG") != nullptr;  // per-iteration trace and phase times on stderr (synchronises)
+    double ph_ms[6] = {0, 0, 0, 0, 0, 0};  // residual, preconditioner, H apply, Gram, small dense, tall products + copies
+    auto t_last = std::chrono::steady_clock::now();
+    auto phase = [&](int q) {
+        if (!dbg) return;
+        cudaStreamSynchronize(ctx->stream);
+        const auto t = std::chrono::steady_clock::now();
+        ph_ms[q] += std::chrono::duration<double, std::milli>(t - t_last).count();
+        t_last = t;
+    };
+    bool verified = true;  // the residuals about to be computed come from a freshly applied H X
+    // Locking: the leading Ritz vectors that pass the test (whole chunks of 8) stay in X and in the Rayleigh-Ritz but get no
+    // new search directions: W and P have na = b - nl columns, the basis b + 2 na.  nl never decreases between restarts.
+    int nl = 0;        // locked leading columns
+    int np_cols = 0;   // columns of P' (in Pn / HPn) from the last iteration; they belong to X columns [b - np_cols, b)
+    CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+    for (int it = 0; it <= max_iters; ++it) {
+        // residuals R = HX - X theta: norms of all b columns, R itself for the active ones into the W slot (columns b ..)
+        int nl_new = nl;
+        k_resid_write_parts<<<rgrid, 256, 0, ctx->stream>>>(N, ld, b, X, HX, d_theta, Xn, rparts);
+        k_reduce_parts<<<1, kThreads, 0, ctx->stream>>>(rgrid, b, rparts, rsum);
+        ctx->launches += 2;
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(theta.data(), d_theta, b * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaMemcpyAsync(res2.data(), rsum, b * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        bool ok = true;
+        if (dbg) {
+            int info_h[2] = {0, 0};
+            cudaMemcpy(info_h, d_info, sizeof info_h, cudaMemcpyDeviceToHost);
+            double mx = 0.0;
+            for (int j = 0; j < k; ++j) mx = std::max(mx, std::sqrt(std::max(res2[j], 0.0)) / std::fabs(theta[j]));
+            fprintf(stderr, "lobpcg it %d: nl %d kept %d max rel resid %.3e theta[0] %.6e theta[k-1] %.6e | ms resid %.1f prec %.1f H %.1f gram %.1f dense %.1f mult %.1f\n",
+                    it, nl, info_h[0], mx, theta[0], theta[k - 1], ph_ms[0], ph_ms[1], ph_ms[2], ph_ms[3], ph_ms[4], ph_ms[5]);
+            t_last = std::chrono::steady_clock::now();
+        }
+        for (int j = 0; j < b; ++j) {
+            if (j < k && (!(theta[j] > 0.0) || !std::isfinite(theta[j]))) return fail(ctx, RD_ENOTSPD, "Ritz value %d = %g", j, theta[j]);
+            resid[j] = std::sqrt(std::max(res2[j], 0.0)) / std::fabs(theta[j]);
+            if (j < k && !(resid[j] <= tol)) ok = false;
+        }
+        if (ok && verified) { status = RD_OK; break; }
+        if (ok) {
+            // the recurrence of HX passed: confirm with a freshly applied operator and a fresh Rayleigh-Ritz before stopping
+            RDTRY(orthonormalise());
+            RDTRY(fresh_ritz());
+            np_cols = 0;  // P's companion HP no longer matches the rotated block
+            nl = 0;
+            verified = true;
+            continue;
+        }
+        verified = false;
+        if (it == max_iters) break;
+        iters = it + 1;
+        if ((it & 15) == 15) {
+            // the blocks HX and HP follow X and P through the same small products: every 16 iterations they are recomputed
+            // from the operator so that their rounding errors do not accumulate into the Ritz values
+            block_apply(X, HX, b);
+            if (np_cols > 0) block_apply(Pn, HPn, np_cols);
+        }
+        while (nl_new < k && resid[nl_new] <= tol) ++nl_new;
+        nl_new = std::min((nl_new / RD_EIG_CB) * RD_EIG_CB, b - RD_EIG_CB);
+        nl = std::max(nl, nl_new);
+        const int na = b - nl;
+        double* Wb = S + nb;
+        double* HW = HS + nb;
+        double* Pb = Wb + (size_t)na * ld;
+        double* HP = HW + (size_t)na * ld;
+        RDTRY(copy_cols(Wb, Xn + (size_t)nl * ld, na));
+        phase(0);
+        RDTRY(precondition(Wb, na));
+        phase(1);
+        block_apply(Wb, HW, na);
+        phase(2);
+        // P: the trailing min(na, np_cols) columns of the last P'
+        const int npc = std::min(na, np_cols);
+        RDTRY(copy_cols(Pb, Pn + (size_t)(np_cols - npc) * ld, npc));
+        RDTRY(copy_cols(HP, HPn + (size_t)(np_cols - npc) * ld, npc));
+        const int ns = b + na + npc;
+        gram(ns, S, S, Gs);
+        gram(ns, S, HS, Gh);
+        phase(3);
+        RDTRY(small_rr(ns));
+        phase(4);
+        // P' = [W, P] C[b:, :],  X' = X C[:b, :] + P'  (all b columns; the next iteration uses the trailing na columns of P');
+        // the same combinations of the H blocks
+        tall_mult(Wb, ns - b, Cm + b, ns, nullptr, Pn, b);
+        tall_mult(HW, ns - b, Cm + b, ns, nullptr, HPn, b);
+        tall_mult(X, b, Cm, ns, Pn, Xn, b);
+        tall_mult(HX, b, Cm, ns, HPn, HXn, b);
+        np_cols = b;
+        RDTRY(copy_cols(X, Xn, b));
+        RDTRY(copy_cols(HX, HXn, b));
+        CU(cudaGetLastError());
+        phase(5);
+    }
+    CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    // W <- the k lowest Ritz vectors (pad columns zero)
+    RDTRY(alloc_reference(ctx, k));
+    CU(cudaMemsetAsync(ctx->W, 0, (size_t)ld * ctx->kp * sizeof(double), ctx->stream));
+    CU(cudaMemcpyAsync(ctx->W, X, (size_t)ld * k * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    float loop_ms = 0.0f;
+    CU(cudaEventElapsedTime(&loop_ms, ctx->ev[0], ctx->ev[1]));
+    ctx->have_ref = true;
+    ctx->ref_kind = 0;
+    if (theta_out) memcpy(theta_out, theta.data(), k * sizeof(double));
+    if (resid_out) memcpy(resid_out, resid.data(), k * sizeof(double));
+    if (iters_out) *iters_out = iters;
+    ctx->ref_degree = iters;
+    ctx->ref_block = b;
+    ctx->ref_col_applies = 0;  // the Chebyshev filter's counters: not this solver's
+    ctx->ref_filter_ms = 0.0;
+    ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+    ctx->ref_ms_last = ctx->ref_ms_pending;
+    (void)prec_applies;
+    (void)col_applies;
+    (void)loop_ms;
+    if (status != RD_OK) fail(ctx, status, "reference not converged to tol %g in %d LOBPCG iterations (worst residual %g)", tol, iters,
+                              *std::max_element(resid.begin(), resid.begin() + k));
+    return status;
 }

@@ -140,3 +140,52 @@ def test_fullsize_reference_build_config2(oracle_mod):
         assert np.linalg.norm(rj) <= 2e-5 * theta[j]
     assert np.abs(W.T @ W - np.eye(w.k)).max() <= 1e-10
     g.close()
+
+
+def test_fullsize_lobpcg_reference_config2(oracle_mod):
+    """The second eigensolver of S0 (rd_build_reference_lobpcg) at full size: 512 x 512, k = 32, against the library
+    eigensolver of the oracle, as for the filter-based one above."""
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_17971_b200 as pkg
+
+    w = make_config(2)
+    g = pkg.RefDef.from_workload(w)
+    theta, resid, iters, st = g.build_reference_lobpcg(w.k, w.dims, kappa_ref=1.0, tol=1e-5, max_iters=3000)
+    assert st == 0 and resid.max() <= 1e-5, (st, iters, resid.max())
+    th_ref, _ = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+    assert np.abs(theta / th_ref - 1.0).max() <= 1e-8
+    W = g.get_reference()
+    o = oracle_mod.Oracle.from_workload(w, threaded=True)
+    for j in (0, w.k // 2, w.k - 1):
+        rj = o.apply_H(W[:, j]) - theta[j] * W[:, j]
+        assert np.linalg.norm(rj) <= 2e-5 * theta[j]
+    assert np.abs(W.T @ W - np.eye(w.k)).max() <= 1e-9
+    g.close()
+
+
+def test_fullsize_lobpcg_reference_config3_agrees_with_the_filter(oracle_mod):
+    """96^3, k = 48 (the library eigensolver of the oracle does not fit a test at this size): the two eigensolvers of the
+    library, which share only the block apply of H, agree on the eigenvalues, and the LOBPCG vectors have small
+    residuals against the ORACLE's operator."""
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2606_17971_b200 as pkg
+
+    w = make_config(3)
+    g = pkg.RefDef.from_workload(w)
+    th_f, res_f, _, st_f = g.build_reference(w.k, tol=1e-4, max_block_iters=200)
+    th_l, res_l, iters, st_l = g.build_reference_lobpcg(w.k, w.dims, kappa_ref=1.0, tol=1e-4, max_iters=1000)
+    assert st_f == 0 and st_l == 0, (st_f, st_l, iters)
+    assert np.abs(th_l / th_f - 1.0).max() <= 1e-6, np.abs(th_l / th_f - 1.0).max()
+    W = g.get_reference()
+    o = oracle_mod.Oracle.from_workload(w, threaded=True)
+    for j in (0, w.k // 2, w.k - 1):
+        rj = o.apply_H(W[:, j]) - th_l[j] * W[:, j]
+        assert np.linalg.norm(rj) <= 2e-4 * th_l[j]
+    assert np.abs(W.T @ W - np.eye(w.k)).max() <= 1e-9
+    g.close()

@@ -105,9 +105,10 @@ def test_reference_work_accounting_and_tensor_probe(rd):
         info = g.reference_info()
         nnz = len(w.val)
         assert info["filter_bytes_per_column_apply"] == 3 * nnz + 48 * w.N
-        # every sweep filters at most `block` columns with that sweep's degree; locked columns drop out
-        assert 0 < info["filter_column_applies"] <= info["block"] * info["total_degree"]
-        assert info["filter_column_applies"] >= info["total_degree"]
+        # every sweep applies H to at most `block` columns per degree of its filter (locked columns drop out), and once
+        # more to the whole block for the Rayleigh-Ritz step
+        assert 0 < info["filter_column_applies"] <= info["block"] * (info["total_degree"] + sweeps)
+        assert info["filter_column_applies"] >= info["total_degree"] + info["block"] * sweeps
         assert 0 < info["filter_ms"] <= info["build_ms"]
         assert info["filter_GBs"] > 0
         # an analytical reference resets the counters
