@@ -37,7 +37,7 @@ struct GemmOp {
 };
 
 template <bool AM, bool BN, int TN>
-__global__ void __launch_bounds__(256) k_dgemm_dmma(int M, int Nn, int Kk, int nb2, GemmOp A, GemmOp B, GemmOp E, GemmOp D)
+__global__ void __launch_bounds__(256, 2) k_dgemm_dmma(int M, int Nn, int Kk, int nb2, GemmOp A, GemmOp B, GemmOp E, GemmOp D)
 {
     constexpr int TNC = 8 * TN;                  // n columns per CTA
     constexpr int LDA_M = 64 + 4, LDA_K = 32 + 4;
@@ -54,35 +54,46 @@ __global__ void __launch_bounds__(256) k_dgemm_dmma(int M, int Nn, int Kk, int n
 #pragma unroll
     for (int t = 0; t < TN; ++t) acc[t][0] = acc[t][1] = 0.0;
     const bool live = (m0 + warp * 8) < M;
+    // Register-staged pipeline: the global loads of chunk c + 1 are issued before the tensor-core work on chunk c and land in
+    // shared memory after it, so their latency overlaps the DMMAs of this CTA as well as those of the other resident CTAs.
+    constexpr int NA = (64 * 32) / 256, NB = (TNC * 32) / 256;
+    double ra[NA], rb[NB];
+    auto fetch = [&](int k0) {
+#pragma unroll
+        for (int u = 0; u < NA; ++u) {
+            const int e = threadIdx.x + u * 256;
+            const int mm = AM ? (e & 63) : (e >> 5), kk = AM ? (e >> 6) : (e & 31);
+            const int gm = m0 + mm, gk = k0 + kk;
+            ra[u] = (gm < M && gk < Kk) ? ldg_f64(Ap + (int64_t)gm * A.s0 + (int64_t)gk * A.s1) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int e = threadIdx.x + u * 256;
+            const int kk = BN ? (e / TNC) : (e & 31), nn = BN ? (e - (e / TNC) * TNC) : (e >> 5);
+            const int gn = n0 + nn, gk = k0 + kk;
+            rb[u] = (gn < Nn && gk < Kk) ? ldg_f64(Bp + (int64_t)gk * B.s0 + (int64_t)gn * B.s1) : 0.0;
+        }
+    };
+    auto stage = [&]() {
+#pragma unroll
+        for (int u = 0; u < NA; ++u) {
+            const int e = threadIdx.x + u * 256;
+            if (AM) sA[(e >> 6) * LDA_M + (e & 63)] = ra[u];   // sA[k][m], lanes along m
+            else sA[(e >> 5) * LDA_K + (e & 31)] = ra[u];      // sA[m][k], lanes along k
+        }
+#pragma unroll
+        for (int u = 0; u < NB; ++u) {
+            const int e = threadIdx.x + u * 256;
+            if (BN) sB[(e / TNC) * LDB_N + (e - (e / TNC) * TNC)] = rb[u];  // sB[k][n], lanes along n
+            else sB[(e >> 5) * LDB_K + (e & 31)] = rb[u];                   // sB[n][k], lanes along k
+        }
+    };
+    fetch(0);
     for (int k0 = 0; k0 < Kk; k0 += 32) {
+        __syncthreads();  // every warp is done with the previous chunk
+        stage();
         __syncthreads();
-        if (AM) {  // sA[k][m], lanes along m
-            for (int e = threadIdx.x; e < 32 * 64; e += 256) {
-                const int kk = e >> 6, mm = e & 63;
-                const int gm = m0 + mm, gk = k0 + kk;
-                sA[kk * LDA_M + mm] = (gm < M && gk < Kk) ? ldg_f64(Ap + (int64_t)gm * A.s0 + (int64_t)gk * A.s1) : 0.0;
-            }
-        } else {  // sA[m][k], lanes along k
-            for (int e = threadIdx.x; e < 64 * 32; e += 256) {
-                const int mm = e >> 5, kk = e & 31;
-                const int gm = m0 + mm, gk = k0 + kk;
-                sA[mm * LDA_K + kk] = (gm < M && gk < Kk) ? ldg_f64(Ap + (int64_t)gm * A.s0 + (int64_t)gk * A.s1) : 0.0;
-            }
-        }
-        if (BN) {  // sB[k][n], lanes along n
-            for (int e = threadIdx.x; e < 32 * TNC; e += 256) {
-                const int kk = e / TNC, nn = e - kk * TNC;
-                const int gn = n0 + nn, gk = k0 + kk;
-                sB[kk * LDB_N + nn] = (gn < Nn && gk < Kk) ? ldg_f64(Bp + (int64_t)gk * B.s0 + (int64_t)gn * B.s1) : 0.0;
-            }
-        } else {  // sB[n][k], lanes along k
-            for (int e = threadIdx.x; e < TNC * 32; e += 256) {
-                const int nn = e >> 5, kk = e & 31;
-                const int gn = n0 + nn, gk = k0 + kk;
-                sB[nn * LDB_K + kk] = (gn < Nn && gk < Kk) ? ldg_f64(Bp + (int64_t)gk * B.s0 + (int64_t)gn * B.s1) : 0.0;
-            }
-        }
-        __syncthreads();
+        if (k0 + 32 < Kk) fetch(k0 + 32);
         if (live) {
 #pragma unroll
             for (int kk = 0; kk < 32; kk += 4) {
