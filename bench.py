@@ -623,6 +623,12 @@ def run_setup(args):
     else:
         build_analytical_reference(g, w)
         ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
+    if "lobpcg_TFLOPs" in ref:
+        # S0 by LOBPCG is bound by the FP64 tensor pipe: its roofline entry is flop over the iteration loop's time against the
+        # probe's peak (the same probe the Gram kernels of S2 are quoted against)
+        ref["roofline"] = {"bound": "tensor", "achieved": round(ref["lobpcg_TFLOPs"], 2), "peak": round(peak_tf, 2), "unit": "TFLOP/s",
+                           "frac": round(ref["lobpcg_TFLOPs"] / peak_tf, 3), "peak_source": "rd_probe_fp64_tensor_peak (m8n8k4 on registers)",
+                           "note": "whole iteration loop, incl. the block applies of H (HBM-bound) and the ns x ns Rayleigh-Ritz (latency-bound)"}
     act = torch.zeros(w.N, dtype=torch.uint8, device=dev)
     ms = []
     info = None

@@ -192,6 +192,12 @@ int rd_build_reference_scaled(rd_ctx* ctx, int32_t k, double tol, int32_t max_bl
  * used.  The result is checked with a freshly applied H before RD_OK is returned.  3 (k + guard) <= 256 and <= N. */
 int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int32_t max_iters, int32_t ndim, const int64_t* dims,
                               double kappa_ref, double* theta_out, double* resid_out, int32_t* iters_out);
+/* Work of the last rd_build_reference_lobpcg (zeros otherwise): tensor_flop = FP64 flop issued to the tensor cores
+ * (sine transforms 4 sum(dims) N per column apply of T, the upper tiles of the two Gram products, the tall products),
+ * loop_ms = CUDA-event time of the iteration loop, and the numbers of column applies of H and of T.  tensor_flop /
+ * loop_ms against rd_probe_fp64_tensor_peak is the solver's share of the FP64 tensor peak.  Any pointer may be NULL. */
+int rd_reference_lobpcg_work(const rd_ctx* ctx, double* tensor_flop, double* loop_ms, int64_t* h_column_applies,
+                             int64_t* t_column_applies);
 /* The analytical Cartesian spatial reference of the paper (section 2.2.3, eq. (15)) for steady
  * problems on a Cartesian grid of dims[0] x ... x dims[ndim-1] cells (ndim <= 3, x = dims[0] fastest, product = N,
  * else RD_EINVAL): the k lowest products of the 1-D sine modes of the constant-coefficient Dirichlet Laplacian,

@@ -22,7 +22,7 @@ STATUS_NAMES = {0: "ok", -1: "einval", -2: "enomem", -3: "ecuda", -4: "enoref", 
 SOFT = (-5, -6, -7, -8, -9)
 
 EXPORTS = ["rd_default_options", "rd_create", "rd_destroy", "rd_last_error", "rd_kernel_launches", "rd_set_options",
-           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_lobpcg", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
+           "rd_build_reference", "rd_build_reference_scaled", "rd_build_reference_lobpcg", "rd_reference_lobpcg_work", "rd_build_reference_sine", "rd_build_reference_spacetime", "rd_build_reference_spacetime_cover", "rd_reference_storage", "rd_build_reference_prolonged", "rd_build_reference_transient", "rd_reference_info", "rd_reference_work", "rd_probe_fp64_tensor_peak", "rd_set_reference", "rd_get_reference", "rd_solve_query", "rd_reset_sequence",
            "rd_apply_K", "rd_apply_KT", "rd_apply_H", "rd_apply_H_noalloc", "rd_diag_H", "rd_solve_inactive", "rd_coarse_setup", "rd_energy_fraction", "rd_kkt", "rd_pdas_update"]
 
 
@@ -105,6 +105,7 @@ def load_library(path: Optional[str] = None):
     lib.rd_set_options.argtypes = [vp, C.POINTER(_Options)]
     lib.rd_build_reference.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_scaled.argtypes = [vp, i32, dbl, i32, vp, vp, C.POINTER(i32)]
+    lib.rd_reference_lobpcg_work.argtypes = [vp, vp, vp, vp, vp]
     lib.rd_build_reference_lobpcg.argtypes = [vp, i32, dbl, i32, i32, vp, dbl, vp, vp, C.POINTER(i32)]
     lib.rd_build_reference_sine.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.rd_build_reference_spacetime.argtypes = [vp, i32, i32, vp, i32, dbl, vp, vp]
@@ -334,6 +335,14 @@ class RefDef:
         ca, fms, bpc = C.c_int64(0), C.c_double(0), C.c_double(0)
         self._check(self._lib.rd_reference_work(self._h, C.byref(ca), C.byref(fms), C.byref(bpc)), "rd_reference_work")
         d = dict(block=b.value, total_degree=deg.value, build_ms=ms.value)
+        fl, lms, ha, ta = C.c_double(0), C.c_double(0), C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.rd_reference_lobpcg_work(self._h, C.byref(fl), C.byref(lms), C.byref(ha), C.byref(ta)),
+                    "rd_reference_lobpcg_work")
+        if fl.value > 0 and lms.value > 0:
+            # S0 by LOBPCG: FP64 tensor-core flop of the whole iteration loop over its CUDA-event time
+            d.update(lobpcg_iterations=deg.value, lobpcg_tensor_flop=fl.value, lobpcg_loop_ms=lms.value,
+                     lobpcg_TFLOPs=fl.value / (lms.value * 1e-3) / 1e12, lobpcg_h_column_applies=ha.value,
+                     lobpcg_t_column_applies=ta.value)
         if ca.value > 0 and fms.value > 0:
             # S0's Chebyshev filter: algorithmic bytes (3 nnz + 48 N per column and degree) over its CUDA-event time
             d.update(filter_column_applies=ca.value, filter_ms=fms.value, filter_bytes_per_column_apply=bpc.value,

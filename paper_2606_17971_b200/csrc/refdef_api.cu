@@ -107,6 +107,10 @@ struct rd_ctx {
     int ref_block = 0;       // its block size b
     int64_t ref_col_applies = 0;  // sum over filter degrees of the columns H was applied to (locked columns excluded)
     double ref_filter_ms = 0.0;   // CUDA-event time of all filter applies of the last build
+    // work of the last rd_build_reference_lobpcg: FP64 tensor-core flop (sine transforms, Gram products, tall products),
+    // column applies of H and of the preconditioner, CUDA-event time of the iteration loop
+    double lob_flop = 0.0, lob_ms = 0.0;
+    int64_t lob_h_applies = 0, lob_t_applies = 0;
     int64_t launches = 0;  // kernels launched so far (rd_kernel_launches)
 };
 
@@ -847,6 +851,8 @@ int rd_build_reference_prolonged(rd_ctx* ctx, int32_t k, int32_t ndim, const int
     ctx->ref_kind = 0;
     ctx->ref_degree = 0;
     ctx->ref_col_applies = 0;
+    ctx->lob_flop = 0.0;
+    ctx->lob_ms = 0.0;
     ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
@@ -1078,6 +1084,8 @@ int rd_build_reference(rd_ctx* ctx, int32_t k, double tol, int32_t max_block_ite
     ctx->ref_degree = total_degree;
     ctx->ref_block = b;
     ctx->ref_col_applies = col_applies;
+    ctx->lob_flop = 0.0;
+    ctx->lob_ms = 0.0;
     ctx->ref_filter_ms = filter_ms;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
@@ -1135,6 +1143,8 @@ int rd_build_reference_sine(rd_ctx* ctx, int32_t k, int32_t ndim, const int64_t*
     ctx->ref_kind = 0;
     ctx->ref_degree = 0;
     ctx->ref_col_applies = 0;
+    ctx->lob_flop = 0.0;
+    ctx->lob_ms = 0.0;
     ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
@@ -1239,6 +1249,8 @@ static int build_spacetime(rd_ctx* ctx, int32_t k, int32_t pool, int32_t ndim, c
     RDTRY(store_kron(ctx, k, Ns, nt, rs_used, d_Phi, cols, d_sel, d_Q, /*normalise=*/0, nullptr));
     ctx->ref_degree = 0;
     ctx->ref_col_applies = 0;
+    ctx->lob_flop = 0.0;
+    ctx->lob_ms = 0.0;
     ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
@@ -1363,6 +1375,8 @@ int rd_build_reference_transient(rd_ctx* ctx, int32_t k, int32_t rs, int32_t nt,
     RDTRY(store_kron(ctx, k, Ns, nt, rs_used, d_used, cols, d_sel, d_Q, /*normalise=*/1, d_phin2));
     ctx->ref_degree = 0;
     ctx->ref_col_applies = 0;
+    ctx->lob_flop = 0.0;
+    ctx->lob_ms = 0.0;
     ctx->ref_filter_ms = 0.0;
     ctx->ref_block = k;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
@@ -1957,6 +1971,9 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
     const int gs = grid_for(ctx->K.nslices * 32, kThreads, big_grid(ctx));
     int64_t col_applies = 0;
     int64_t prec_applies = 0;
+    double tensor_flop = 0.0;  // m8n8k4 work as issued: products of the logical sizes (tile padding not counted)
+    double sum_dims = 0.0;
+    for (int a = 0; a < ndim; ++a) sum_dims += (double)dims[a];
 
     auto block_apply = [&](const double* Y, double* HY, int nc) {  // HY = H Y for nc columns (a multiple of 8); tmp holds M^{-1} K Y
         const int nch = nc / RD_EIG_CB;
@@ -1982,6 +1999,7 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
         }
         // 2 ndim passes: the result is back in Y
         prec_applies += nc;
+        tensor_flop += 4.0 * sum_dims * (double)N * nc;  // forward and inverse transform: 2 n_a flop per entry, axis and direction
         return RD_OK;
     };
     auto gram = [&](int p, const double* A, const double* B, double* out) {  // out (p x p) = A^T B
@@ -1990,12 +2008,17 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
         k_reduce_parts<<<grid_for((int64_t)p * p, kThreads, 64), kThreads, 0, ctx->stream>>>(nparts, (int64_t)p * p, parts, out);
         k_mirror_upper_tiles<<<grid_for((int64_t)p * p, kThreads, 64), kThreads, 0, ctx->stream>>>(p, out);
         ctx->launches += 3;
+        {
+            const double nt = (double)((p + 63) / 64);
+            tensor_flop += 2.0 * (double)N * 64.0 * 64.0 * (nt * (nt + 1.0) / 2.0);  // the upper 64 x 64 tiles
+        }
     };
     // Out (N x nout) = A[:, 0:kk] Cs (kk x nout, column-major with leading dimension ldc) (+ Add)
     auto tall_mult = [&](const double* A, int kk, const double* Cs, int ldc, const double* Add, double* Out, int nout) {
         const GemmOp a{A, 1, ld, 0, 0}, c{Cs, 1, ldc, 0, 0}, e{Add, 1, ld, 0, 0}, d{Out, 1, ld, 0, 0};
         launch_gemm<true, false>(ctx->stream, 10, (int)N, nout, kk, 1, 1, a, c, e, d);
         ctx->launches++;
+        tensor_flop += 2.0 * (double)N * kk * nout;
     };
     auto copy_cols = [&](double* dst, const double* src, int nc) -> int {
         if (nc > 0) CU(cudaMemcpyAsync(dst, src, (size_t)nc * ld * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
@@ -2173,10 +2196,22 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
     ctx->ref_filter_ms = 0.0;
     ctx->ref_ms_pending = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
     ctx->ref_ms_last = ctx->ref_ms_pending;
-    (void)prec_applies;
-    (void)col_applies;
-    (void)loop_ms;
+    ctx->lob_flop = tensor_flop;
+    ctx->lob_ms = loop_ms;
+    ctx->lob_h_applies = col_applies;
+    ctx->lob_t_applies = prec_applies;
     if (status != RD_OK) fail(ctx, status, "reference not converged to tol %g in %d LOBPCG iterations (worst residual %g)", tol, iters,
                               *std::max_element(resid.begin(), resid.begin() + k));
     return status;
+}
+
+extern "C" int rd_reference_lobpcg_work(const rd_ctx* ctx, double* tensor_flop, double* loop_ms, int64_t* h_column_applies,
+                                        int64_t* t_column_applies)
+{
+    if (!ctx) return RD_EINVAL;
+    if (tensor_flop) *tensor_flop = ctx->lob_flop;
+    if (loop_ms) *loop_ms = ctx->lob_ms;
+    if (h_column_applies) *h_column_applies = ctx->lob_h_applies;
+    if (t_column_applies) *t_column_applies = ctx->lob_t_applies;
+    return RD_OK;
 }

@@ -126,3 +126,25 @@ def test_lobpcg_reference_edge_cases(rd, oracle_mod):
                 g.build_reference_lobpcg(kw["k"], kw["dims"], kappa_ref=kw["kappa_ref"], tol=kw["tol"])
     finally:
         g.close()
+
+
+def test_lobpcg_work_accounting(rd):
+    """rd_reference_lobpcg_work: zeros before / after another construction, a flop count that matches the iteration count."""
+    w = make_config(twin="c3_16")
+    g = rd.RefDef.from_workload(w)
+    try:
+        assert "lobpcg_TFLOPs" not in g.reference_info()
+        theta, resid, iters, st = g.build_reference_lobpcg(w.k, w.dims, tol=1e-4)
+        assert st == 0
+        info = g.reference_info()
+        b = info["block"]
+        assert info["lobpcg_iterations"] == iters and info["lobpcg_loop_ms"] > 0
+        # every iteration preconditions and applies H to at most b columns, at least 8; the start adds b applies of each
+        assert 8 * iters <= info["lobpcg_t_column_applies"] - b <= b * iters
+        assert info["lobpcg_h_column_applies"] >= info["lobpcg_t_column_applies"]
+        # lower bound of the tensor work: the sine transforms alone
+        assert info["lobpcg_tensor_flop"] >= 4.0 * sum(w.dims) * w.N * info["lobpcg_t_column_applies"]
+        g.build_reference_sine(w.k, list(w.dims))
+        assert "lobpcg_TFLOPs" not in g.reference_info()
+    finally:
+        g.close()
