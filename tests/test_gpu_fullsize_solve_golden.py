@@ -1,0 +1,61 @@
+"""Complete Algorithm-1 solves at BASELINE.json's full sizes against stored oracle results
+(tests/golden/fullsize_solve_c<config>.json, written by tests/golden/make_golden_fullsize_solve.py from the oracle only).
+
+The live oracle needs minutes per solve at these sizes, so the other full-size tests compare capped loops; here the
+whole solve of one realistic inactive system per configuration (J = {y_d > psi} of query 0, direct restriction of the
+analytical sine reference, eps = 1e-8) is compared: status, retained rank, the iteration count (within 5 %: the two
+sides sum in different orders, and a count of thousands moves by a few iterations), the M-norm of the solution and the
+solution itself at 4096 stored sample positions (relative M-norm of the difference over the sample <= 1e-6, the bar of
+the complete-query tests)."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.mark.parametrize("config", [2, 3, 5])
+def test_fullsize_complete_solve_matches_oracle_golden(config):
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    path = os.path.join(HERE, "golden", f"fullsize_solve_c{config}.json")
+    if not os.path.exists(path):
+        pytest.skip(f"{os.path.basename(path)} not generated")
+    with open(path) as f:
+        gold = json.load(f)
+    import paper_2606_17971_b200 as pkg
+
+    w = make_config(config)
+    assert w.operator_hash() == gold["operator_sha256"] and w.N == gold["N"] and w.k == gold["k"]
+    yd, psi = w.target(0)
+    J = yd > psi
+    idx = np.flatnonzero(~J)
+    assert int(J.sum()) == gold["n_active"] and len(idx) == gold["n_inactive"]
+    g = pkg.RefDef.from_workload(w, pkg.Options(pdas_cap=w.pdas_cap, eps=gold["eps"], eps_c=gold["eps_c"]))
+    try:
+        g.build_reference_sine(w.k, list(w.dims))
+        act = J.astype(np.uint8)
+        b = np.where(J, 0.0, w.m * yd - g.apply_H(np.where(J, psi, 0.0)))
+        assert abs(np.linalg.norm(b[idx]) / gold["b_norm"] - 1.0) <= 1e-12
+        x, rep = g.solve_inactive(pkg.REFDEF, act, b, np.zeros(w.N))
+    finally:
+        g.close()
+    assert rep["status"] == gold["status"] == 0
+    assert rep["rank_used"] == gold["rank_used"]
+    assert rep["rel_resid_verified"] <= gold["eps"]
+    assert abs(rep["iters"] - gold["iters"]) <= 0.05 * gold["iters"], (rep["iters"], gold["iters"])
+    assert (x[J] == 0).all()
+    xI, mI = x[idx], w.m[idx]
+    assert abs(np.sqrt((mI * xI * xI).sum()) / gold["x_Mnorm"] - 1.0) <= 1e-6
+    pos = np.array(gold["sample_positions_in_I"])
+    xs = np.array(gold["x_samples"])
+    num = np.sqrt((mI[pos] * (xI[pos] - xs) ** 2).sum())
+    den = np.sqrt((mI[pos] * xs ** 2).sum())
+    assert num <= 1e-6 * den, (num / den, rep["iters"], gold["iters"])
