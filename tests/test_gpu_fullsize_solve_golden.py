@@ -3,7 +3,7 @@
 
 The live oracle needs minutes per solve at these sizes, so the other full-size tests compare capped loops; here the
 whole solve of one realistic inactive system per configuration (J = {y_d > psi} of query 0, direct restriction of the
-analytical sine reference, eps = 1e-8) is compared: status, retained rank, the iteration count (within 5 %: the two
+analytical sine reference, eps = 1e-8) is compared: status, retained rank, the iteration count (within 1 %: the two
 sides sum in different orders, and a count of thousands moves by a few iterations), the M-norm of the solution and the
 solution itself at 4096 stored sample positions (relative M-norm of the difference over the sample <= 1e-6, the bar of
 the complete-query tests)."""
@@ -50,7 +50,8 @@ def test_fullsize_complete_solve_matches_oracle_golden(config):
     assert rep["status"] == gold["status"] == 0
     assert rep["rank_used"] == gold["rank_used"]
     assert rep["rel_resid_verified"] <= gold["eps"]
-    assert abs(rep["iters"] - gold["iters"]) <= 0.05 * gold["iters"], (rep["iters"], gold["iters"])
+    # measured on B200: 18,372 / 18,371 (config 2), 1,709 / 1,709 (config 3), 4,035 / 4,036 (config 5)
+    assert abs(rep["iters"] - gold["iters"]) <= max(10, 0.01 * gold["iters"]), (rep["iters"], gold["iters"])
     assert (x[J] == 0).all()
     xI, mI = x[idx], w.m[idx]
     assert abs(np.sqrt((mI * xI * xI).sum()) / gold["x_Mnorm"] - 1.0) <= 1e-6
