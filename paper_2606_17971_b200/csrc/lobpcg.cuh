@@ -327,11 +327,11 @@ __global__ void __launch_bounds__(1024) k_rr_select(int ns, const double* A0, co
 // Step 2, fast path (one CTA): Cholesky of the scaled Gram, A0 = L L^T; Tm = D^{-1/2} L^{-T}, all ns directions kept.
 // info[2] = 1 on success; a pivot below 1e-10 (a basis that is dependent to working accuracy) leaves info[2] = 0 and the
 // eigenvalue path (k_jacobi_grid + k_rr_select) runs instead.  Linv: ns x ns scratch.
-__global__ void __launch_bounds__(1024) k_rr_chol(int ns, double* A0, const double* dsc, double* Linv, double* Tm, int* info)
+__global__ void __launch_bounds__(1024) k_rr_chol(int ns, double* A0, const double* dsc, double* Linv, double* Tm, int* info, int force_fallback)
 {
     __shared__ DenseShared ds;
     __shared__ int s_ok;
-    const bool ok = cta_cholesky(A0, ns, ns, ds);
+    const bool ok = !force_fallback && cta_cholesky(A0, ns, ns, ds);
     if (threadIdx.x == 0) {
         int good = ok ? 1 : 0;
         for (int j = 0; j < ns && good; ++j)

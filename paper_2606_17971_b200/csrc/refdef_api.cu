@@ -2026,6 +2026,7 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
     };
     double* X = S;
     double* HX = HS;
+    const bool no_chol = std::getenv("RD_LOBPCG_NO_CHOL") != nullptr;  // tests: take the eigenvalue whitening on every iteration
     // the ns x ns part: two grid-parallel Jacobi eigensolves and the small products between them (lobpcg.cuh)
     auto small_rr = [&](int ns) -> int {
         const size_t nn = (size_t)ns_max * ns_max;
@@ -2037,7 +2038,7 @@ extern "C" int rd_build_reference_lobpcg(rd_ctx* ctx, int32_t k, double tol, int
         const int gsm = grid_for((int64_t)ns * ns, kThreads, 256);
         k_rr_scale<<<gsm, kThreads, 0, ctx->stream>>>(ns, Gs, Gh, dsc, A0, GhS);
         CU(cudaMemcpyAsync(A1, A0, (size_t)ns * ns * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));  // the Cholesky works on a copy
-        k_rr_chol<<<1, 1024, 0, ctx->stream>>>(ns, A1, dsc, Q, Tm, info);
+        k_rr_chol<<<1, 1024, 0, ctx->stream>>>(ns, A1, dsc, Q, Tm, info, no_chol ? 1 : 0);
         int n_arg = ns;
         const int* n_ptr = nullptr;
         const int* skip1 = info + 2;

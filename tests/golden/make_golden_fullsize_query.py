@@ -1,0 +1,57 @@
+"""Writes tests/golden/fullsize_query_c<config>.json / .npz from the CPU oracle ONLY (never from the CUDA path).
+
+Run:  python tests/golden/make_golden_fullsize_query.py [config ...]      (no arguments: 3; about an hour of 8-thread oracle time)
+
+One COMPLETE PDAS query (eq. (7)-(8), Algorithm 1 inside every step) at BASELINE.json's full size: query 0 of the sequence
+from the all-active start of PAPER.md:339, RefDef (direct restriction) with the paper's analytical sine reference
+(oracle.sine_reference, a deterministic closed form), at the paper's accuracy (verified relative residual
+1e-10, recurrence trigger 1e-11) so that the active-set decisions sit above the solver's noise, PDAS cap 400.
+Stored per step: FNV-1a hash of the packed active set, |I|, CG iterations, retained rank, status, margin (json); y at 65,536
+seeded sample positions with the M-norm of y and u over those positions (npz).  tests/test_gpu_fullsize_query_golden.py runs
+the same query through the C ABI and compares.  The oracle is the threaded build of the same source
+(oracle.Oracle(..., threaded=True)): sums are taken in another order, nothing else differs.
+"""
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+sys.path.insert(0, ROOT)
+
+import oracle  # noqa: E402
+from workloads import make_config  # noqa: E402
+
+EPS, EPS_C, PDAS_CAP, N_SAMPLES = 1e-10, 1e-11, 400, 65536
+
+
+def run(config):
+    w = make_config(config)
+    assert w.nt == 1
+    o = oracle.Oracle.from_workload(w, threaded=True)
+    W = np.asfortranarray(oracle.sine_reference(w.dims, w.k)[-1])
+    yd, psi = w.target(0)
+    t0 = time.time()
+    r = o.solve_query(oracle.REFDEF, yd, psi, W, oracle.OracleOptions(eps=EPS, eps_c=EPS_C, pdas_cap=PDAS_CAP))
+    dt = time.time() - t0
+    pos = np.sort(np.random.default_rng(777 + config).choice(w.N, size=min(N_SAMPLES, w.N), replace=False))
+    out = {"config": config, "workload": w.name, "N": w.N, "k": w.k, "operator_sha256": w.operator_hash(), "eps": EPS, "eps_c": EPS_C,
+           "pdas_cap": PDAS_CAP, "method": "refdef, analytical sine reference", "query": 0, "status": r["status"], "n_steps": r["n_steps"],
+           "kkt": [float(v) for v in r["kkt"]], "n_inactive": [s["n_inactive"] for s in r["steps"]],
+           "active_hash": [f"{s['active_hash']:016x}" for s in r["steps"]], "cg_iters": [s["cg_iters"] for s in r["steps"]],
+           "rank_used": [s["rank_used"] for s in r["steps"]], "inner_status": [s["status"] for s in r["steps"]],
+           "margin": [float(s["margin"]) for s in r["steps"]], "y_absmax": float(np.abs(r["y"]).max()),
+           "y_Mnorm": float(np.sqrt((w.m * r["y"] ** 2).sum())), "u_Mnorm": float(np.sqrt((w.m * r["u"] ** 2).sum())),
+           "oracle_seconds": round(dt, 1), "oracle_threads": o.threads}
+    with open(os.path.join(HERE, f"fullsize_query_c{config}.json"), "w") as f:
+        json.dump(out, f)
+    np.savez_compressed(os.path.join(HERE, f"fullsize_query_c{config}.npz"), pos=pos, y=r["y"][pos], u=r["u"][pos])
+    print("config", config, "status", r["status"], "steps", r["n_steps"], "iters", sum(out["cg_iters"]), f"{dt:.0f} s", flush=True)
+
+
+if __name__ == "__main__":
+    for c in ([int(a) for a in sys.argv[1:]] or [3]):
+        run(c)

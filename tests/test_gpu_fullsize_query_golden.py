@@ -1,0 +1,70 @@
+"""A COMPLETE PDAS query at BASELINE.json's full size against a stored oracle result
+(tests/golden/fullsize_query_c<config>.json / .npz, written by tests/golden/make_golden_fullsize_query.py from the oracle
+only; about an hour of 8-thread oracle time, hence stored): query 0 of config 3 (96^3, N = 884,736, k = 48) from the
+all-active start, RefDef with the analytical sine reference at the paper's accuracy (eps 1e-10, eps_c 1e-11).
+
+Compared: the whole active-set sequence (FNV-1a hash of the packed set and |I| at every PDAS step: bit-exact, with the
+near-tie rule of tests/test_gpu_twins_golden.py), status, retained rank and CG iterations per step (5 %), y and u = M^-1 K y
+at 65,536 stored sample positions to 1e-6 in the M-norm over the sample, their full M-norms, the KKT measures."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.mark.parametrize("config", [3])
+def test_fullsize_query_matches_oracle_golden(oracle_mod, config):
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    jpath, zpath = os.path.join(GOLD, f"fullsize_query_c{config}.json"), os.path.join(GOLD, f"fullsize_query_c{config}.npz")
+    if not (os.path.exists(jpath) and os.path.exists(zpath)):
+        pytest.skip(f"golden not generated (python tests/golden/make_golden_fullsize_query.py {config})")
+    import paper_2606_17971_b200 as pkg
+
+    gold = json.load(open(jpath))
+    z = np.load(zpath)
+    pos, y_o, u_o = z["pos"], z["y"], z["u"]
+    w = make_config(config)
+    assert w.operator_hash() == gold["operator_sha256"] and w.N == gold["N"] and w.k == gold["k"]
+    assert gold["status"] == 0 and max(gold["kkt"]) <= 1e-8
+    g = pkg.RefDef.from_workload(w, pkg.Options(eps=gold["eps"], eps_c=gold["eps_c"], pdas_cap=gold["pdas_cap"]))
+    try:
+        g.build_reference_sine(w.k, list(w.dims))
+        yd, psi = w.target(gold["query"])
+        r = g.solve_query(pkg.REFDEF, yd, psi, want_sets=False)
+    finally:
+        g.close()
+    assert r["status"] == 0 and r["worst_inner_status"] == 0 and max(r["kkt"]) <= 1e-8
+    mp = w.m[pos]
+    snrm = lambda v: float(np.sqrt((mp * v * v).sum()))
+    nrm = lambda v: float(np.sqrt((w.m * v * v).sum()))
+    hashes = [f"{h:016x}" for h in r["hashes"]]
+    n_in = [s["n_inactive"] for s in r["steps"]]
+    same = hashes == gold["active_hash"]
+    if not same:
+        first = next(i for i, (a, b) in enumerate(zip(hashes, gold["active_hash"])) if a != b)
+        noise = 10.0 * gold["eps"] * gold["y_absmax"]
+        assert gold["margin"][first - 1] <= noise, (
+            f"active sets differ first at step {first} of {gold['n_steps']} (|I| {n_in[first]} vs {gold['n_inactive'][first]}); "
+            f"oracle margin {gold['margin'][first - 1]:.2e} is not a near-tie (noise level {noise:.1e})")
+    else:
+        assert r["n_steps"] == gold["n_steps"] and n_in == gold["n_inactive"]
+        for s, it_o, rk_o in zip(r["steps"], gold["cg_iters"], gold["rank_used"]):
+            assert s["rank_used"] <= rk_o
+            if s["rank_used"] == rk_o:
+                assert abs(s["cg_iters"] - it_o) <= max(4, 0.05 * it_o), (s["cg_iters"], it_o)
+        tot, tot_o = sum(s["cg_iters"] for s in r["steps"]), sum(gold["cg_iters"])
+        assert abs(tot - tot_o) <= 0.05 * tot_o
+    # the solution of the QP is unique: y, u at the stored positions and their full norms
+    assert snrm(r["y"][pos] - y_o) <= 1e-6 * snrm(y_o)
+    assert snrm(r["u"][pos] - u_o) <= 1e-6 * snrm(u_o)
+    assert abs(nrm(r["y"]) / gold["y_Mnorm"] - 1.0) <= 1e-6
+    assert abs(nrm(r["u"]) / gold["u_Mnorm"] - 1.0) <= 1e-6

@@ -148,3 +148,19 @@ def test_lobpcg_work_accounting(rd):
         assert "lobpcg_TFLOPs" not in g.reference_info()
     finally:
         g.close()
+
+
+def test_lobpcg_eigenvalue_whitening_path(rd, oracle_mod, monkeypatch):
+    """The fallback of the Rayleigh-Ritz step (eigen-decomposition of the Gram matrix with dropped directions instead of its
+    Cholesky factor) is what runs when the basis [X, W, P] is dependent to working accuracy; RD_LOBPCG_NO_CHOL takes it on
+    every iteration.  Same result."""
+    w = make_config(twin="c3_16")
+    monkeypatch.setenv("RD_LOBPCG_NO_CHOL", "1")
+    g = rd.RefDef.from_workload(w)
+    try:
+        theta, resid, iters, st = g.build_reference_lobpcg(w.k, w.dims, tol=1e-7, max_iters=400)
+        assert st == 0 and resid.max() <= 1e-7 and iters <= 250
+        th_o, _ = oracle_mod.reference_eigs(w.rowptr, w.colidx, w.val, w.m, w.alpha, w.k)
+        assert np.allclose(theta, th_o, rtol=1e-9)
+    finally:
+        g.close()
