@@ -18,15 +18,18 @@ pytestmark = pytest.mark.gpu
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
 
-@pytest.mark.parametrize("config", [3])
-def test_fullsize_query_matches_oracle_golden(oracle_mod, config):
+@pytest.mark.parametrize("config,tag", [(3, "c3"), (5, "c5_first3")])
+def test_fullsize_query_matches_oracle_golden(oracle_mod, config, tag):
+    """c3: the complete query 0 of config 3.  c5_first3: the first three PDAS steps of query 0 of config 5 (N = 4,096,000; the
+    complete query needs 95 steps of 12 minutes of oracle time each): both sides stop at the step cap with the same status,
+    the same active sets and the same iterate."""
     import torch
 
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
-    jpath, zpath = os.path.join(GOLD, f"fullsize_query_c{config}.json"), os.path.join(GOLD, f"fullsize_query_c{config}.npz")
+    jpath, zpath = os.path.join(GOLD, f"fullsize_query_{tag}.json"), os.path.join(GOLD, f"fullsize_query_{tag}.npz")
     if not (os.path.exists(jpath) and os.path.exists(zpath)):
-        pytest.skip(f"golden not generated (python tests/golden/make_golden_fullsize_query.py {config})")
+        pytest.skip(f"golden {tag} not generated (python tests/golden/make_golden_fullsize_query.py)")
     import paper_2606_17971_b200 as pkg
 
     gold = json.load(open(jpath))
@@ -34,7 +37,8 @@ def test_fullsize_query_matches_oracle_golden(oracle_mod, config):
     pos, y_o, u_o = z["pos"], z["y"], z["u"]
     w = make_config(config)
     assert w.operator_hash() == gold["operator_sha256"] and w.N == gold["N"] and w.k == gold["k"]
-    assert gold["status"] == 0 and max(gold["kkt"]) <= 1e-8
+    capped = bool(gold.get("first_steps_only"))
+    assert gold["status"] == (-7 if capped else 0) and (capped or max(gold["kkt"]) <= 1e-8)
     g = pkg.RefDef.from_workload(w, pkg.Options(eps=gold["eps"], eps_c=gold["eps_c"], pdas_cap=gold["pdas_cap"]))
     try:
         g.build_reference_sine(w.k, list(w.dims))
@@ -42,13 +46,15 @@ def test_fullsize_query_matches_oracle_golden(oracle_mod, config):
         r = g.solve_query(pkg.REFDEF, yd, psi, want_sets=False)
     finally:
         g.close()
-    assert r["status"] == 0 and r["worst_inner_status"] == 0 and max(r["kkt"]) <= 1e-8
+    assert r["status"] == gold["status"] and r["worst_inner_status"] == 0 and (capped or max(r["kkt"]) <= 1e-8)
     mp = w.m[pos]
     snrm = lambda v: float(np.sqrt((mp * v * v).sum()))
     nrm = lambda v: float(np.sqrt((w.m * v * v).sum()))
     hashes = [f"{h:016x}" for h in r["hashes"]]
     n_in = [s["n_inactive"] for s in r["steps"]]
     same = hashes == gold["active_hash"]
+    if capped:
+        assert same, "the first PDAS steps must take the same decisions (margins are far above the solver's noise there)"
     if not same:
         first = next(i for i, (a, b) in enumerate(zip(hashes, gold["active_hash"])) if a != b)
         noise = 10.0 * gold["eps"] * gold["y_absmax"]
@@ -63,7 +69,8 @@ def test_fullsize_query_matches_oracle_golden(oracle_mod, config):
                 assert abs(s["cg_iters"] - it_o) <= max(4, 0.05 * it_o), (s["cg_iters"], it_o)
         tot, tot_o = sum(s["cg_iters"] for s in r["steps"]), sum(gold["cg_iters"])
         assert abs(tot - tot_o) <= 0.05 * tot_o
-    # the solution of the QP is unique: y, u at the stored positions and their full norms
+    # the solution of the QP is unique (and so is the iterate after the same steps on the same sets): y, u at the stored
+    # positions and their full norms
     assert snrm(r["y"][pos] - y_o) <= 1e-6 * snrm(y_o)
     assert snrm(r["u"][pos] - u_o) <= 1e-6 * snrm(u_o)
     assert abs(nrm(r["y"]) / gold["y_Mnorm"] - 1.0) <= 1e-6
