@@ -180,7 +180,7 @@ def build_eig_reference(g, w, reference, ref_tol, sweeps=60):
     """The k lowest eigenvectors of H (BASELINE.json's reference) to ||H w - theta w|| <= ref_tol theta.
     Returns (theta, residuals, iterations or sweeps, status)."""
     if eig_solver_for(w, reference) == "lobpcg":
-        return g.build_reference_lobpcg(w.k, w.dims, kappa_ref=KAPPA_REF, tol=ref_tol, max_iters=600)
+        return g.build_reference_lobpcg(w.k, w.dims, kappa_ref=KAPPA_REF, tol=ref_tol, max_iters=800)
     return g.build_reference(w.k, tol=ref_tol, max_block_iters=sweeps)
 
 
@@ -619,7 +619,7 @@ def run_setup(args):
     if args.reference in ("eig", "eig-filter", "eig-lobpcg"):
         _, resid, sweeps, st = build_eig_reference(g, w, args.reference, args.ref_tol, args.ref_sweeps)
         ref = dict(g.reference_info(), sweeps=sweeps, status=st, worst_rel_residual=float(resid.max()),
-                   solver=eig_solver_for(w, args.reference))
+                   solver=eig_solver_for(w, args.reference), kappa_ref=KAPPA_REF)
     else:
         build_analytical_reference(g, w)
         ref = dict(g.reference_info(), kind="analytical (PAPER.md:186-208)")
@@ -871,6 +871,8 @@ def build_parser():
                          "steady Cartesian grids); sine: the paper's analytical "
                          "references (rd_build_reference_sine on the steady configs, rd_build_reference_spacetime on config 4); "
                          "coarse: Jacobi-scaled modes of the half-resolution operator, P1-prolonged (PAPER.md:176)")
+    ap.add_argument("--kappa-ref", type=float, default=None,
+                    help="conductivity of the homogeneous comparison medium of the LOBPCG preconditioner (default 1.0, the generator's solid)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="host-buffer queries after the timed region; 0 = one full pass of the sequence")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -884,6 +886,9 @@ def build_parser():
 
 def main(argv=None):
     args = build_parser().parse_args(argv)
+    if args.kappa_ref is not None:
+        global KAPPA_REF
+        KAPPA_REF = float(args.kappa_ref)
     if args.impl == "reference":
         out = run_reference(args)
     elif args.mode == "loop":

@@ -69,6 +69,9 @@ def test_fullsize_query_matches_oracle_golden(oracle_mod, config, tag):
                 assert abs(s["cg_iters"] - it_o) <= max(4, 0.05 * it_o), (s["cg_iters"], it_o)
         tot, tot_o = sum(s["cg_iters"] for s in r["steps"]), sum(gold["cg_iters"])
         assert abs(tot - tot_o) <= 0.05 * tot_o
+    print(f"\nfullsize query {tag}: steps GPU {r['n_steps']} / oracle {gold['n_steps']}, same active sets {same}, CG iterations GPU "
+          f"{sum(s_['cg_iters'] for s_ in r['steps'])} / oracle {sum(gold['cg_iters'])}, sampled relative M-norm of y - y_oracle "
+          f"{snrm(r['y'][pos] - y_o) / snrm(y_o):.2e}, of u - u_oracle {snrm(r['u'][pos] - u_o) / snrm(u_o):.2e}")  # shown with pytest -s
     # the solution of the QP is unique (and so is the iterate after the same steps on the same sets): y, u at the stored
     # positions and their full norms
     assert snrm(r["y"][pos] - y_o) <= 1e-6 * snrm(y_o)
